@@ -1,0 +1,216 @@
+"""CPU ORACLE -- TEST INFRASTRUCTURE, NOT A PRODUCT PATH.
+
+ctypes binding of ``oracle/cc_oracle.c`` (plain C, float64, naive DFTs): the
+slow, obviously-correct restatement of the displacement estimator of
+arxiv 2310.08770 (Eq. (4); Sec. III) that the
+CUDA library is checked against.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package.  It
+imports nothing from ``paper_2310_08770_b200`` and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cc_oracle.c")
+_HDR = os.path.join(_HERE, "cc_oracle.h")
+_LIB = os.path.join(_HERE, "libcc_oracle.so")
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile cc_oracle.c with gcc (-O2 -fopenmp) into oracle/libcc_oracle.so."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-Wall",
+               "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Result(ctypes.Structure):
+    _fields_ = [("dy", ctypes.c_double), ("dx", ctypes.c_double),
+                ("peak", ctypes.c_double),
+                ("wy", ctypes.c_int), ("wx", ctypes.c_int),
+                ("m", ctypes.c_int), ("n", ctypes.c_int),
+                ("cc_top1", ctypes.c_double), ("cc_top2", ctypes.c_double),
+                ("up_top1", ctypes.c_double), ("up_top2", ctypes.c_double)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.cco_dft2_real.argtypes = [dp, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.cco_dft2_literal.argtypes = [dp, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.cco_idft2.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.cco_cc_direct.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int, dp]
+        lib.cco_cc_dft.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int, dp, dp, dp]
+        lib.cco_argmax.argtypes = [dp, ctypes.c_long]
+        lib.cco_argmax.restype = ctypes.c_long
+        lib.cco_grid_size.argtypes = [ctypes.c_int]
+        lib.cco_upsampled.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                      ctypes.c_int, ctypes.c_int, dp, ip, ip, dp, dp]
+        lib.cco_upsampled_literal.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_int, ctypes.c_int, dp]
+        lib.cco_interp_at.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int,
+                                      ctypes.c_double, ctypes.c_double]
+        lib.cco_interp_at.restype = ctypes.c_double
+        lib.cco_track.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                  ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float),
+                                  ctypes.POINTER(_Result), ctypes.c_int]
+        lib.cco_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def dft2(img, literal: bool = False):
+    """O2: naive 2D DFT of a real image -> complex128 (H, W)."""
+    img = _f64(img)
+    H, W = img.shape
+    re, im = np.empty((H, W)), np.empty((H, W))
+    fn = _load().cco_dft2_literal if literal else _load().cco_dft2_real
+    if fn(_d(img), H, W, _d(re), _d(im)):
+        raise MemoryError("oracle dft2")
+    return re + 1j * im
+
+
+def idft2(P):
+    """O4: naive inverse 2D DFT (1/(HW) included) -> complex128 (H, W)."""
+    P = np.asarray(P, dtype=np.complex128)
+    H, W = P.shape
+    pr, pi = _f64(P.real), _f64(P.imag)
+    re, im = np.empty((H, W)), np.empty((H, W))
+    if _load().cco_idft2(_d(pr), _d(pi), H, W, _d(re), _d(im)):
+        raise MemoryError("oracle idft2")
+    return re + 1j * im
+
+
+def cc_direct(I, E):
+    """Left side of Eq. (4): brute-force circular cross-correlation."""
+    I, E = _f64(I), _f64(E)
+    H, W = I.shape
+    cc = np.empty((H, W))
+    _load().cco_cc_direct(_d(I), _d(E), H, W, _d(cc))
+    return cc
+
+
+def cc_dft(I, E):
+    """Right side of Eq. (4): returns (cc, P) with P = F[I] conj(F[E])."""
+    I, E = _f64(I), _f64(E)
+    H, W = I.shape
+    cc, pr, pi = np.empty((H, W)), np.empty((H, W)), np.empty((H, W))
+    if _load().cco_cc_dft(_d(I), _d(E), H, W, _d(cc), _d(pr), _d(pi)):
+        raise MemoryError("oracle cc_dft")
+    return cc, pr + 1j * pi
+
+
+def argmax(a) -> int:
+    a = _f64(a).ravel()
+    return int(_load().cco_argmax(_d(a), a.size))
+
+
+def grid_size(u: int) -> int:
+    return int(_load().cco_grid_size(int(u)))
+
+
+def upsampled(P, u: int, y0: int, x0: int, want_grid: bool = True, literal: bool = False):
+    """O6: upsampled CC around integer peak (y0, x0).
+
+    Returns dict(C, m, n, top1, top2); C is None when want_grid is False."""
+    P = np.asarray(P, dtype=np.complex128)
+    H, W = P.shape
+    pr, pi = _f64(P.real), _f64(P.imag)
+    M = grid_size(u)
+    lib = _load()
+    if literal:
+        C = np.empty((M, M))
+        if lib.cco_upsampled_literal(_d(pr), _d(pi), H, W, u, y0, x0, _d(C)):
+            raise MemoryError("oracle upsampled_literal")
+        i = argmax(C)
+        return dict(C=C, m=i // M, n=i % M, top1=float(C.ravel()[i]), top2=None)
+    C = np.empty((M, M)) if want_grid else None
+    m, n = ctypes.c_int(), ctypes.c_int()
+    t1, t2 = ctypes.c_double(), ctypes.c_double()
+    rc = lib.cco_upsampled(_d(pr), _d(pi), H, W, u, y0, x0,
+                           _d(C) if C is not None else None,
+                           ctypes.byref(m), ctypes.byref(n), ctypes.byref(t1), ctypes.byref(t2))
+    if rc:
+        raise MemoryError("oracle upsampled")
+    return dict(C=C, m=m.value, n=n.value, top1=t1.value, top2=t2.value)
+
+
+def interp_at(P, sy: float, sx: float) -> float:
+    P = np.asarray(P, dtype=np.complex128)
+    H, W = P.shape
+    pr, pi = _f64(P.real), _f64(P.imag)
+    return float(_load().cco_interp_at(_d(pr), _d(pi), H, W, float(sy), float(sx)))
+
+
+@dataclass
+class TrackResult:
+    dy: np.ndarray
+    dx: np.ndarray
+    peak: np.ndarray
+    wy: np.ndarray
+    wx: np.ndarray
+    m: np.ndarray
+    n: np.ndarray
+    cc_top1: np.ndarray
+    cc_top2: np.ndarray
+    up_top1: np.ndarray
+    up_top2: np.ndarray
+
+
+def num_threads() -> int:
+    return int(_load().cco_num_threads())
+
+
+def track(frames, reference, u: int, threads: int = 0) -> TrackResult:
+    """The whole path O1-O7 for a batch of uint8/uint16 frames (B, H, W)
+    against a float32 reference (H, W)."""
+    frames = np.ascontiguousarray(frames)
+    if frames.ndim == 2:
+        frames = frames[None]
+    if frames.dtype == np.uint8:
+        dt = 0
+    elif frames.dtype == np.uint16:
+        dt = 1
+    else:
+        raise TypeError("frames must be uint8 or uint16")
+    B, H, W = frames.shape
+    ref = np.ascontiguousarray(reference, dtype=np.float32)
+    if ref.shape != (H, W):
+        raise ValueError("reference shape mismatch")
+    out = (_Result * max(B, 1))()
+    rc = _load().cco_track(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                           ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), out, int(threads))
+    if rc:
+        raise RuntimeError("oracle cco_track failed: %d" % rc)
+    arr = np.frombuffer(out, dtype=np.dtype([
+        ("dy", "f8"), ("dx", "f8"), ("peak", "f8"), ("wy", "i4"), ("wx", "i4"),
+        ("m", "i4"), ("n", "i4"), ("cc_top1", "f8"), ("cc_top2", "f8"),
+        ("up_top1", "f8"), ("up_top2", "f8")], align=True))[:B]
+    return TrackResult(*(arr[k].copy() for k in
+                         ("dy", "dx", "peak", "wy", "wx", "m", "n",
+                          "cc_top1", "cc_top2", "up_top1", "up_top2")))

@@ -1,0 +1,413 @@
+/*
+ * cc_oracle.c -- CPU ORACLE (TEST INFRASTRUCTURE, NOT A PRODUCT PATH).
+ * See cc_oracle.h for the conventions and citations.  Plain C, double
+ * precision, naive DFTs (no FFT), no blocking / fusion / reordering beyond
+ * what the definitions state.  OpenMP is used only across frames (cco_track)
+ * and across independent output rows of a single upsampled grid.
+ */
+#include "cc_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+/* cos/sin(2*pi*j/N), j = 0..N-1 */
+static int unit_table(int N, double **c_out, double **s_out)
+{
+    double *c = (double *)malloc(sizeof(double) * (size_t)N);
+    double *s = (double *)malloc(sizeof(double) * (size_t)N);
+    if (!c || !s) { free(c); free(s); return -1; }
+    for (int j = 0; j < N; ++j) {
+        double a = 2.0 * M_PI * (double)j / (double)N;
+        c[j] = cos(a);
+        s[j] = sin(a);
+    }
+    *c_out = c; *s_out = s;
+    return 0;
+}
+
+/* One pass of a naive DFT along one axis of a complex H x W array.
+ * axis = 1: along x (rows), axis = 0: along y (columns).
+ * sign = -1 forward, +1 inverse (no scaling here). */
+static int dft_axis(const double *in_re, const double *in_im, int H, int W,
+                    int axis, int sign, double *out_re, double *out_im)
+{
+    int N = axis ? W : H;
+    double *c, *s;
+    if (unit_table(N, &c, &s)) return -1;
+    if (axis == 1) {
+        for (int y = 0; y < H; ++y) {
+            const double *xr = in_re + (size_t)y * W;
+            const double *xi = in_im ? in_im + (size_t)y * W : NULL;
+            for (int k = 0; k < W; ++k) {
+                double ar = 0.0, ai = 0.0;
+                int idx = 0;                       /* (k*n) mod N */
+                for (int n = 0; n < W; ++n) {
+                    double wr = c[idx], wi = sign * s[idx];
+                    double vr = xr[n], vi = xi ? xi[n] : 0.0;
+                    ar += vr * wr - vi * wi;
+                    ai += vr * wi + vi * wr;
+                    idx += k; if (idx >= N) idx -= N;
+                }
+                out_re[(size_t)y * W + k] = ar;
+                out_im[(size_t)y * W + k] = ai;
+            }
+        }
+    } else {
+        for (int k = 0; k < H; ++k) {
+            for (int x = 0; x < W; ++x) {
+                double ar = 0.0, ai = 0.0;
+                int idx = 0;
+                for (int n = 0; n < H; ++n) {
+                    double wr = c[idx], wi = sign * s[idx];
+                    double vr = in_re[(size_t)n * W + x];
+                    double vi = in_im ? in_im[(size_t)n * W + x] : 0.0;
+                    ar += vr * wr - vi * wi;
+                    ai += vr * wi + vi * wr;
+                    idx += k; if (idx >= N) idx -= N;
+                }
+                out_re[(size_t)k * W + x] = ar;
+                out_im[(size_t)k * W + x] = ai;
+            }
+        }
+    }
+    free(c); free(s);
+    return 0;
+}
+
+int cco_dft2_real(const double *img, int H, int W, double *F_re, double *F_im)
+{
+    size_t n = (size_t)H * W;
+    double *t_re = (double *)malloc(sizeof(double) * n);
+    double *t_im = (double *)malloc(sizeof(double) * n);
+    if (!t_re || !t_im) { free(t_re); free(t_im); return -1; }
+    int rc = dft_axis(img, NULL, H, W, 1, -1, t_re, t_im);      /* rows    */
+    if (!rc) rc = dft_axis(t_re, t_im, H, W, 0, -1, F_re, F_im); /* columns */
+    free(t_re); free(t_im);
+    return rc;
+}
+
+int cco_dft2_literal(const double *img, int H, int W, double *F_re, double *F_im)
+{
+    for (int ky = 0; ky < H; ++ky)
+        for (int kx = 0; kx < W; ++kx) {
+            double ar = 0.0, ai = 0.0;
+            for (int y = 0; y < H; ++y)
+                for (int x = 0; x < W; ++x) {
+                    double a = -2.0 * M_PI * ((double)((long)ky * y % H) / H +
+                                              (double)((long)kx * x % W) / W);
+                    ar += img[(size_t)y * W + x] * cos(a);
+                    ai += img[(size_t)y * W + x] * sin(a);
+                }
+            F_re[(size_t)ky * W + kx] = ar;
+            F_im[(size_t)ky * W + kx] = ai;
+        }
+    return 0;
+}
+
+int cco_idft2(const double *P_re, const double *P_im, int H, int W,
+              double *out_re, double *out_im)
+{
+    size_t n = (size_t)H * W;
+    double *t_re = (double *)malloc(sizeof(double) * n);
+    double *t_im = (double *)malloc(sizeof(double) * n);
+    if (!t_re || !t_im) { free(t_re); free(t_im); return -1; }
+    int rc = dft_axis(P_re, P_im, H, W, 0, +1, t_re, t_im);       /* columns */
+    if (!rc) rc = dft_axis(t_re, t_im, H, W, 1, +1, out_re, out_im); /* rows */
+    double inv = 1.0 / ((double)H * (double)W);
+    for (size_t i = 0; i < n; ++i) { out_re[i] *= inv; out_im[i] *= inv; }
+    free(t_re); free(t_im);
+    return rc;
+}
+
+int cco_cc_direct(const double *I, const double *E, int H, int W, double *cc)
+{
+    for (int sy = 0; sy < H; ++sy)
+        for (int sx = 0; sx < W; ++sx) {
+            double acc = 0.0;
+            for (int y = 0; y < H; ++y)
+                for (int x = 0; x < W; ++x)
+                    acc += I[(size_t)((y + sy) % H) * W + (x + sx) % W] *
+                           E[(size_t)y * W + x];
+            cc[(size_t)sy * W + sx] = acc;
+        }
+    return 0;
+}
+
+/* O3: P = F (x) conj(G) */
+static void conj_product(const double *F_re, const double *F_im,
+                         const double *G_re, const double *G_im, size_t n,
+                         double *P_re, double *P_im)
+{
+    for (size_t i = 0; i < n; ++i) {
+        P_re[i] = F_re[i] * G_re[i] + F_im[i] * G_im[i];
+        P_im[i] = F_im[i] * G_re[i] - F_re[i] * G_im[i];
+    }
+}
+
+int cco_cc_dft(const double *I, const double *E, int H, int W,
+               double *cc, double *P_re, double *P_im)
+{
+    size_t n = (size_t)H * W;
+    double *buf = (double *)malloc(sizeof(double) * n * 5);
+    if (!buf) return -1;
+    double *F_re = buf, *F_im = buf + n, *G_re = buf + 2 * n, *G_im = buf + 3 * n;
+    double *c_im = buf + 4 * n;
+    int rc = cco_dft2_real(I, H, W, F_re, F_im);
+    if (!rc) rc = cco_dft2_real(E, H, W, G_re, G_im);
+    if (!rc) {
+        conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);
+        rc = cco_idft2(P_re, P_im, H, W, cc, c_im);
+    }
+    free(buf);
+    return rc;
+}
+
+long cco_argmax(const double *a, long n)
+{
+    long best = 0;
+    for (long i = 1; i < n; ++i)
+        if (a[i] > a[best]) best = i;      /* strict: smallest index on ties */
+    return best;
+}
+
+int cco_grid_size(int u) { return (3 * u + 1) / 2; }   /* ceil(1.5 u) */
+
+/* Interpolation row A[k] = exp(2*pi*i*f_N(k)*q/(u*N)), k = 0..N-1, for the
+ * lag s = q/u (q integer): signed frequencies f_N(k) = k for k < N/2,
+ * k - N above; for even N the Nyquist bin is split half/half between +N/2
+ * and -N/2, i.e. A[N/2] = cos(pi*s).  Phases are reduced exactly: the
+ * numerator f*q is an integer, taken mod (u*N) before cos/sin. */
+static void interp_row(int N, int u, long q, double *a_re, double *a_im)
+{
+    long long den = (long long)u * N;
+    for (int k = 0; k < N; ++k) {
+        long long f = (2 * k < N) ? k : (long long)k - N;
+        int nyq = (N % 2 == 0 && 2 * k == N);
+        if (nyq) f = N / 2;
+        long long num = (f * (long long)q) % den;
+        if (num < 0) num += den;
+        double ang = 2.0 * M_PI * (double)num / (double)den;
+        a_re[k] = cos(ang);
+        a_im[k] = nyq ? 0.0 : sin(ang);
+    }
+}
+
+int cco_upsampled(const double *P_re, const double *P_im, int H, int W, int u,
+                  int y0, int x0, double *C,
+                  int *best_m, int *best_n, double *top1, double *top2)
+{
+    int M = cco_grid_size(u), c = M / 2;
+    size_t mw = (size_t)M * W, mh = (size_t)M * H;
+    double *Ay_re = (double *)malloc(sizeof(double) * mh);
+    double *Ay_im = (double *)malloc(sizeof(double) * mh);
+    double *Ax_re = (double *)malloc(sizeof(double) * mw);
+    double *Ax_im = (double *)malloc(sizeof(double) * mw);
+    double *T_re = (double *)malloc(sizeof(double) * mw);
+    double *T_im = (double *)malloc(sizeof(double) * mw);
+    double *r_t1 = (double *)malloc(sizeof(double) * M);
+    double *r_t2 = (double *)malloc(sizeof(double) * M);
+    int *r_n = (int *)malloc(sizeof(int) * M);
+    if (!Ay_re || !Ay_im || !Ax_re || !Ax_im || !T_re || !T_im || !r_t1 || !r_t2 || !r_n) {
+        free(Ay_re); free(Ay_im); free(Ax_re); free(Ax_im); free(T_re); free(T_im);
+        free(r_t1); free(r_t2); free(r_n);
+        return -1;
+    }
+    for (int m = 0; m < M; ++m) {
+        interp_row(H, u, (long)y0 * u + (m - c), Ay_re + (size_t)m * H, Ay_im + (size_t)m * H);
+        interp_row(W, u, (long)x0 * u + (m - c), Ax_re + (size_t)m * W, Ax_im + (size_t)m * W);
+    }
+    double inv = 1.0 / ((double)H * (double)W);
+    /* T = A_y * P   (M x H times H x W) */
+    #pragma omp parallel for schedule(static)
+    for (int m = 0; m < M; ++m) {
+        const double *ar = Ay_re + (size_t)m * H, *ai = Ay_im + (size_t)m * H;
+        for (int kx = 0; kx < W; ++kx) {
+            double sr = 0.0, si = 0.0;
+            for (int ky = 0; ky < H; ++ky) {
+                double pr = P_re[(size_t)ky * W + kx], pi = P_im[(size_t)ky * W + kx];
+                sr += ar[ky] * pr - ai[ky] * pi;
+                si += ar[ky] * pi + ai[ky] * pr;
+            }
+            T_re[(size_t)m * W + kx] = sr;
+            T_im[(size_t)m * W + kx] = si;
+        }
+    }
+    /* C = Re(T * A_x^T) / (H W)   (M x W times W x M), argmax per row */
+    #pragma omp parallel for schedule(static)
+    for (int m = 0; m < M; ++m) {
+        const double *tr = T_re + (size_t)m * W, *ti = T_im + (size_t)m * W;
+        double t1 = -INFINITY, t2 = -INFINITY; int bn = 0;
+        for (int n = 0; n < M; ++n) {
+            const double *ar = Ax_re + (size_t)n * W, *ai = Ax_im + (size_t)n * W;
+            double sr = 0.0;
+            for (int kx = 0; kx < W; ++kx) sr += tr[kx] * ar[kx] - ti[kx] * ai[kx];
+            sr *= inv;
+            if (C) C[(size_t)m * M + n] = sr;
+            if (sr > t1) { t2 = t1; t1 = sr; bn = n; }
+            else if (sr > t2) t2 = sr;
+        }
+        r_t1[m] = t1; r_t2[m] = t2; r_n[m] = bn;
+    }
+    double t1 = -INFINITY, t2 = -INFINITY; int bm = 0, bn = 0;
+    for (int m = 0; m < M; ++m) {                 /* row-major order: strict > */
+        if (r_t1[m] > t1) {
+            if (t1 > t2) t2 = t1;
+            if (r_t2[m] > t2) t2 = r_t2[m];
+            t1 = r_t1[m]; bm = m; bn = r_n[m];
+        } else {
+            if (r_t1[m] > t2) t2 = r_t1[m];
+        }
+    }
+    if (best_m) *best_m = bm;
+    if (best_n) *best_n = bn;
+    if (top1) *top1 = t1;
+    if (top2) *top2 = t2;
+    free(Ay_re); free(Ay_im); free(Ax_re); free(Ax_im); free(T_re); free(T_im);
+    free(r_t1); free(r_t2); free(r_n);
+    return 0;
+}
+
+int cco_upsampled_literal(const double *P_re, const double *P_im, int H, int W,
+                          int u, int y0, int x0, double *C)
+{
+    int M = cco_grid_size(u), c = M / 2;
+    double *ay_re = (double *)malloc(sizeof(double) * H), *ay_im = (double *)malloc(sizeof(double) * H);
+    double *ax_re = (double *)malloc(sizeof(double) * W), *ax_im = (double *)malloc(sizeof(double) * W);
+    if (!ay_re || !ay_im || !ax_re || !ax_im) { free(ay_re); free(ay_im); free(ax_re); free(ax_im); return -1; }
+    double inv = 1.0 / ((double)H * (double)W);
+    for (int m = 0; m < M; ++m)
+        for (int n = 0; n < M; ++n) {
+            interp_row(H, u, (long)y0 * u + (m - c), ay_re, ay_im);
+            interp_row(W, u, (long)x0 * u + (n - c), ax_re, ax_im);
+            double acc = 0.0;
+            for (int ky = 0; ky < H; ++ky)
+                for (int kx = 0; kx < W; ++kx) {
+                    /* Re( P * Ay * Ax ) */
+                    double wr = ay_re[ky] * ax_re[kx] - ay_im[ky] * ax_im[kx];
+                    double wi = ay_re[ky] * ax_im[kx] + ay_im[ky] * ax_re[kx];
+                    acc += P_re[(size_t)ky * W + kx] * wr - P_im[(size_t)ky * W + kx] * wi;
+                }
+            C[(size_t)m * M + n] = acc * inv;
+        }
+    free(ay_re); free(ay_im); free(ax_re); free(ax_im);
+    return 0;
+}
+
+double cco_interp_at(const double *P_re, const double *P_im, int H, int W,
+                     double sy, double sx)
+{
+    double acc = 0.0;
+    for (int ky = 0; ky < H; ++ky) {
+        double fy = (2 * ky < H) ? ky : (double)ky - H;
+        int nyq_y = (H % 2 == 0 && 2 * ky == H);
+        double ayr = cos(2.0 * M_PI * fy * sy / H);
+        double ayi = nyq_y ? 0.0 : sin(2.0 * M_PI * fy * sy / H);
+        for (int kx = 0; kx < W; ++kx) {
+            double fx = (2 * kx < W) ? kx : (double)kx - W;
+            int nyq_x = (W % 2 == 0 && 2 * kx == W);
+            double axr = cos(2.0 * M_PI * fx * sx / W);
+            double axi = nyq_x ? 0.0 : sin(2.0 * M_PI * fx * sx / W);
+            double wr = ayr * axr - ayi * axi, wi = ayr * axi + ayi * axr;
+            acc += P_re[(size_t)ky * W + kx] * wr - P_im[(size_t)ky * W + kx] * wi;
+        }
+    }
+    return acc / ((double)H * (double)W);
+}
+
+/* two largest values of a[0..n): top1 at the smallest index attaining the
+ * max, top2 the largest value at any other index */
+static void top_two(const double *a, long n, long *i1, double *t1, double *t2)
+{
+    long b = cco_argmax(a, n);
+    double s = -INFINITY;
+    for (long i = 0; i < n; ++i)
+        if (i != b && a[i] > s) s = a[i];
+    *i1 = b; *t1 = a[b]; *t2 = s;
+}
+
+int cco_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
+              const float *reference, cco_result *out, int threads)
+{
+    if (!frames || !reference || !out || batch < 0 || H <= 0 || W <= 0 || u < 1 ||
+        (dtype != 0 && dtype != 1))
+        return -2;
+    size_t n = (size_t)H * W;
+    /* O1/O2 for the reference: E = (double) reference_f32, G = DFT2(E) */
+    double *E = (double *)malloc(sizeof(double) * n * 3);
+    if (!E) return -1;
+    double *G_re = E + n, *G_im = E + 2 * n;
+    for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    if (cco_dft2_real(E, H, W, G_re, G_im)) { free(E); return -1; }
+
+    int fail = 0;
+#ifdef _OPENMP
+    int nt = threads > 0 ? threads : omp_get_max_threads();
+#else
+    int nt = 1; (void)threads;
+#endif
+    #pragma omp parallel for schedule(dynamic) num_threads(nt)
+    for (int b = 0; b < batch; ++b) {
+        double *buf = (double *)malloc(sizeof(double) * n * 7);
+        if (!buf) {
+            #pragma omp atomic write
+            fail = 1;
+            continue;
+        }
+        double *I = buf, *F_re = buf + n, *F_im = buf + 2 * n, *P_re = buf + 3 * n,
+               *P_im = buf + 4 * n, *cc = buf + 5 * n, *cc_im = buf + 6 * n;
+        /* O1: pixels to double */
+        if (dtype == 0) {
+            const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
+            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+        } else {
+            const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
+            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+        }
+        int rc = cco_dft2_real(I, H, W, F_re, F_im);                 /* O2 */
+        conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);          /* O3 */
+        if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);         /* O4 */
+        cco_result r;
+        memset(&r, 0, sizeof r);
+        long idx;                                                     /* O5 */
+        top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
+        int y0 = (int)(idx / W), x0 = (int)(idx % W);
+        r.wy = (2 * y0 >= H) ? y0 - H : y0;
+        r.wx = (2 * x0 >= W) ? x0 - W : x0;
+        if (u == 1) {
+            r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
+            r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
+        } else {
+            int M = cco_grid_size(u), c = M / 2;                      /* O6 */
+            if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL,
+                                        &r.m, &r.n, &r.up_top1, &r.up_top2);
+            r.dy = (double)r.wy + (double)(r.m - c) / (double)u;      /* O7 */
+            r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
+            r.peak = r.up_top1;
+        }
+        out[b] = r;
+        if (rc) {
+            #pragma omp atomic write
+            fail = 1;
+        }
+        free(buf);
+    }
+    free(E);
+    return fail ? -1 : 0;
+}

@@ -1,0 +1,353 @@
+"""Pins of the CPU oracle (oracle/cc_oracle.c) against what the paper and the
+mathematics fix -- never against itself and never against the CUDA path.
+
+P1  integer circular shifts recovered exactly            (PAPER.md:L55 periodic b.c.)
+P2  Parseval                                              (DFT invariant)
+P3  direct correlation == DFT correlation                 (Eq. (4))
+P4  upsampled values at integer offsets == cc             (ties stage 2 to stage 1)
+P5  local upsampled window == zero-padded inverse DFT     ("as if the
+    original image had u^2 x the pixels"; textbook trigonometric interpolation)
+P6  Fourier-shift theorem, fractional shifts on the 1/u grid recovered exactly
+P7  noiseless Gaussian spots recovered to 1e-4 px         (north_star)
+P8  self-correlation: d = 0, peak = sum I^2
+P9  factored == unfactored upsampled DFT
+P10 invariances (constant offsets, positive scaling, integer rolls)
+P0  worked size example of the paper: u = 256 -> 384 samples
+numpy.fft is used here only as an independent library routine to cross-check
+the naive DFT (a "special case that reduces to a library routine").
+"""
+import numpy as np
+import pytest
+
+
+def _rng(seed):
+    return np.random.default_rng(seed)
+
+
+def _int_image(rng, H, W, hi=200):
+    return rng.integers(0, hi, size=(H, W)).astype(np.float64)
+
+
+def _track_f(oracle, frame, ref, u):
+    """Oracle path on float64 images (pins need non-integer inputs too)."""
+    cc, P = oracle.cc_dft(frame, ref)
+    H, W = cc.shape
+    i = oracle.argmax(cc)
+    y0, x0 = divmod(i, W)
+    wy = y0 - H if 2 * y0 >= H else y0
+    wx = x0 - W if 2 * x0 >= W else x0
+    up = oracle.upsampled(P, u, y0, x0, want_grid=False)
+    M = oracle.grid_size(u)
+    c = M // 2
+    return dict(wy=wy, wx=wx, m=up["m"], n=up["n"], c=c,
+                dy=wy + (up["m"] - c) / u, dx=wx + (up["n"] - c) / u,
+                peak=up["top1"], cc=cc, P=P, y0=y0, x0=x0)
+
+
+# ---------------------------------------------------------------- P0
+def test_p0_grid_size_worked_example(oracle_mod):
+    # golden: tests/golden/grid_size.txt -- "When u = 256 ... 384 x 384"
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "grid_size.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    for u, M in rows:
+        assert oracle_mod.grid_size(int(u)) == int(M)
+
+
+# ---------------------------------------------------------------- DFT vs library / literal
+@pytest.mark.parametrize("shape", [(8, 8), (12, 16), (16, 6), (7, 9)])
+def test_dft2_matches_literal_and_library(oracle_mod, shape):
+    img = _int_image(_rng(1), *shape)
+    F = oracle_mod.dft2(img)
+    Fl = oracle_mod.dft2(img, literal=True)
+    Fn = np.fft.fft2(img)
+    s = np.abs(Fn).max()
+    assert np.abs(F - Fl).max() <= 1e-12 * s
+    assert np.abs(F - Fn).max() <= 1e-12 * s
+    back = oracle_mod.idft2(F)
+    assert np.abs(back.real - img).max() <= 1e-12 * img.max()
+    assert np.abs(back.imag).max() <= 1e-12 * img.max()
+
+
+def test_dft2_delta_and_plane_wave(oracle_mod):
+    # closed forms: delta at (a,b) -> pure phase; cos plane wave -> two bins
+    H, W = 8, 16
+    img = np.zeros((H, W)); img[3, 5] = 1.0
+    F = oracle_mod.dft2(img)
+    ky, kx = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
+    assert np.abs(F - np.exp(-2j * np.pi * (ky * 3 / H + kx * 5 / W))).max() < 1e-13
+    y, x = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
+    img = np.cos(2 * np.pi * (2 * y / H + 3 * x / W))
+    F = oracle_mod.dft2(img)
+    exp = np.zeros((H, W), complex); exp[2, 3] = H * W / 2; exp[H - 2, W - 3] = H * W / 2
+    assert np.abs(F - exp).max() < 1e-11
+
+
+# ---------------------------------------------------------------- P2
+def test_p2_parseval(oracle_mod):
+    rng = _rng(2)
+    H, W = 16, 24
+    I, E = _int_image(rng, H, W), _int_image(rng, H, W)
+    F, G = oracle_mod.dft2(I), oracle_mod.dft2(E)
+    assert abs((np.abs(F) ** 2).sum() / (H * W) - (I * I).sum()) <= 1e-12 * (I * I).sum()
+    assert abs((np.abs(G) ** 2).sum() / (H * W) - (E * E).sum()) <= 1e-12 * (E * E).sum()
+    cc, P = oracle_mod.cc_dft(I, E)
+    cross = (I * E).sum()
+    assert abs((F * G.conj()).sum().real / (H * W) - cross) <= 1e-12 * cross
+    assert abs(cc[0, 0] - cross) <= 1e-12 * cross
+
+
+# ---------------------------------------------------------------- P3
+@pytest.mark.parametrize("shape", [(8, 8), (16, 16), (12, 16), (5, 7)])
+def test_p3_direct_equals_dft_correlation(oracle_mod, shape):
+    rng = _rng(3)
+    I, E = _int_image(rng, *shape), _int_image(rng, *shape)
+    cc, _ = oracle_mod.cc_dft(I, E)
+    ccd = oracle_mod.cc_direct(I, E)
+    assert np.abs(cc - ccd).max() <= 1e-9 * np.abs(ccd).max()
+    assert oracle_mod.argmax(cc) == oracle_mod.argmax(ccd)
+    # brute force of the brute force, in numpy, on the defining sum of Eq. (4)
+    H, W = shape
+    s = (2 % H, 3 % W)
+    val = sum(I[(y + s[0]) % H, (x + s[1]) % W] * E[y, x] for y in range(H) for x in range(W))
+    assert abs(ccd[s] - val) <= 1e-9 * abs(val)
+
+
+# ---------------------------------------------------------------- P1 / P8
+def test_p1_integer_circular_shifts_all_lags_tiny(oracle_mod):
+    rng = _rng(4)
+    H, W, u = 8, 8, 4
+    ref = _int_image(rng, H, W)
+    M = oracle_mod.grid_size(u); c = M // 2
+    for a in range(H):
+        for b in range(W):
+            frame = np.roll(ref, (a, b), axis=(0, 1))
+            r = _track_f(oracle_mod, frame, ref, u)
+            assert (r["wy"], r["wx"]) == (a - H if 2 * a >= H else a, b - W if 2 * b >= W else b)
+            assert (r["m"], r["n"]) == (c, c)
+            assert abs(r["peak"] - (ref * ref).sum()) <= 1e-12 * (ref * ref).sum()
+
+
+@pytest.mark.parametrize("H,W,u", [(64, 64, 100), (32, 128, 20), (128, 32, 7)])
+def test_p1_integer_circular_shifts_through_track(oracle_mod, H, W, u):
+    rng = _rng(5)
+    ref_px = rng.integers(0, 4000, size=(H, W)).astype(np.uint16)
+    sh = [(0, 0), (1, 0), (0, -1), (H // 2 - 1, W // 2 - 1), (-H // 2, -W // 2), (5, -17 % W)]
+    frames = np.stack([np.roll(ref_px, s, axis=(0, 1)) for s in sh])
+    r = oracle_mod.track(frames, ref_px.astype(np.float32), u)
+    e2 = (ref_px.astype(np.float64) ** 2).sum()
+    for i, (a, b) in enumerate(sh):
+        a = (a + H // 2) % H - H // 2
+        b = (b + W // 2) % W - W // 2
+        assert (r.wy[i], r.wx[i]) == (a, b)
+        assert r.dy[i] == a and r.dx[i] == b          # sub-pixel offset exactly 0
+        assert abs(r.peak[i] - e2) <= 1e-12 * e2      # P8 for shift (0,0): peak = sum I^2
+        assert r.cc_top1[i] > r.cc_top2[i]
+
+
+# ---------------------------------------------------------------- P4
+@pytest.mark.parametrize("H,W,u", [(8, 8, 2), (12, 16, 4), (9, 7, 2)])
+def test_p4_integer_offsets_reproduce_cc(oracle_mod, H, W, u):
+    rng = _rng(6)
+    I, E = _int_image(rng, H, W), _int_image(rng, H, W)
+    cc, P = oracle_mod.cc_dft(I, E)
+    y0, x0 = divmod(oracle_mod.argmax(cc), W)
+    up = oracle_mod.upsampled(P, u, y0, x0)
+    M = oracle_mod.grid_size(u); c = M // 2
+    hits = 0
+    for m in range(M):
+        for n in range(M):
+            if (m - c) % u == 0 and (n - c) % u == 0:
+                j, i = (m - c) // u, (n - c) // u
+                ref = cc[(y0 + j) % H, (x0 + i) % W]
+                assert abs(up["C"][m, n] - ref) <= 1e-12 * np.abs(cc).max()
+                hits += 1
+    assert hits >= 1
+
+
+# ---------------------------------------------------------------- P5
+def _zero_padded_upsample(P, u):
+    """Textbook trigonometric interpolation: embed the H x W spectrum in a
+    uH x uW one (Nyquist bins of even axes split half/half), inverse DFT
+    (numpy, library routine), scale u^2."""
+    H, W = P.shape
+
+    def embed_axis(A, N, axis):
+        A = np.moveaxis(A, axis, 0)
+        big = np.zeros((u * N,) + A.shape[1:], complex)
+        for k in range(N):
+            f = k if 2 * k < N else k - N
+            if N % 2 == 0 and 2 * k == N:
+                big[N // 2] += 0.5 * A[k]
+                big[u * N - N // 2] += 0.5 * A[k]
+            else:
+                big[f % (u * N)] += A[k]
+        return np.moveaxis(big, 0, axis)
+
+    big = embed_axis(embed_axis(P, H, 0), W, 1)
+    return np.fft.ifft2(big) * (u * u)
+
+
+@pytest.mark.parametrize("H,W,u", [(8, 8, 2), (12, 16, 4), (8, 8, 4), (7, 10, 2)])
+def test_p5_window_of_zero_padded_inverse_dft(oracle_mod, H, W, u):
+    rng = _rng(7)
+    I, E = _int_image(rng, H, W), _int_image(rng, H, W)
+    cc, P = oracle_mod.cc_dft(I, E)
+    full = _zero_padded_upsample(P, u)
+    assert np.abs(full.imag).max() <= 1e-10 * np.abs(full.real).max()
+    y0, x0 = divmod(oracle_mod.argmax(cc), W)
+    up = oracle_mod.upsampled(P, u, y0, x0)
+    M = oracle_mod.grid_size(u); c = M // 2
+    for m in range(M):
+        for n in range(M):
+            ref = full.real[(y0 * u + m - c) % (u * H), (x0 * u + n - c) % (u * W)]
+            assert abs(up["C"][m, n] - ref) <= 1e-12 * np.abs(full.real).max()
+    # interp_at (general real lag) agrees with the grid at grid lags
+    v = oracle_mod.interp_at(P, y0 + (1 - c) / u, x0 + (2 - c) / u)
+    assert abs(v - up["C"][1, 2]) <= 1e-12 * np.abs(full.real).max()
+
+
+# ---------------------------------------------------------------- P9
+@pytest.mark.parametrize("H,W,u", [(8, 8, 3), (6, 10, 4)])
+def test_p9_factored_equals_unfactored(oracle_mod, H, W, u):
+    rng = _rng(8)
+    I, E = _int_image(rng, H, W), _int_image(rng, H, W)
+    cc, P = oracle_mod.cc_dft(I, E)
+    y0, x0 = divmod(oracle_mod.argmax(cc), W)
+    a = oracle_mod.upsampled(P, u, y0, x0)
+    b = oracle_mod.upsampled(P, u, y0, x0, literal=True)
+    assert np.abs(a["C"] - b["C"]).max() <= 1e-12 * np.abs(b["C"]).max()
+    assert (a["m"], a["n"]) == (b["m"], b["n"])
+    # argmax bookkeeping of cco_upsampled against numpy on its own grid
+    i = int(np.argmax(a["C"]))
+    assert (a["m"], a["n"]) == divmod(i, a["C"].shape[1])
+    srt = np.sort(a["C"].ravel())
+    assert a["top1"] == srt[-1] and a["top2"] == srt[-2]
+
+
+# ---------------------------------------------------------------- P6
+def _fourier_shift(ref, dy, dx):
+    """Band-limited ref (Nyquist rows/cols already zero) shifted by (dy, dx)
+    through the phase ramp (library FFT; shift theorem)."""
+    H, W = ref.shape
+    fy = np.fft.fftfreq(H)[:, None]
+    fx = np.fft.fftfreq(W)[None, :]
+    return np.fft.ifft2(np.fft.fft2(ref) * np.exp(-2j * np.pi * (fy * dy + fx * dx))).real
+
+
+@pytest.mark.parametrize("u,delta", [(10, (0.3, -0.7)), (10, (2.4, 5.0)), (20, (-3.35, 1.7)),
+                                     (4, (0.25, 0.5))])
+def test_p6_fourier_shift_theorem(oracle_mod, u, delta):
+    rng = _rng(9)
+    H, W = 16, 20
+    ref = rng.normal(size=(H, W)) + 5.0
+    Fr = np.fft.fft2(ref); Fr[H // 2, :] = 0; Fr[:, W // 2] = 0
+    ref = np.fft.ifft2(Fr).real
+    frame = _fourier_shift(ref, *delta)
+    r = _track_f(oracle_mod, frame, ref, u)
+    assert abs(r["dy"] - delta[0]) <= 1e-12 and abs(r["dx"] - delta[1]) <= 1e-12
+    e2 = (ref * ref).sum()
+    assert abs(r["peak"] - e2) <= 1e-11 * e2
+
+
+# ---------------------------------------------------------------- P7
+def _gauss_spot(H, W, cy, cx, sigma, amp=1000.0, bg=10.0):
+    y = np.arange(H)[:, None]; x = np.arange(W)[None, :]
+    return amp * np.exp(-((y - cy) ** 2 + (x - cx) ** 2) / (2 * sigma ** 2)) + bg
+
+
+def test_p7_gaussian_on_grid_shifts_exact(oracle_mod):
+    H = W = 64; u = 100
+    ref = _gauss_spot(H, W, 32, 32, 3.0)
+    for sy, sx in [(0.37, -1.42), (-4.99, 3.5), (2.0, 0.01), (-0.74, 0.74)]:
+        r = _track_f(oracle_mod, _gauss_spot(H, W, 32 + sy, 32 + sx, 3.0), ref, u)
+        assert abs(r["dy"] - sy) < 1e-9 and abs(r["dx"] - sx) < 1e-9
+
+
+def test_p7_gaussian_arbitrary_shifts_to_1e_4(oracle_mod):
+    # u = 5000 -> grid spacing 2e-4, so the nearest grid point is within 1e-4 px
+    H = W = 32; u = 5000
+    ref = _gauss_spot(H, W, 16, 16, 2.5)
+    for sy, sx in [(1.234567, -2.718281), (-3.141592, 0.577215)]:
+        r = _track_f(oracle_mod, _gauss_spot(H, W, 16 + sy, 16 + sx, 2.5), ref, u)
+        assert abs(r["dy"] - sy) <= 1e-4 + 1e-9 and abs(r["dx"] - sx) <= 1e-4 + 1e-9
+
+
+# ---------------------------------------------------------------- P10 + degenerate cases
+def test_p10_invariances(oracle_mod):
+    rng = _rng(10)
+    H, W, u = 16, 16, 8
+    ref = _gauss_spot(H, W, 8, 8, 1.7, amp=300, bg=4) + rng.normal(size=(H, W))
+    frame = _gauss_spot(H, W, 9.3, 6.6, 1.7, amp=300, bg=4) + rng.normal(size=(H, W))
+    base = _track_f(oracle_mod, frame, ref, u)
+    r = _track_f(oracle_mod, frame + 37.0, ref, u)
+    assert (r["dy"], r["dx"]) == (base["dy"], base["dx"])
+    r = _track_f(oracle_mod, frame, ref + 11.0, u)
+    assert (r["dy"], r["dx"]) == (base["dy"], base["dx"])
+    r = _track_f(oracle_mod, 3.0 * frame, 0.5 * ref, u)
+    assert (r["dy"], r["dx"]) == (base["dy"], base["dx"])
+    assert abs(r["peak"] - 1.5 * base["peak"]) <= 1e-12 * abs(base["peak"])
+    r = _track_f(oracle_mod, np.roll(frame, (2, -3), axis=(0, 1)), ref, u)
+    assert abs(r["dy"] - (base["dy"] + 2)) < 1e-12 and abs(r["dx"] - (base["dx"] - 3)) < 1e-12
+
+
+def test_constant_frame_degenerate_case(oracle_mod):
+    # cc constant -> (y0,x0) = (0,0); C constant up to rounding is NOT guaranteed
+    # in floating point, so use frame = 0: everything is exactly 0 and the
+    # smallest-index rule decides: (m*,n*) = (0,0), d = (-c/u, -c/u).
+    H, W, u = 8, 8, 4
+    frames = np.zeros((1, H, W), np.uint8)
+    ref = _rng(11).random((H, W)).astype(np.float32)
+    r = oracle_mod.track(frames, ref, u)
+    c = oracle_mod.grid_size(u) // 2
+    assert (r.wy[0], r.wx[0], r.m[0], r.n[0]) == (0, 0, 0, 0)
+    assert r.dy[0] == -c / u and r.dx[0] == -c / u and r.peak[0] == 0.0
+
+
+def test_exact_tie_smallest_index(oracle_mod):
+    # reference = single bright pixel, frame = two equal bright pixels:
+    # cc has two exactly equal maxima (integers, exact in double); the smaller
+    # row-major index must win.
+    H, W = 8, 8
+    ref = np.zeros((H, W), np.float32); ref[0, 0] = 2.0
+    fr = np.zeros((1, H, W), np.uint16); fr[0, 1, 5] = 7; fr[0, 3, 2] = 7
+    r = oracle_mod.track(fr, ref, 1)
+    assert (r.wy[0], r.wx[0]) == (1, 5 - W)
+    assert r.cc_top1[0] == r.cc_top2[0] == 14.0
+
+
+def test_upsample_one_is_integer_peak_only(oracle_mod):
+    rng = _rng(12)
+    fr = rng.integers(0, 255, size=(3, 8, 16)).astype(np.uint8)
+    ref = rng.random((8, 16)).astype(np.float32)
+    r = oracle_mod.track(fr, ref, 1)
+    for i in range(3):
+        cc = oracle_mod.cc_direct(fr[i].astype(float), ref.astype(float))
+        y0, x0 = divmod(int(np.argmax(cc)), 16)
+        assert (r.wy[i], r.wx[i]) == (y0 - 8 if y0 >= 4 else y0, x0 - 16 if x0 >= 8 else x0)
+        assert r.dy[i] == r.wy[i] and r.dx[i] == r.wx[i]
+
+
+def test_track_matches_piecewise_pipeline(oracle_mod):
+    # cco_track (pixels in, result out) equals the step-by-step calls
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, [3, 7]); ref = wl.reference(cfg)
+    r = oracle_mod.track(fr, ref, cfg.upsample)
+    for i in range(2):
+        p = _track_f(oracle_mod, fr[i].astype(np.float64), ref.astype(np.float64), cfg.upsample)
+        assert (p["wy"], p["wx"], p["m"], p["n"]) == (r.wy[i], r.wx[i], r.m[i], r.n[i])
+        assert p["dy"] == r.dy[i] and p["dx"] == r.dx[i]
+
+
+def test_p11_shot_noise_sanity_band(oracle_mod):
+    # informational band: CC-U error within ~1x-3x of the
+    # shot-noise limit w0/(2 sqrt(N_gamma)) = sigma/sqrt(N_gamma)
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    idx = np.arange(48)
+    r = oracle_mod.track(wl.frames(cfg, idx), wl.reference(cfg), cfg.upsample)
+    s = wl.shifts(cfg)[idx]
+    err = np.sqrt(np.mean((r.dy - s[:, 0]) ** 2 + (r.dx - s[:, 1]) ** 2) / 2)
+    limit = 3.0 / np.sqrt(2 * np.pi * 9 * 1000)
+    assert 0.5 * limit < err < 4.0 * limit
