@@ -1,0 +1,137 @@
+/*
+ * cc.h -- C-ABI boundary of the B200-native cross-correlation tracker.
+ *
+ * The library computes, for every camera frame, the displacement of a single
+ * particle against a fixed reference image (RI) by the method of Werneck et
+ * al., arxiv 2310.08770:
+ *
+ *   cc(s) = sum_r I(r+s) E(r) = F^-1[ F[I] (x) conj(F[E]) ](s)
+ *                                    -- PAPER.md:L66-70, Eq. (4), Sec. II (CC-U)
+ *   integer peak  = argmax_s cc(s)   -- PAPER.md:L90, Sec. III, sentence 1
+ *   sub-pixel peak = argmax over a 1.5-pixel window around the integer peak,
+ *                    sampled at ceil(1.5*u) points per axis (spacing 1/u), of
+ *                    the element-wise product "interpolated into the upsampled
+ *                    region, followed by an inverse discrete Fourier transform"
+ *                                    -- PAPER.md:L90, Sec. III, sentences 2-5
+ *
+ * Every step runs in hand-written CUDA kernels for sm_100a (one fused kernel
+ * per frame shape).  There is no CPU fallback: on a device
+ * that is not compute capability 10.x every entry point returns CC_ERR_ARCH.
+ *
+ * Conventions:
+ *   - images are row-major [y][x]; +x = increasing column, +y = increasing row;
+ *   - the displacement d = (dy, dx) is the lag that maximises cc, i.e.
+ *     frame(r) ~ reference(r - d); it is a multiple of 1/upsample;
+ *   - the integer peak is wrapped to [-N/2, N/2) per axis; ties are resolved
+ *     towards the smallest row-major index;
+ *   - `peak` is the (upsampled) correlation sum at the maximum, in
+ *     pixel-value^2 units (sum_r I(r+d) E(r)).
+ *
+ * Threading: a plan is immutable after creation.  cc_track() on one plan may
+ * be enqueued on several streams concurrently only when cc_plan_info()
+ * reports scratch_bytes == 0; otherwise serialise the calls.  cc_track_host()
+ * uses plan-owned staging buffers and must be serialised per plan.
+ */
+#ifndef CC_H
+#define CC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cc_plan cc_plan; /* opaque; owned by the library */
+
+typedef enum { CC_U8 = 0, CC_U16 = 1 } cc_dtype; /* pixel type of the frames */
+
+typedef enum {
+    CC_OK = 0,
+    CC_ERR_INVALID_ARG = 1, /* NULL pointer, batch < 0, H/W <= 0, upsample < 1, misaligned frames */
+    CC_ERR_UNSUPPORTED = 2, /* frame shape outside the built kernel variants                        */
+    CC_ERR_NOMEM = 3,       /* host or device allocation failed                                    */
+    CC_ERR_CUDA = 4,        /* a CUDA runtime call failed; text in cc_last_error()                 */
+    CC_ERR_ARCH = 5         /* no CUDA device of compute capability 10.x                           */
+} cc_status;
+
+/* Static description of the kernel variant(s) a plan selected. */
+typedef struct {
+    int H, W, upsample, dtype;
+    int grid_M;               /* M = ceil(1.5*upsample) upsampled samples per axis */
+    int cluster_size;         /* CTAs per frame, throughput variant                               */
+    int threads;              /* threads per CTA                                                   */
+    int smem_bytes;           /* dynamic shared memory per CTA                                     */
+    int max_clusters;         /* co-resident clusters = frames in flight                           */
+    int lat_cluster_size;     /* CTAs per frame of the small-batch (latency) variant, 0 if none    */
+    int lat_max_clusters;
+    long long scratch_bytes;  /* plan-owned device scratch used by cc_track (0: stream-concurrent)  */
+    long long table_bytes;    /* plan-owned constant tables (reference spectrum, upsampling tables) */
+} cc_plan_info_t;
+
+/*
+ * cc_plan_create -- PAPER.md:L98/L108 ("F[E_0] = F[I_0]": the RI is held as its
+ * spectrum) plus the plan-time tables of the upsampled DFT.
+ *   out        receives the plan (host pointer); untouched on error
+ *   H, W       frame rows / columns; supported: powers of two, 64..1024 each
+ *   dtype      pixel type of the frames later passed to cc_track
+ *   upsample   u >= 1; u == 1 means "integer peak only"
+ *   reference  H*W float32, row-major, HOST or DEVICE pointer; copied, the
+ *              caller may free it on return
+ * May synchronise the device.  Returns CC_OK or an error code.
+ */
+cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype, int upsample,
+                         const float *reference);
+
+/*
+ * cc_track -- the hot path (Eq. (4)):
+ * ingest -> real 2D FFT -> (x) conj(F[E]) -> inverse FFT -> integer argmax ->
+ * upsampled DFT -> sub-pixel argmax, fused so that each frame is read from HBM
+ * once and 12 bytes are written back.
+ *   frames   DEVICE pointer, batch*H*W pixels of the plan's dtype, contiguous,
+ *            16-byte aligned; owned by the caller, read only
+ *   batch    number of frames (0 -> CC_OK, nothing enqueued)
+ *   dx,dy    DEVICE pointers, batch float32 each: displacement in pixels
+ *   peak     DEVICE pointer, batch float32, or NULL
+ *   stream   cudaStream_t (as void*), NULL = default stream
+ * Only enqueues work on `stream`; never synchronises, never allocates.
+ */
+cc_status cc_track(const cc_plan *plan, const void *frames, int batch,
+                   float *dx, float *dy, float *peak, void *stream);
+
+/*
+ * cc_track_debug -- cc_track that additionally returns the wrapped integer
+ * peak of step a5 (PAPER.md:L90 sentence 1).
+ *   iy, ix   DEVICE pointers, batch int32 each, or NULL
+ */
+cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch,
+                         float *dx, float *dy, float *peak, int *iy, int *ix, void *stream);
+
+/*
+ * cc_track_host -- the same path for HOST buffers (pageable or pinned): frames
+ * are copied host->device in chunks overlapped with compute, results are
+ * copied back, and the call returns after everything has completed.
+ *   frames            HOST pointer, batch*H*W pixels
+ *   dx, dy, peak      HOST pointers, batch float32 each (peak may be NULL)
+ * Uses plan-owned streams and staging buffers (grown on first use).
+ */
+cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
+                        float *dx, float *dy, float *peak);
+
+/* Frees every device/host allocation of the plan.  NULL is a no-op. */
+cc_status cc_plan_destroy(cc_plan *plan);
+
+/* Fills *info; returns CC_ERR_INVALID_ARG on NULL. */
+cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info);
+
+/*
+ * cc_fp32_peak_probe -- measurement aid for bench.py's roofline: runs a
+ * dependent-free FFMA loop on every SM and returns the achieved FP32 rate.
+ *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
+ */
+cc_status cc_fp32_peak_probe(double *tflops, void *stream);
+
+const char *cc_status_string(cc_status s);
+const char *cc_last_error(void); /* thread-local detail of the last failure */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CC_H */

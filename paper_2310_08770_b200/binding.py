@@ -1,0 +1,176 @@
+"""Thin ctypes binding of the C-ABI library (include/cc.h): argument
+marshalling only -- every step of the path runs in the CUDA kernels of
+``libcc_b200.so``.  PyTorch is used for device memory and streams.
+
+There is no CPU fallback: if the extension is missing or the device is not a
+compute-capability-10.x GPU, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcc_b200.so")
+
+CC_U8, CC_U16 = 0, 1
+_STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
+           4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
+
+EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_host", "cc_plan_destroy",
+           "cc_plan_info", "cc_fp32_peak_probe", "cc_status_string", "cc_last_error"]
+
+
+class CcError(RuntimeError):
+    def __init__(self, status: int, detail: str):
+        super().__init__("%s: %s" % (_STATUS.get(status, str(status)), detail))
+        self.status = status
+
+
+class PlanInfo(ctypes.Structure):
+    _fields_ = [("H", ctypes.c_int), ("W", ctypes.c_int), ("upsample", ctypes.c_int), ("dtype", ctypes.c_int),
+                ("grid_M", ctypes.c_int), ("cluster_size", ctypes.c_int), ("threads", ctypes.c_int),
+                ("smem_bytes", ctypes.c_int), ("max_clusters", ctypes.c_int),
+                ("lat_cluster_size", ctypes.c_int), ("lat_max_clusters", ctypes.c_int),
+                ("scratch_bytes", ctypes.c_longlong), ("table_bytes", ctypes.c_longlong)]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libcc_b200.so (built in-tree by ``python -m paper_2310_08770_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("CUDA extension %s is missing: run `python -m paper_2310_08770_b200.build` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, ci = ctypes.c_void_p, ctypes.c_int
+        lib.cc_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, vp]
+        lib.cc_plan_create.restype = ci
+        lib.cc_track.argtypes = [vp, vp, ci, vp, vp, vp, vp]
+        lib.cc_track.restype = ci
+        lib.cc_track_debug.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp, vp]
+        lib.cc_track_debug.restype = ci
+        lib.cc_track_host.argtypes = [vp, vp, ci, vp, vp, vp]
+        lib.cc_track_host.restype = ci
+        lib.cc_plan_destroy.argtypes = [vp]
+        lib.cc_plan_destroy.restype = ci
+        lib.cc_plan_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
+        lib.cc_plan_info.restype = ci
+        lib.cc_fp32_peak_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
+        lib.cc_fp32_peak_probe.restype = ci
+        lib.cc_status_string.argtypes = [ci]
+        lib.cc_status_string.restype = ctypes.c_char_p
+        lib.cc_last_error.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+def _check(st: int):
+    if st != 0:
+        raise CcError(st, load_library().cc_last_error().decode())
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("a CUDA device is required (no CPU fallback)")
+    return torch
+
+
+class Plan:
+    """cc_plan_create / cc_track / cc_plan_destroy (include/cc.h)."""
+
+    def __init__(self, H: int, W: int, dtype, upsample: int, reference):
+        lib = load_library()
+        _torch()
+        dt = np.dtype(dtype)
+        if dt == np.uint8:
+            self.cc_dtype = CC_U8
+        elif dt == np.uint16:
+            self.cc_dtype = CC_U16
+        else:
+            raise TypeError("pixel dtype must be uint8 or uint16")
+        self.np_dtype = dt
+        self.H, self.W, self.upsample = int(H), int(W), int(upsample)
+        ref = np.ascontiguousarray(reference, dtype=np.float32)
+        if ref.shape != (self.H, self.W):
+            raise ValueError("reference must be (H, W)")
+        self._h = ctypes.c_void_p()
+        _check(lib.cc_plan_create(ctypes.byref(self._h), self.H, self.W, self.cc_dtype, self.upsample,
+                                  ref.ctypes.data_as(ctypes.c_void_p)))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().cc_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def info(self) -> dict:
+        inf = PlanInfo()
+        _check(load_library().cc_plan_info(self._h, ctypes.byref(inf)))
+        return {k: getattr(inf, k) for k, _ in PlanInfo._fields_}
+
+    def device_frames(self, frames_np):
+        """Copy a (B, H, W) uint8/uint16 numpy array to the device (torch has no
+        uint16 arithmetic; the tensor is only a byte container)."""
+        torch = _torch()
+        a = np.ascontiguousarray(frames_np, dtype=self.np_dtype)
+        if a.ndim == 2:
+            a = a[None]
+        assert a.shape[1:] == (self.H, self.W)
+        t = torch.from_numpy(a.view(np.uint8).reshape(a.shape[0], -1)).cuda()
+        return t
+
+    def track(self, frames_dev, batch: int | None = None, want_peak: bool = True, debug: bool = False,
+              out=None, stream=None):
+        """cc_track on a device tensor of raw frame bytes.  Returns device
+        tensors (dx, dy, peak[, iy, ix]); nothing is synchronised."""
+        torch = _torch()
+        lib = load_library()
+        fb = self.H * self.W * self.np_dtype.itemsize
+        if batch is None:
+            batch = frames_dev.numel() * frames_dev.element_size() // fb
+        dev = frames_dev.device
+        if out is None:
+            dx = torch.empty(batch, dtype=torch.float32, device=dev)
+            dy = torch.empty(batch, dtype=torch.float32, device=dev)
+            pk = torch.empty(batch, dtype=torch.float32, device=dev) if want_peak else None
+        else:
+            dx, dy, pk = out
+        s = (stream.cuda_stream if stream is not None else torch.cuda.current_stream(dev).cuda_stream)
+        pkp = pk.data_ptr() if pk is not None else None
+        if debug:
+            iy = torch.empty(batch, dtype=torch.int32, device=dev)
+            ix = torch.empty(batch, dtype=torch.int32, device=dev)
+            _check(lib.cc_track_debug(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(), pkp,
+                                      iy.data_ptr(), ix.data_ptr(), s))
+            return dx, dy, pk, iy, ix
+        _check(lib.cc_track(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(), pkp, s))
+        return dx, dy, pk
+
+    def track_host(self, frames_np, dx=None, dy=None, peak=None):
+        """cc_track_host: host numpy frames in, host numpy results out (H2D/D2H inside)."""
+        lib = load_library()
+        a = frames_np
+        assert a.dtype == self.np_dtype and a.flags["C_CONTIGUOUS"]
+        batch = a.shape[0] if a.ndim == 3 else 1
+        dx = np.empty(batch, np.float32) if dx is None else dx
+        dy = np.empty(batch, np.float32) if dy is None else dy
+        peak = np.empty(batch, np.float32) if peak is None else peak
+        _check(lib.cc_track_host(self._h, a.ctypes.data_as(ctypes.c_void_p), batch,
+                                 dx.ctypes.data_as(ctypes.c_void_p), dy.ctypes.data_as(ctypes.c_void_p),
+                                 peak.ctypes.data_as(ctypes.c_void_p)))
+        return dx, dy, peak
+
+
+def fp32_peak_probe() -> float:
+    _torch()
+    v = ctypes.c_double()
+    _check(load_library().cc_fp32_peak_probe(ctypes.byref(v), None))
+    return v.value

@@ -1,0 +1,509 @@
+// cc_api.cu -- C-ABI boundary (include/cc.h): plan creation (reference
+// spectrum and upsampling tables, fp64 on the host, rounded once to fp32),
+// variant selection, launches.  Product code: shares nothing with oracle/.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <complex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/cc.h"
+#include "cc_common.h"
+
+// ------------------------------------------------------------------ variants
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG) CcVariant cc_variant_##name();
+#include "cc_variant_list.h"
+#undef CCV
+
+typedef CcVariant (*cc_variant_fn)();
+static const cc_variant_fn g_variant_fns[] = {
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG) &cc_variant_##name,
+#include "cc_variant_list.h"
+#undef CCV
+};
+
+static thread_local std::string g_err;
+static cc_status fail(cc_status s, const std::string &msg)
+{
+    g_err = msg;
+    return s;
+}
+static cc_status fail_cuda(cudaError_t e, const char *what)
+{
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return CC_ERR_CUDA;
+}
+#define CK(call)                                         \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return fail_cuda(e_, #call); \
+    } while (0)
+
+static const int SMEM_LIMIT = 232448;  // 227 KB per CTA on sm_100
+
+// Per-variant launch geometry derived from the plan (M etc.).
+struct VarPlan {
+    CcVariant v;
+    int smem_bytes = 0, max_clusters = 0;
+    int MS = 0, nsb = 0, NCH2 = 0, TPN2 = 0, u_bytes = 0, stg_floats = 0;
+    int MC1 = 0, np2_need = 0;
+    float2 *Sg = nullptr;  // global spectrum scratch (s_global variants)
+    size_t sg_bytes = 0;
+    bool ready = false;
+};
+
+struct cc_plan {
+    int H = 0, W = 0, u = 0, M = 0, c = 0, dtype = 0;
+    int Mp1 = 0, Np2 = 0, c0 = 0;
+    double Emean = 0.0;
+    // device tables
+    float2 *tw = nullptr, *Gt = nullptr;
+    uint16_t *row_slot = nullptr, *col_partner = nullptr;
+    float4 *ab = nullptr;
+    float *Dt = nullptr, *AxT = nullptr;
+    size_t table_bytes = 0;
+    VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
+    bool has_lat = false;
+    // cc_track_host resources
+    cudaStream_t hs[2] = {nullptr, nullptr};
+    cudaEvent_t hev[2] = {nullptr, nullptr};
+    void *dframes[2] = {nullptr, nullptr};
+    float *dres = nullptr;  // [3][cap]
+    int chunk_cap = 0, res_cap = 0;
+};
+
+// ------------------------------------------------------------------ host fp64 FFT (plan time only)
+static void fft1d(std::vector<std::complex<double>> &a, int n, int stride, size_t off, bool inv,
+                  const std::vector<std::complex<double>> &w)  // w[j] = exp(-2 pi i j / n)
+{
+    // iterative radix-2, in place on a[off + i*stride]
+    for (int i = 1, j = 0; i < n; ++i) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) std::swap(a[off + (size_t)i * stride], a[off + (size_t)j * stride]);
+    }
+    for (int len = 2; len <= n; len <<= 1) {
+        const int step = n / len;
+        for (int i = 0; i < n; i += len)
+            for (int k = 0; k < len / 2; ++k) {
+                std::complex<double> t = w[(size_t)k * step];
+                if (inv) t = std::conj(t);
+                const std::complex<double> x = a[off + (size_t)(i + k) * stride];
+                const std::complex<double> y = a[off + (size_t)(i + k + len / 2) * stride] * t;
+                a[off + (size_t)(i + k) * stride] = x + y;
+                a[off + (size_t)(i + k + len / 2) * stride] = x - y;
+            }
+    }
+}
+
+static std::vector<std::complex<double>> unit_roots(int n)
+{
+    std::vector<std::complex<double>> w(n);
+    for (int j = 0; j < n; ++j) {
+        // exact octant values keep the table symmetric
+        const double a = -2.0 * M_PI * (double)j / (double)n;
+        w[j] = std::complex<double>(cos(a), sin(a));
+    }
+    return w;
+}
+
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+static int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+template <class T>
+static cudaError_t upload(T **dptr, const std::vector<T> &h, size_t *acc)
+{
+    cudaError_t e = cudaMalloc((void **)dptr, h.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    *acc += h.size() * sizeof(T);
+    return cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+// geometry of one variant for this plan; returns false if it cannot fit
+static bool plan_variant(VarPlan &vp, int M, int W, int H)
+{
+    const CcVariant &v = vp.v;
+    const int NC = W / 2 / v.CS;
+    const int TPN1 = 2 * NC / v.TN1, TPM1 = v.NT / TPN1;
+    vp.MC1 = TPM1 * v.TM1;
+    const int want = (M + v.TN2 - 1) / v.TN2;
+    vp.TPN2 = std::min(v.NT, std::max(1, want));
+    if (want > v.NT) {  // several n-chunks: chunk starts must stay 16-byte aligned
+        while ((vp.TPN2 * v.TN2) % 4) --vp.TPN2;
+    }
+    vp.NCH2 = round_up(vp.TPN2 * v.TN2, 4);
+    const int nch = (M + vp.TPN2 * v.TN2 - 1) / (vp.TPN2 * v.TN2);
+    vp.np2_need = round_up((nch - 1) * vp.TPN2 * v.TN2 + vp.NCH2, 4);
+    vp.stg_floats = v.BK * std::max(vp.MC1, vp.NCH2);
+    const int NSL = std::max(1, v.NT / NC);
+    const int polish = 3 * H * 8 + 3 * NSL * NC * 16 + 3 * NC * 16 + 9 * NC * 8;
+    const int lower = std::max(v.raw_scratch_bytes(), polish);
+    const long avail = (long)SMEM_LIMIT - (long)v.fixed_smem() - (long)v.NSTG * vp.stg_floats * 4 - 32;
+    if (avail < lower) return false;
+    const int LDT = W + 4;
+    const int ms_cap = (int)(avail / ((long)LDT * 4));
+    if (ms_cap < 1) return false;
+    int nsb = 1, MS;
+    for (;; ++nsb) {
+        const int msb = (M + nsb - 1) / nsb;
+        MS = (msb + v.CS - 1) / v.CS;
+        if (MS <= ms_cap) break;
+    }
+    vp.MS = MS;
+    vp.nsb = (M + MS * v.CS - 1) / (MS * v.CS);
+    vp.u_bytes = round_up(std::max(lower, MS * LDT * 4), 16);
+    vp.smem_bytes = (int)v.fixed_smem() + vp.u_bytes + v.NSTG * vp.stg_floats * 4 + 32;
+    return vp.smem_bytes <= SMEM_LIMIT;
+}
+
+static cc_status check_device()
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(CC_ERR_ARCH, std::string("no CUDA device: ") + cudaGetErrorString(e));
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaDeviceGetAttribute");
+    if (major != 10) return fail(CC_ERR_ARCH, "device is not compute capability 10.x (sm_100a kernels only; no fallback)");
+    return CC_OK;
+}
+
+extern "C" cc_status cc_plan_destroy(cc_plan *plan)
+{
+    if (!plan) return CC_OK;
+    cudaFree(plan->tw), cudaFree(plan->Gt), cudaFree(plan->row_slot), cudaFree(plan->col_partner);
+    cudaFree(plan->ab), cudaFree(plan->Dt), cudaFree(plan->AxT);
+    cudaFree(plan->thr.Sg), cudaFree(plan->lat.Sg);
+    for (int i = 0; i < 2; ++i) {
+        if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
+        if (plan->hev[i]) cudaEventDestroy(plan->hev[i]);
+        cudaFree(plan->dframes[i]);
+    }
+    cudaFree(plan->dres);
+    delete plan;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype, int upsample, const float *reference)
+{
+    if (!out || !reference || H <= 0 || W <= 0 || upsample < 1 || (dtype != CC_U8 && dtype != CC_U16))
+        return fail(CC_ERR_INVALID_ARG, "cc_plan_create: bad argument");
+    if (upsample > 4096) return fail(CC_ERR_UNSUPPORTED, "upsample factor above 4096");
+    if (!is_pow2(H) || !is_pow2(W) || cc_radix(H, 0) == 0 || cc_radix(W, 0) == 0)
+        return fail(CC_ERR_UNSUPPORTED, "frame sides must be powers of two in 64..1024");
+    cc_status st = check_device();
+    if (st != CC_OK) return st;
+
+    cc_plan *pl = new (std::nothrow) cc_plan();
+    if (!pl) return fail(CC_ERR_NOMEM, "host allocation failed");
+    pl->H = H, pl->W = W, pl->u = upsample, pl->dtype = (int)dtype;
+    pl->M = (3 * upsample + 1) / 2;  // ceil(1.5 u)
+    pl->c = pl->M / 2;
+    const int M = pl->M, c = pl->c, u = upsample;
+
+    // ---- variants: smallest cluster = throughput variant, largest = small-batch (latency) variant
+    {
+        std::vector<VarPlan> fits;
+        for (cc_variant_fn fn : g_variant_fns) {
+            VarPlan vp;
+            vp.v = fn();
+            if (vp.v.H != H || vp.v.W != W || vp.v.dtype != (int)dtype) continue;
+            if (plan_variant(vp, M, W, H)) fits.push_back(vp);
+        }
+        if (fits.empty()) {
+            delete pl;
+            return fail(CC_ERR_UNSUPPORTED, "no kernel variant for this frame shape / pixel type");
+        }
+        std::sort(fits.begin(), fits.end(), [](const VarPlan &a, const VarPlan &b) { return a.v.CS < b.v.CS; });
+        pl->thr = fits.front();
+        if (fits.back().v.CS != fits.front().v.CS) pl->lat = fits.back(), pl->has_lat = true;
+    }
+
+    // ---- reference image to the host
+    std::vector<float> ref((size_t)H * W);
+    {
+        cudaError_t e = cudaMemcpy(ref.data(), reference, ref.size() * sizeof(float), cudaMemcpyDefault);
+        if (e != cudaSuccess) {
+            delete pl;
+            return fail_cuda(e, "copy of the reference image");
+        }
+    }
+
+    // ---- G = DFT2(E) in fp64 (row pass, column pass)
+    std::vector<std::complex<double>> G((size_t)H * W);
+    for (size_t i = 0; i < G.size(); ++i) G[i] = std::complex<double>((double)ref[i], 0.0);
+    {
+        const auto wW = unit_roots(W), wH = unit_roots(H);
+        for (int y = 0; y < H; ++y) fft1d(G, W, 1, (size_t)y * W, false, wW);
+        for (int x = 0; x < W; ++x) fft1d(G, H, W, (size_t)x, false, wH);
+    }
+    const double HW = (double)H * (double)W;
+    pl->Emean = G[0].real() / HW;
+    pl->c0 = (int)std::min(65535.0, std::max(0.0, nearbyint(pl->Emean)));
+
+    // ---- tables
+    const int NTW = std::max(H, W);
+    std::vector<float2> tw(NTW);
+    for (int j = 0; j < NTW; ++j) {
+        const double a = 2.0 * M_PI * (double)j / (double)NTW;
+        tw[j] = make_float2((float)cos(a), (float)(-sin(a)));
+    }
+    std::vector<uint16_t> row_slot(W), col_slot(H), col_partner(H);
+    for (int p = 0; p < W; ++p) row_slot[cc_freq_of_slot(W, p)] = (uint16_t)p;
+    for (int p = 0; p < H; ++p) col_slot[cc_freq_of_slot(H, p)] = (uint16_t)p;
+    for (int p = 0; p < H; ++p) col_partner[p] = col_slot[(H - cc_freq_of_slot(H, p)) % H];
+
+    const int Wh = W / 2;
+    std::vector<float2> Gt((size_t)H * Wh);
+    std::vector<float4> ab(H);
+    for (int p = 0; p < H; ++p) {
+        const int ky = cc_freq_of_slot(H, p);
+        for (int q = 1; q < Wh; ++q) {
+            const std::complex<double> g = std::conj(G[(size_t)ky * W + q]) / HW;
+            Gt[(size_t)p * Wh + q] = make_float2((float)g.real(), (float)g.imag());
+        }
+        Gt[(size_t)p * Wh] = make_float2(0.f, 0.f);
+        // packed column: DC bin of the reference zeroed (shift-independent constant; R10)
+        std::complex<double> g0 = (ky == 0) ? std::complex<double>(0.0, 0.0) : std::conj(G[(size_t)ky * W]) / HW;
+        std::complex<double> gn = std::conj(G[(size_t)ky * W + Wh]) / HW;
+        const std::complex<double> al = 0.5 * (g0 + gn), be = 0.5 * (g0 - gn);
+        ab[p] = make_float4((float)al.real(), (float)al.imag(), (float)be.real(), (float)be.imag());
+    }
+
+    int maxMC1 = pl->thr.MC1, np2 = pl->thr.np2_need;
+    if (pl->has_lat) maxMC1 = std::max(maxMC1, pl->lat.MC1), np2 = std::max(np2, pl->lat.np2_need);
+    pl->Mp1 = round_up(M, 4) + round_up(maxMC1, 4);
+    pl->Np2 = np2;
+    std::vector<float> Dt((size_t)H * pl->Mp1, 0.f), AxT((size_t)W * pl->Np2, 0.f);
+    if (u > 1) {
+        // Dt[j][m] = D_H((m - c)/u - j),  D_H(t) = sin(pi t) cot(pi t / H) / H   (Nyquist bin split half/half)
+        for (int j = 0; j < H; ++j)
+            for (int m = 0; m < M; ++m) {
+                const long long tnum = (long long)(m - c) - (long long)j * u;  // t = tnum / u
+                const long long den = (long long)u * H;
+                long long r = ((tnum % den) + den) % den;
+                double d;
+                if (r == 0) d = 1.0;
+                else {
+                    long long r2 = ((tnum % (2LL * u)) + 2LL * u) % (2LL * u);
+                    const double s1 = sin(M_PI * (double)r2 / (double)u);
+                    const double x = M_PI * (double)r / (double)den;
+                    d = (r2 == 0 || r2 == u) ? 0.0 : s1 * cos(x) / ((double)H * sin(x));
+                }
+                Dt[(size_t)j * pl->Mp1 + m] = (float)d;
+            }
+        // AxT[2q][n] = w_q cos(theta), AxT[2q+1][n] = -w_q sin(theta), theta = 2 pi q (n - c) / (u W);
+        // packed column q = 0: (1, cos(pi (n - c) / u))
+        const long long denx = (long long)u * W;
+        for (int n = 0; n < M; ++n) {
+            AxT[(size_t)0 * pl->Np2 + n] = 1.f;
+            long long r2 = (((long long)(n - c) % (2LL * u)) + 2LL * u) % (2LL * u);
+            AxT[(size_t)1 * pl->Np2 + n] = (float)cos(M_PI * (double)r2 / (double)u);
+            for (int q = 1; q < Wh; ++q) {
+                long long num = (((long long)q * (n - c)) % denx + denx) % denx;
+                const double th = 2.0 * M_PI * (double)num / (double)denx;
+                AxT[(size_t)(2 * q) * pl->Np2 + n] = (float)(2.0 * cos(th));
+                AxT[(size_t)(2 * q + 1) * pl->Np2 + n] = (float)(-2.0 * sin(th));
+            }
+        }
+    }
+
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = upload(&pl->tw, tw, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->row_slot, row_slot, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->col_partner, col_partner, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->Gt, Gt, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->ab, ab, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->Dt, Dt, &pl->table_bytes);
+    if (e == cudaSuccess) e = upload(&pl->AxT, AxT, &pl->table_bytes);
+
+    // ---- kernel attributes, occupancy, scratch
+    VarPlan *vps[2] = {&pl->thr, pl->has_lat ? &pl->lat : nullptr};
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        VarPlan *vp = vps[i];
+        if (!vp) continue;
+        e = vp->v.prepare(vp->smem_bytes);
+        if (e == cudaSuccess) e = vp->v.max_clusters(vp->smem_bytes, &vp->max_clusters);
+        if (e == cudaSuccess && vp->max_clusters < 1) {
+            cc_plan_destroy(pl);
+            return fail(CC_ERR_UNSUPPORTED, "kernel variant cannot be made resident (cluster occupancy 0)");
+        }
+        if (e == cudaSuccess && vp->v.s_global) {
+            vp->sg_bytes = (size_t)vp->max_clusters * vp->v.CS * ((size_t)H * (W / 2 / vp->v.CS)) * sizeof(float2);
+            e = cudaMalloc((void **)&vp->Sg, vp->sg_bytes);
+        }
+        vp->ready = (e == cudaSuccess);
+    }
+    if (e != cudaSuccess) {
+        cc_status s = (e == cudaErrorMemoryAllocation) ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "plan setup");
+        cc_plan_destroy(pl);
+        return s;
+    }
+    *out = pl;
+    return CC_OK;
+}
+
+static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
+{
+    p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
+    p.Dt = pl->Dt, p.AxT = pl->AxT, p.Sg = vp.Sg;
+    p.u = pl->u, p.M = pl->M, p.c = pl->c, p.Mp1 = pl->Mp1, p.Np2 = pl->Np2;
+    p.MS = vp.MS, p.nsb = vp.nsb, p.NCH2 = vp.NCH2, p.TPN2 = vp.TPN2;
+    p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.stg_floats = vp.stg_floats, p.Emean = pl->Emean;
+}
+
+extern "C" cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                                    int *iy, int *ix, void *stream)
+{
+    if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track: bad plan or batch");
+    if (batch == 0) return CC_OK;
+    if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track: null pointer");
+    if (((uintptr_t)frames & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_track: frames must be 16-byte aligned");
+    const VarPlan *vp = &plan->thr;
+    if (plan->has_lat && batch <= plan->lat.max_clusters && batch * plan->lat.v.CS <= plan->thr.max_clusters * plan->thr.v.CS)
+        vp = &plan->lat;
+    CcParams p{};
+    fill_params(plan, *vp, p);
+    p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix;
+    const int ncl = std::min(batch, vp->max_clusters);
+    cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
+    return CC_OK;
+}
+
+extern "C" cc_status cc_track(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                              void *stream)
+{
+    return cc_track_debug(plan, frames, batch, dx, dy, peak, nullptr, nullptr, stream);
+}
+
+extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak)
+{
+    if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_host: bad plan or batch");
+    if (batch == 0) return CC_OK;
+    if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track_host: null pointer");
+    const size_t fbytes = (size_t)plan->H * plan->W * (plan->dtype == CC_U8 ? 1 : 2);
+    // chunk: about 64 MB of frames, at least one wave of clusters
+    int chunk = (int)std::max<size_t>((size_t)plan->thr.max_clusters, (size_t)(64u << 20) / fbytes);
+    chunk = std::min(chunk, batch);
+    if (!plan->hs[0]) {
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaStreamCreateWithFlags(&plan->hs[i], cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&plan->hev[i], cudaEventDisableTiming));
+        }
+    }
+    if (chunk > plan->chunk_cap) {
+        for (int i = 0; i < 2; ++i) {
+            cudaFree(plan->dframes[i]);
+            plan->dframes[i] = nullptr;
+            CK(cudaMalloc(&plan->dframes[i], (size_t)chunk * fbytes));
+        }
+        plan->chunk_cap = chunk;
+    }
+    if (batch > plan->res_cap) {
+        cudaFree(plan->dres);
+        plan->dres = nullptr;
+        CK(cudaMalloc((void **)&plan->dres, (size_t)3 * batch * sizeof(float)));
+        plan->res_cap = batch;
+    }
+    float *ddx = plan->dres, *ddy = plan->dres + plan->res_cap, *dpk = plan->dres + 2 * (size_t)plan->res_cap;
+    int nchunks = (batch + chunk - 1) / chunk;
+    for (int ci = 0; ci < nchunks; ++ci) {
+        const int b = ci & 1, f0 = ci * chunk, n = std::min(chunk, batch - f0);
+        cudaStream_t s = plan->hs[b];
+        CK(cudaMemcpyAsync(plan->dframes[b], (const unsigned char *)frames + (size_t)f0 * fbytes, (size_t)n * fbytes,
+                           cudaMemcpyHostToDevice, s));
+        cc_status st = cc_track(plan, plan->dframes[b], n, ddx + f0, ddy + f0, dpk + f0, (void *)s);
+        if (st != CC_OK) return st;
+        CK(cudaMemcpyAsync(dx + f0, ddx + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(dy + f0, ddy + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+        if (peak) CK(cudaMemcpyAsync(peak + f0, dpk + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+    }
+    CK(cudaStreamSynchronize(plan->hs[0]));
+    CK(cudaStreamSynchronize(plan->hs[1]));
+    return CC_OK;
+}
+
+extern "C" cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info)
+{
+    if (!plan || !info) return fail(CC_ERR_INVALID_ARG, "cc_plan_info: null pointer");
+    memset(info, 0, sizeof(*info));
+    info->H = plan->H, info->W = plan->W, info->upsample = plan->u, info->dtype = plan->dtype, info->grid_M = plan->M;
+    info->cluster_size = plan->thr.v.CS, info->threads = plan->thr.v.NT, info->smem_bytes = plan->thr.smem_bytes;
+    info->max_clusters = plan->thr.max_clusters;
+    info->lat_cluster_size = plan->has_lat ? plan->lat.v.CS : 0;
+    info->lat_max_clusters = plan->has_lat ? plan->lat.max_clusters : 0;
+    info->scratch_bytes = (long long)(plan->thr.sg_bytes + (plan->has_lat ? plan->lat.sg_bytes : 0));
+    info->table_bytes = (long long)plan->table_bytes;
+    return CC_OK;
+}
+
+// ------------------------------------------------------------------ FP32 peak probe
+__global__ void __launch_bounds__(1024, 1) cc_ffma_probe_kernel(float *out, int iters)
+{
+    float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f,
+          a7 = a0 + 7.f;
+    const float b = 0.999f, c = 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            a0 = fmaf(a0, b, c), a1 = fmaf(a1, b, c), a2 = fmaf(a2, b, c), a3 = fmaf(a3, b, c);
+            a4 = fmaf(a4, b, c), a5 = fmaf(a5, b, c), a6 = fmaf(a6, b, c), a7 = fmaf(a7, b, c);
+        }
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+}
+
+extern "C" cc_status cc_fp32_peak_probe(double *tflops, void *stream)
+{
+    if (!tflops) return fail(CC_ERR_INVALID_ARG, "cc_fp32_peak_probe: null pointer");
+    cc_status st = check_device();
+    if (st != CC_OK) return st;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 2, threads = 1024, iters = 4096;
+    float *out = nullptr;
+    CK(cudaMalloc((void **)&out, (size_t)blocks * threads * sizeof(float)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    cudaStream_t s = (cudaStream_t)stream;
+    cc_ffma_probe_kernel<<<blocks, threads, 0, s>>>(out, 64);
+    float best = 1e30f;
+    for (int r = 0; r < 3; ++r) {
+        CK(cudaEventRecord(e0, s));
+        cc_ffma_probe_kernel<<<blocks, threads, 0, s>>>(out, iters);
+        CK(cudaEventRecord(e1, s));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        best = std::min(best, ms);
+    }
+    cudaEventDestroy(e0), cudaEventDestroy(e1), cudaFree(out);
+    const double flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)blocks * (double)threads;
+    *tflops = flops / ((double)best * 1e-3) / 1e12;
+    return CC_OK;
+}
+
+extern "C" const char *cc_status_string(cc_status s)
+{
+    switch (s) {
+        case CC_OK: return "CC_OK";
+        case CC_ERR_INVALID_ARG: return "CC_ERR_INVALID_ARG";
+        case CC_ERR_UNSUPPORTED: return "CC_ERR_UNSUPPORTED";
+        case CC_ERR_NOMEM: return "CC_ERR_NOMEM";
+        case CC_ERR_CUDA: return "CC_ERR_CUDA";
+        case CC_ERR_ARCH: return "CC_ERR_ARCH";
+    }
+    return "CC_ERR_UNKNOWN";
+}
+
+extern "C" const char *cc_last_error(void) { return g_err.c_str(); }

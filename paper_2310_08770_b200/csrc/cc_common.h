@@ -1,0 +1,78 @@
+// cc_common.h -- definitions shared by the host plan code (cc_api.cu) and the
+// fused device kernel (cc_fused.cuh).  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+// Mixed-radix decomposition of the in-place FFTs (forward = decimation in
+// frequency, natural order in -> "slot" order out; inverse = the transpose,
+// slot order in -> natural order out).  N = r[0]*r[1]*r[2].
+__host__ __device__ constexpr int cc_radix(int N, int p)
+{
+    return N == 64   ? (p == 0 ? 8 : p == 1 ? 8 : 1)
+         : N == 128  ? (p == 0 ? 16 : p == 1 ? 8 : 1)
+         : N == 256  ? (p == 0 ? 16 : p == 1 ? 16 : 1)
+         : N == 512  ? (p == 0 ? 8 : p == 1 ? 8 : 8)
+         : N == 1024 ? (p == 0 ? 16 : p == 1 ? 8 : 8)
+                     : 0;
+}
+
+// Frequency held by slot p after the forward FFT of length N:
+// p = k1*(N/r0) + k2*(N/(r0 r1)) + k3  <->  k = k1 + r0*k2 + r0*r1*k3.
+static inline int cc_freq_of_slot(int N, int p)
+{
+    int k = 0, mult = 1, L = N, rem = p;
+    for (int i = 0; i < 3; ++i) {
+        int r = cc_radix(N, i);
+        if (r <= 1) break;
+        L /= r;
+        int d = rem / L;
+        rem %= L;
+        k += d * mult;
+        mult *= r;
+    }
+    return k;
+}
+
+// Kernel parameters (passed by value).  All table pointers are device memory
+// owned by the plan.
+struct CcParams {
+    const void *frames;  // batch * H * W pixels
+    int batch;
+    float *dx, *dy, *peak;  // peak may be null
+    int *iy, *ix;           // may be null
+
+    const float2 *tw;             // [NTW] (cos, -sin)(2 pi j / NTW), NTW = max(H, W)
+    const uint16_t *row_slot;     // [W] slot holding row frequency k
+    const float2 *Gt;             // [H][W/2]: conj(G[ky(p)][q]) / (H W), p = column slot; q = 0 unused
+    const float4 *ab;             // [H]: (alpha, beta) of the packed DC/Nyquist column, by slot
+    const uint16_t *col_partner;  // [H]: slot of -ky for the frequency at slot p
+    const float *Dt;              // [H][Mp1]: Dirichlet interpolation matrix, j-major
+    const float *AxT;             // [W][Np2]: x-axis upsampling matrix, k-major (re, -im interleaved along k)
+    float2 *Sg;                   // global spectrum scratch (variants with S in L2), else null
+
+    int u, M, c;  // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
+    int Mp1;      // padded row length of Dt
+    int Np2;      // padded row length of AxT
+    int MS;       // rows of T held per CTA per super-block
+    int nsb;      // number of super-blocks
+    int NCH2;     // staged width (floats) of an AxT tile
+    int TPN2;     // threads across n in stage 2
+    int c0;       // integer constant subtracted from every pixel before the FFT
+    int u_bytes;  // bytes of the raw/scratch/T union region
+    int stg_floats;  // floats per staging buffer
+    double Emean;    // mean of the reference image (DC add-back for `peak`)
+};
+
+// Launcher interface of one compiled kernel variant.
+struct CcVariant {
+    int H, W, CS, NT, dtype;  // dtype: 0 = u8, 1 = u16
+    int TM1, TN1, TM2, TN2;
+    int s_global;  // 1: spectrum array lives in global memory (L2), 0: shared memory / DSMEM
+    int BK, NSTG;
+    size_t (*fixed_smem)();                 // bytes that do not depend on M (S, tables, misc), before U/stg
+    int (*raw_scratch_bytes)();             // raw ring + FFT scratch (lower bound of the U region)
+    cudaError_t (*prepare)(int smem_bytes);  // sets func attributes
+    cudaError_t (*max_clusters)(int smem_bytes, int *n);
+    cudaError_t (*launch)(const CcParams &p, int n_clusters, int smem_bytes, cudaStream_t st);
+};

@@ -1,0 +1,969 @@
+// cc_fused.cuh -- the fused per-frame displacement kernel for sm_100a.
+//
+// One thread-block cluster of CS CTAs processes one frame at a time
+// (persistent over the batch).  Steps (PAPER.md citations in
+// include/cc.h and DESIGN.md):
+//   a1 ingest    : cp.async.bulk (TMA) of raw u8/u16 rows into shared memory
+//   a2 fwd FFT   : two real rows per complex row FFT (per warp), results
+//                  scattered to the column owners through DSMEM; column FFT
+//   a3 product   : fused into the last forward / first inverse column pass
+//   a4 inv FFT   : column inverse -> Q[y][kx] (kept: it feeds a6), row C2R
+//   a5 argmax    : streamed out of the row C2R, never stored; fp64 3x3 polish
+//   a6 upsampled : stage 1  T = D(real Dirichlet) * Q      (FP32 register-tiled GEMM)
+//                  stage 2  C = T' * AxT                   (FP32 register-tiled GEMM)
+//   a7 argmax    : streamed out of stage 2, fp64 3x3 hill-climb polish, compose
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "cc_common.h"
+
+namespace ccf {
+namespace cg = cooperative_groups;
+
+constexpr int BK = 8;     // k-depth of a staged GEMM tile
+constexpr int NSTG = 3;   // staging ring depth
+constexpr int XN = 10;    // doubles per cluster-exchange record
+constexpr int NBARS = NSTG + 2;
+
+// ------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *b, uint32_t cnt)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(cnt) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity)
+{
+    uint32_t ok;
+    const uint32_t a = smem_u32(b);
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(ok)
+            : "r"(a), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+// TMA 1D bulk copy global -> shared, completion on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+// ------------------------------------------------------------------ small complex helpers
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a*conj(b)
+
+__device__ __forceinline__ float c16(int t)  // cos(2 pi t / 16)
+{
+    switch (t & 15) {
+        case 0: return 1.f;
+        case 1: return 0.92387953251128674f;
+        case 2: return 0.70710678118654752f;
+        case 3: return 0.38268343236508977f;
+        case 4: return 0.f;
+        case 5: return -0.38268343236508977f;
+        case 6: return -0.70710678118654752f;
+        case 7: return -0.92387953251128674f;
+        case 8: return -1.f;
+        case 9: return -0.92387953251128674f;
+        case 10: return -0.70710678118654752f;
+        case 11: return -0.38268343236508977f;
+        case 12: return 0.f;
+        case 13: return 0.38268343236508977f;
+        case 14: return 0.70710678118654752f;
+        default: return 0.92387953251128674f;
+    }
+}
+__device__ __forceinline__ float s16(int t) { return c16(t - 4); }  // sin(2 pi t / 16)
+
+__host__ __device__ constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
+__host__ __device__ constexpr int brev(int k, int bits)
+{
+    int r = 0;
+    for (int i = 0; i < bits; ++i) r |= ((k >> i) & 1) << (bits - 1 - i);
+    return r;
+}
+
+// In-register DFT of size R (2..16) by radix-2 DIF stages; X[k] ends up in
+// v[brev(k)].  INV selects exp(+i...).  Fully unrolled: all twiddles are
+// compile-time constants.
+template <int R, bool INV>
+__device__ __forceinline__ void dft_reg(float2 (&v)[R])
+{
+#pragma unroll
+    for (int span = R / 2; span >= 1; span >>= 1) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            if ((i & span) == 0) {
+                const int j = i | span;
+                const float2 a = v[i], b = v[j];
+                v[i] = make_float2(a.x + b.x, a.y + b.y);
+                const float2 d = make_float2(a.x - b.x, a.y - b.y);
+                const int t16 = (i & (span - 1)) * (8 / span);  // twiddle angle in units of 2 pi / 16
+                if (t16 == 0) {
+                    v[j] = d;
+                } else if (t16 == 4) {
+                    v[j] = INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);
+                } else {
+                    const float c = c16(t16), s = s16(t16);
+                    v[j] = INV ? make_float2(d.x * c - d.y * s, d.y * c + d.x * s)
+                               : make_float2(d.x * c + d.y * s, d.y * c - d.x * s);
+                }
+            }
+        }
+    }
+}
+
+// One radix-R butterfly of an in-place FFT pass.  addr(i) -> float2* of the
+// i-th element.  Forward (DIF): DFT then twiddle w^(k*twstep); inverse (DIT):
+// conj twiddle w^(i*twstep) then inverse DFT.  tw[j] = (cos, -sin)(2 pi j / NTW).
+template <int R, bool INV, bool TW, int NTW, class Addr>
+__device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw)
+{
+    float2 v[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) v[i] = *addr(i);
+    if (INV && TW) {
+#pragma unroll
+        for (int i = 1; i < R; ++i) v[i] = cmulc(v[i], tw[(i * twstep) & (NTW - 1)]);
+    }
+    dft_reg<R, INV>(v);
+    constexpr int bits = ilog2c(R);
+#pragma unroll
+    for (int k = 0; k < R; ++k) {
+        float2 o = v[brev(k, bits)];
+        if (!INV && TW && k > 0) o = cmul(o, tw[(k * twstep) & (NTW - 1)]);
+        *addr(k) = o;
+    }
+}
+
+__device__ __forceinline__ int padi(int i) { return i + (i >> 4); }  // 1 float2 of padding per 16
+
+// One pass (sub-FFT length L, radix R) of a length-N FFT held by one warp in a
+// padded scratch row.
+template <int N, int L, int R, bool INV, int NTW>
+__device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *tw, int lane)
+{
+    constexpr int ST = L / R;
+    for (int g = lane; g < N / R; g += 32) {
+        const int blk = g / ST, b = g % ST;
+        const int base = blk * L + b;
+        fft_bfly<R, INV, (ST > 1), NTW>([&](int i) { return sc + padi(base + i * ST); }, b * (NTW / L), tw);
+    }
+    __syncwarp();
+}
+
+template <int N, bool INV, int NTW>
+__device__ __forceinline__ void warp_fft(float2 *sc, const float2 *tw, int lane)
+{
+    constexpr int R0 = cc_radix(N, 0), R1 = cc_radix(N, 1), R2 = cc_radix(N, 2);
+    if (!INV) {
+        warp_fft_pass<N, N, R0, false, NTW>(sc, tw, lane);
+        warp_fft_pass<N, N / R0, R1, false, NTW>(sc, tw, lane);
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, NTW>(sc, tw, lane);
+    } else {
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, NTW>(sc, tw, lane);
+        warp_fft_pass<N, N / R0, R1, true, NTW>(sc, tw, lane);
+        warp_fft_pass<N, N, R0, true, NTW>(sc, tw, lane);
+    }
+}
+
+// argmax record: larger value wins; equal values -> smaller index wins.
+struct Best {
+    float v;
+    int i;
+};
+__device__ __forceinline__ bool better(float v1, int i1, float v2, int i2) { return v1 > v2 || (v1 == v2 && i1 < i2); }
+__device__ __forceinline__ Best warp_best(Best b)
+{
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        const float v = __shfl_xor_sync(0xffffffffu, b.v, o);
+        const int i = __shfl_xor_sync(0xffffffffu, b.i, o);
+        if (better(v, i, b.v, b.i)) {
+            b.v = v;
+            b.i = i;
+        }
+    }
+    return b;
+}
+
+template <int n>
+__device__ __forceinline__ void load_vec(float (&d)[n], const float *s)
+{
+    if constexpr (n % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < n / 4; ++i) {
+            const float4 t = reinterpret_cast<const float4 *>(s)[i];
+            d[4 * i] = t.x, d[4 * i + 1] = t.y, d[4 * i + 2] = t.z, d[4 * i + 3] = t.w;
+        }
+    } else if constexpr (n % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < n / 2; ++i) {
+            const float2 t = reinterpret_cast<const float2 *>(s)[i];
+            d[2 * i] = t.x, d[2 * i + 1] = t.y;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < n; ++i) d[i] = s[i];
+    }
+}
+
+// fp64 periodic-sinc (Dirichlet) interpolation weight of the even-length DFT
+// with the Nyquist bin split half/half:  D_H(t) = sin(pi t) cot(pi t / H) / H,
+// t = tnum / u.
+__device__ __forceinline__ double dirichlet64(long long tnum, int u, int Hn)
+{
+    const long long den = (long long)u * Hn;
+    long long r = tnum % den;
+    if (r < 0) r += den;
+    if (r == 0) return 1.0;
+    long long r2 = tnum % (2LL * u);
+    if (r2 < 0) r2 += 2LL * u;
+    const double s1 = sinpi((double)r2 / (double)u);
+    const double x = (double)r / (double)den;  // in (0, 1)
+    return s1 * cospi(x) / ((double)Hn * sinpi(x));
+}
+
+// ------------------------------------------------------------------ the kernel
+template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_>
+struct Cfg {
+    static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
+    static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
+    static constexpr bool SG = SG_;
+    using PIX = PIX_;
+    static constexpr int NC = W / 2 / CS;   // spectrum columns per CTA (column 0 of rank 0 packs DC + Nyquist)
+    static constexpr int NR = H / CS;       // frame rows per CTA
+    static constexpr int NWARP = NT / 32;
+    static constexpr int NTW = H > W ? H : W;
+    static constexpr int PADW = W + W / 16;
+    static constexpr int rch0 = 16384 / (W * (int)sizeof(PIX));
+    static constexpr int rch1 = rch0 > 2 * NWARP ? rch0 : 2 * NWARP;
+    static constexpr int RCH = NR < rch1 ? NR : rch1;  // rows per raw chunk
+    static constexpr int NCHK = NR / RCH;
+    static constexpr int CHB = RCH * W * (int)sizeof(PIX);
+    static constexpr int RAWB = (NCHK > 1 ? 2 : 1) * CHB;
+    static constexpr int SCRB = NWARP * PADW * 8;
+    static constexpr int TPN1 = 2 * NC / TN1;
+    static constexpr int TPM1 = NT / TPN1;
+    static constexpr int MC1 = TPM1 * TM1;
+    static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
+    static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
+    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64;
+    static constexpr size_t FIXED_BYTES = S_BYTES + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES;
+    static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
+    static_assert(NR % RCH == 0 && RCH % 2 == 0, "bad raw chunking");
+    static_assert((2 * NC) % TN1 == 0 && NT % TPN1 == 0 && TN1 % 2 == 0 && MC1 % 4 == 0, "bad stage-1 tiling");
+    static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
+};
+
+template <class C>
+__global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
+{
+    constexpr int H = C::H, W = C::W, CS = C::CS, NT = C::NT, NC = C::NC, NR = C::NR;
+    constexpr int NWARP = C::NWARP, NTW = C::NTW, PADW = C::PADW;
+    constexpr int TM1 = C::TM1, TN1 = C::TN1, TM2 = C::TM2, TN2 = C::TN2;
+    constexpr int LDT = C::LDT;
+    constexpr bool SG = C::SG;
+    using PIX = typename C::PIX;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (CS > 1) ? (int)cluster.block_rank() : 0;
+    const int cid = blockIdx.x / CS, ncl = gridDim.x / CS;
+
+    // ---- shared memory carve-up
+    float2 *const Ssm = reinterpret_cast<float2 *>(smem);
+    unsigned char *const U = smem + C::S_BYTES;
+    float *const stg = reinterpret_cast<float *>(U + p.u_bytes);
+    float2 *const tw = reinterpret_cast<float2 *>(stg + NSTG * p.stg_floats);
+    uint16_t *const rslot = reinterpret_cast<uint16_t *>(tw + NTW);
+    unsigned char *misc = reinterpret_cast<unsigned char *>(rslot + W);
+    misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
+    uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // [NSTG] staging, [NSTG..NSTG+1] raw ring
+    double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
+    double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
+    float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
+    int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
+    float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
+
+    PIX *const raw = reinterpret_cast<PIX *>(U);
+    float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
+    float *const Tb = reinterpret_cast<float *>(U);
+
+    // local spectrum block S[y][ql], y in [0,H), ql in [0,NC)
+    float2 *const Sl = SG ? p.Sg + ((size_t)cid * CS + rank) * ((size_t)H * NC) : Ssm;
+    auto Sof = [&](int r) -> float2 * {
+        if constexpr (SG) return p.Sg + ((size_t)cid * CS + r) * ((size_t)H * NC);
+        if constexpr (CS > 1) return cluster.map_shared_rank(Ssm, r);
+        return Ssm;
+    };
+    auto csync = [&]() {
+        if constexpr (CS > 1) cluster.sync();
+        else __syncthreads();
+    };
+
+    // ---- one-time setup
+    for (int i = tid; i < NTW; i += NT) tw[i] = p.tw[i];
+    for (int i = tid; i < W; i += NT) rslot[i] = p.row_slot[i];
+    if (tid == 0) {
+        for (int i = 0; i < NBARS; ++i) mbar_init(&bars[i], 1);
+        fence_mbar_init();
+    }
+    uint32_t ph = 0;   // mbarrier phase parity bits, one per barrier
+    int xpar = 0;      // exchange buffer parity
+    csync();
+
+    const int u = p.u, M = p.M, cM = p.c;
+
+    // cluster-wide exchange of xsrc[0..n): after the call xchg[par][r][k] holds rank r's record
+    auto exchange = [&](int n) -> const double * {
+        __syncthreads();
+        if (tid < CS * n) {
+            const int r = tid / n, k = tid % n;
+            double *dst = xchg + ((size_t)xpar * CS + rank) * XN + k;
+            if constexpr (CS > 1) dst = cluster.map_shared_rank(dst, r);
+            *dst = xsrc[k];
+        }
+        csync();
+        const double *res = xchg + (size_t)xpar * CS * XN;
+        xpar ^= 1;
+        return res;
+    };
+    // block-wide argmax; result valid in thread 0
+    auto block_best = [&](Best b) -> Best {
+        b = warp_best(b);
+        if (lane == 0) {
+            wv[warp] = b.v;
+            wi[warp] = b.i;
+        }
+        __syncthreads();
+        Best r = b;
+        if (tid == 0) {
+            r.v = wv[0];
+            r.i = wi[0];
+            for (int w = 1; w < NWARP; ++w)
+                if (better(wv[w], wi[w], r.v, r.i)) {
+                    r.v = wv[w];
+                    r.i = wi[w];
+                }
+        }
+        return r;
+    };
+
+    // staged GEMM operand tiles: BK rows of `rowlen` floats, row r of tile t at src + (t*BK + r)*ld
+    auto stage_issue = [&](int slot, const float *src, int t, int ld, int rowlen) {
+        // called by thread 0 only
+        mbar_expect_tx(&bars[slot], (uint32_t)(BK * rowlen * 4));
+        float *dst = stg + (size_t)slot * p.stg_floats;
+        if (ld == rowlen) {
+            bulk_g2s(dst, src + (size_t)t * BK * ld, (uint32_t)(BK * rowlen * 4), &bars[slot]);
+        } else {
+            for (int r = 0; r < BK; ++r)
+                bulk_g2s(dst + r * rowlen, src + ((size_t)t * BK + r) * ld, (uint32_t)(rowlen * 4), &bars[slot]);
+        }
+    };
+    auto bar_wait = [&](int b) {
+        mbar_wait(&bars[b], (ph >> b) & 1u);
+        ph ^= 1u << b;
+    };
+
+    // 3x3 evaluation in fp64 of  sum_q w_q Re( R[a][q] * exp(2 pi i q xnum[b] / den) )  over this
+    // CTA's columns, summed over the cluster in rank order.  R64[a][ql] (double2) in shared memory;
+    // packed column (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b] = cos(pi * x_b).
+    // Scratch `terms` = double[9][NC].  Result: out[a*3+b] valid in all threads of all CTAs.
+    auto xeval9 = [&](const double2 *R64, const long long *xnum, long long den, const double *nyq_c, double *terms,
+                      double *out) {
+        for (int e = tid; e < 3 * NC; e += NT) {
+            const int b = e / NC, ql = e % NC;
+            const int q = rank * NC + ql;
+            double cs, sn, w;
+            if (q == 0) {
+                cs = 1.0, sn = 0.0, w = 1.0;
+            } else {
+                long long num = ((long long)q * xnum[b]) % den;
+                if (num < 0) num += den;
+                sincospi(2.0 * (double)num / (double)den, &sn, &cs);
+                w = 2.0;
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const double2 r = R64[a * NC + ql];
+                double t;
+                if (q == 0) t = r.x + r.y * nyq_c[b];
+                else t = w * (r.x * cs - r.y * sn);
+                terms[(a * 3 + b) * NC + ql] = t;
+            }
+        }
+        __syncthreads();
+        if (tid < 9) {
+            double s = 0.0;
+            for (int ql = 0; ql < NC; ++ql) s += terms[tid * NC + ql];
+            xsrc[tid] = s;
+        }
+        const double *res = exchange(9);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+            double s = 0.0;
+            for (int r = 0; r < CS; ++r) s += res[r * XN + k];
+            out[k] = s;
+        }
+    };
+
+    for (int f = cid; f < p.batch; f += ncl) {
+        // =============================================================== a1 + a2: ingest and row FFTs
+        {
+            const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
+            if (tid == 0) {
+                fence_proxy_async();
+                for (int ck = 0; ck < (C::NCHK > 1 ? 2 : 1); ++ck) {
+                    mbar_expect_tx(&bars[NSTG + ck], C::CHB);
+                    bulk_g2s(raw + (size_t)ck * C::RCH * W, fbase + (size_t)ck * C::RCH * W, C::CHB, &bars[NSTG + ck]);
+                }
+                if (f + ncl < p.batch) {  // pull the next frame of this cluster into L2
+                    const PIX *nb = fbase + (size_t)ncl * H * W;
+                    constexpr uint32_t tot = (uint32_t)NR * W * sizeof(PIX);
+                    for (uint32_t o = 0; o < tot; o += 32768u)
+                        bulk_prefetch_l2(reinterpret_cast<const unsigned char *>(nb) + o, tot - o < 32768u ? tot - o : 32768u);
+                }
+            }
+            const float c0f = (float)p.c0;
+            for (int ck = 0; ck < C::NCHK; ++ck) {
+                const int rb = ck & 1;
+                bar_wait(NSTG + rb);
+                const PIX *rw = raw + (size_t)rb * C::RCH * W;
+                for (int jp = warp; jp < C::RCH / 2; jp += NWARP) {
+                    const PIX *ra = rw + (size_t)jp * W;
+                    const PIX *rbp = rw + (size_t)(jp + C::RCH / 2) * W;
+                    for (int x = lane; x < W; x += 32)
+                        scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
+                    __syncwarp();
+                    warp_fft<W, false, NTW>(scr, tw, lane);
+                    // untangle the two real rows and scatter to the column owners
+                    const int ya = rank * NR + ck * C::RCH + jp, yb = ya + C::RCH / 2;
+                    for (int k = lane; k < W / 2; k += 32) {
+                        float2 A, B;
+                        if (k == 0) {
+                            const float2 z0 = scr[padi(rslot[0])], zn = scr[padi(rslot[W / 2])];
+                            A = make_float2(z0.x, zn.x);
+                            B = make_float2(z0.y, zn.y);
+                        } else {
+                            const float2 z1 = scr[padi(rslot[k])], z2 = scr[padi(rslot[W - k])];
+                            A = make_float2(0.5f * (z1.x + z2.x), 0.5f * (z1.y - z2.y));
+                            B = make_float2(0.5f * (z1.y + z2.y), -0.5f * (z1.x - z2.x));
+                        }
+                        float2 *Sd = Sof(k / NC);
+                        Sd[(size_t)ya * NC + (k % NC)] = A;
+                        Sd[(size_t)yb * NC + (k % NC)] = B;
+                    }
+                    __syncwarp();
+                }
+                __syncthreads();
+                if (tid == 0 && ck + 2 < C::NCHK) {
+                    mbar_expect_tx(&bars[NSTG + rb], C::CHB);
+                    bulk_g2s(raw + (size_t)rb * C::RCH * W, fbase + (size_t)(ck + 2) * C::RCH * W, C::CHB, &bars[NSTG + rb]);
+                }
+            }
+        }
+        csync();  // every F_row[y][kx] is at its column owner
+
+        // =============================================================== a2/a3/a4: column FFT (x) Gc, column inverse
+        {
+            constexpr int R0 = cc_radix(H, 0), R1 = cc_radix(H, 1), R2 = cc_radix(H, 2);
+            constexpr int RL = R2 > 1 ? R2 : R1;   // radix of the last forward pass (fused with the product)
+            constexpr int NPASS = R2 > 1 ? 3 : 2;
+            // forward pass 0
+            for (int it = tid; it < NC * (H / R0); it += NT) {
+                const int ql = it % NC, g = it / NC;
+                constexpr int ST = H / R0;
+                fft_bfly<R0, false, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
+            }
+            __syncthreads();
+            if constexpr (NPASS == 3) {  // forward pass 1 of 3
+                constexpr int L = H / R0, ST = L / R1;
+                for (int it = tid; it < NC * (H / R1); it += NT) {
+                    const int ql = it % NC, g = it / NC;
+                    const int blk = g / ST, b = g % ST;
+                    fft_bfly<R1, false, true, NTW>([&](int i) { return Sl + (size_t)(blk * L + b + i * ST) * NC + ql; },
+                                                   b * (NTW / L), tw);
+                }
+                __syncthreads();
+            }
+            // last forward pass (contiguous slots), product with conj(G)/(HW), first inverse pass
+            for (int it = tid; it < NC * (H / RL); it += NT) {
+                const int ql = it % NC, g = it / NC;
+                const int q = rank * NC + ql;
+                float2 v[RL];
+#pragma unroll
+                for (int i = 0; i < RL; ++i) v[i] = Sl[(size_t)(g * RL + i) * NC + ql];
+                dft_reg<RL, false>(v);
+                constexpr int bits = ilog2c(RL);
+                if (q == 0) {  // packed DC/Nyquist column: needs the -ky partner, handled below
+#pragma unroll
+                    for (int k = 0; k < RL; ++k) Sl[(size_t)(g * RL + k) * NC + ql] = v[brev(k, bits)];
+                } else {
+                    float2 w[RL];
+#pragma unroll
+                    for (int k = 0; k < RL; ++k) w[k] = cmul(v[brev(k, bits)], __ldg(&p.Gt[(size_t)(g * RL + k) * (W / 2) + q]));
+                    dft_reg<RL, true>(w);
+#pragma unroll
+                    for (int n = 0; n < RL; ++n) Sl[(size_t)(g * RL + n) * NC + ql] = w[brev(n, bits)];
+                }
+            }
+            __syncthreads();
+            if (rank == 0) {
+                // P'[p] = alpha[p] Z[p] + beta[p] conj(Z[partner(p)])   (two real columns in one complex FFT)
+                constexpr int PER = (H + NT - 1) / NT;
+                float2 o[PER];
+#pragma unroll
+                for (int e = 0; e < PER; ++e) {
+                    const int s = tid + e * NT;
+                    if (s < H) {
+                        const float2 z = Sl[(size_t)s * NC], zp = Sl[(size_t)p.col_partner[s] * NC];
+                        const float4 ab = p.ab[s];
+                        o[e] = make_float2(ab.x * z.x - ab.y * z.y + ab.z * zp.x + ab.w * zp.y,
+                                           ab.x * z.y + ab.y * z.x - ab.z * zp.y + ab.w * zp.x);
+                        if (s == 0) *f00 = z.x;  // sum of (I - c0): DC add-back for `peak`
+                    }
+                }
+                __syncthreads();
+#pragma unroll
+                for (int e = 0; e < PER; ++e) {
+                    const int s = tid + e * NT;
+                    if (s < H) Sl[(size_t)s * NC] = o[e];
+                }
+                __syncthreads();
+                for (int g = tid; g < H / RL; g += NT)
+                    fft_bfly<RL, true, false, NTW>([&](int i) { return Sl + (size_t)(g * RL + i) * NC; }, 0, tw);
+                __syncthreads();
+            }
+            if constexpr (NPASS == 3) {  // inverse of forward pass 1
+                constexpr int L = H / R0, ST = L / R1;
+                for (int it = tid; it < NC * (H / R1); it += NT) {
+                    const int ql = it % NC, g = it / NC;
+                    const int blk = g / ST, b = g % ST;
+                    fft_bfly<R1, true, true, NTW>([&](int i) { return Sl + (size_t)(blk * L + b + i * ST) * NC + ql; },
+                                                  b * (NTW / L), tw);
+                }
+                __syncthreads();
+            }
+            for (int it = tid; it < NC * (H / R0); it += NT) {
+                const int ql = it % NC, g = it / NC;
+                constexpr int ST = H / R0;
+                fft_bfly<R0, true, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
+            }
+        }
+        csync();  // Q[y][kx] complete everywhere
+
+        // =============================================================== a4/a5: row C2R streamed into the integer argmax
+        int y0, x0;
+        double cc_peak = 0.0;
+        {
+            Best bst{-INFINITY, 0x7fffffff};
+            for (int jp = warp; jp < NR / 2; jp += NWARP) {
+                const int ya = rank * NR + jp, yb = ya + NR / 2;
+                for (int k = lane; k < W / 2; k += 32) {
+                    const float2 *Sd = Sof(k / NC);
+                    const float2 qa = Sd[(size_t)ya * NC + (k % NC)], qb = Sd[(size_t)yb * NC + (k % NC)];
+                    if (k == 0) {
+                        scr[padi(rslot[0])] = make_float2(qa.x, qb.x);
+                        scr[padi(rslot[W / 2])] = make_float2(qa.y, qb.y);
+                    } else {
+                        scr[padi(rslot[k])] = make_float2(qa.x - qb.y, qa.y + qb.x);
+                        scr[padi(rslot[W - k])] = make_float2(qa.x + qb.y, qb.x - qa.y);
+                    }
+                }
+                __syncwarp();
+                warp_fft<W, true, NTW>(scr, tw, lane);
+                for (int x = lane; x < W; x += 32) {
+                    const float2 z = scr[padi(x)];
+                    if (better(z.x, ya * W + x, bst.v, bst.i)) bst.v = z.x, bst.i = ya * W + x;
+                    if (better(z.y, yb * W + x, bst.v, bst.i)) bst.v = z.y, bst.i = yb * W + x;
+                }
+                __syncwarp();
+            }
+            bst = block_best(bst);
+            if (tid == 0) {
+                xsrc[0] = (double)bst.v;
+                xsrc[1] = (double)bst.i;
+            }
+            const double *res = exchange(2);
+            Best g{(float)res[0], (int)res[1]};
+            for (int r = 1; r < CS; ++r) {
+                const float v = (float)res[r * XN];
+                const int i = (int)res[r * XN + 1];
+                if (better(v, i, g.v, g.i)) g.v = v, g.i = i;
+            }
+            y0 = g.i / W;
+            x0 = g.i % W;
+
+            // fp64 re-evaluation of the 3x3 neighbourhood of the fp32 winner
+            double2 *R64 = reinterpret_cast<double2 *>(U);
+            double *terms = reinterpret_cast<double *>(R64 + 3 * NC);
+            for (int e = tid; e < 3 * NC; e += NT) {
+                const int a = e / NC, ql = e % NC;
+                const float2 v = Sl[(size_t)((y0 - 1 + a) & (H - 1)) * NC + ql];
+                R64[e] = make_double2((double)v.x, (double)v.y);
+            }
+            long long xnum[3];
+            double nyq[3], c9[9];
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const int xx = (x0 - 1 + b) & (W - 1);
+                xnum[b] = xx;
+                nyq[b] = (xx & 1) ? -1.0 : 1.0;
+            }
+            __syncthreads();
+            xeval9(R64, xnum, (long long)W, nyq, terms, c9);
+            double bv = -INFINITY;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    const int yy = (y0 - 1 + a) & (H - 1), xx = (x0 - 1 + b) & (W - 1);
+                    const int idx = yy * W + xx;
+                    const double v = c9[a * 3 + b];
+                    if (v > bv || (v == bv && idx < bi)) bv = v, bi = idx;
+                }
+            y0 = bi / W;
+            x0 = bi % W;
+            cc_peak = bv;
+        }
+        const int wy = (2 * y0 >= H) ? y0 - H : y0;
+        const int wx = (2 * x0 >= W) ? x0 - W : x0;
+
+        if (u == 1) {
+            if (rank == 0 && tid == 0) {
+                p.dy[f] = (float)wy;
+                p.dx[f] = (float)wx;
+                if (p.peak) p.peak[f] = (float)(cc_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean);
+                if (p.iy) p.iy[f] = wy;
+                if (p.ix) p.ix[f] = wx;
+            }
+            csync();
+            continue;
+        }
+
+        // =============================================================== a6/a7: upsampled DFT as two FP32 GEMMs
+        Best sub{-INFINITY, 0x7fffffff};
+        {
+            const int MS = p.MS, MSB = MS * CS;
+            constexpr int TPN1 = C::TPN1, MC1 = C::MC1;
+            const int tn1 = tid % TPN1, tm1 = tid / TPN1;
+            const int TPN2 = p.TPN2, TPM2 = NT / TPN2, NCH2 = p.NCH2;
+            const int tn2 = tid % TPN2, tm2 = tid / TPN2;
+            for (int mb = 0; mb < M; mb += MSB) {
+                const int mend = min(M, mb + MSB);
+                // ---------------- stage 1: T[m][kx] = sum_j Dt[j][m] * Q[(y0+j) mod H][kx]
+                for (int mc = mb; mc < mend; mc += MC1) {
+                    float acc[TM1][TN1];
+#pragma unroll
+                    for (int i = 0; i < TM1; ++i)
+#pragma unroll
+                        for (int j = 0; j < TN1; ++j) acc[i][j] = 0.f;
+                    constexpr int NKT = H / BK;
+                    const float *Asrc = p.Dt + mc;
+                    if (tid == 0)
+                        for (int t = 0; t < NSTG - 1 && t < NKT; ++t) stage_issue(t % NSTG, Asrc, t, p.Mp1, MC1);
+                    for (int kt = 0; kt < NKT; ++kt) {
+                        const int slot = kt % NSTG;
+                        if (tid == 0 && kt + NSTG - 1 < NKT) stage_issue((kt + NSTG - 1) % NSTG, Asrc, kt + NSTG - 1, p.Mp1, MC1);
+                        bar_wait(slot);
+                        const float *At = stg + (size_t)slot * p.stg_floats + tm1 * TM1;
+#pragma unroll
+                        for (int kk = 0; kk < BK; ++kk) {
+                            const int ys = (y0 + kt * BK + kk) & (H - 1);
+                            float a[TM1], b[TN1];
+                            load_vec<TM1>(a, At + kk * MC1);
+                            load_vec<TN1>(b, reinterpret_cast<const float *>(Sl + (size_t)ys * NC) + tn1 * TN1);
+#pragma unroll
+                            for (int i = 0; i < TM1; ++i)
+#pragma unroll
+                                for (int j = 0; j < TN1; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+                        }
+                        __syncthreads();  // slot may be refilled
+                    }
+                    // epilogue: rotate by exp(2 pi i kx x0 / W), send rows to the CTA that owns them in stage 2
+#pragma unroll
+                    for (int j = 0; j < TN1 / 2; ++j) {
+                        const int q = rank * NC + tn1 * (TN1 / 2) + j;
+                        if (q == 0) {
+                            const float sg = (x0 & 1) ? -1.f : 1.f;
+#pragma unroll
+                            for (int i = 0; i < TM1; ++i) acc[i][2 * j + 1] *= sg;
+                        } else {
+                            const float2 w = tw[((q * x0) & (W - 1)) * (NTW / W)];  // (cos, -sin)
+#pragma unroll
+                            for (int i = 0; i < TM1; ++i) {
+                                const float2 t = cmulc(make_float2(acc[i][2 * j], acc[i][2 * j + 1]), w);
+                                acc[i][2 * j] = t.x;
+                                acc[i][2 * j + 1] = t.y;
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < TM1; ++i) {
+                        const int m = mc + tm1 * TM1 + i;
+                        if (m < mend) {
+                            const int dr = (m - mb) / MS, row = (m - mb) % MS;
+                            float *Td = Tb;
+                            if constexpr (CS > 1) Td = cluster.map_shared_rank(Tb, dr);
+                            float *dst = Td + (size_t)row * LDT + 2 * (rank * NC + tn1 * (TN1 / 2));
+                            if constexpr (TN1 % 4 == 0) {
+#pragma unroll
+                                for (int j = 0; j < TN1 / 4; ++j)
+                                    reinterpret_cast<float4 *>(dst)[j] =
+                                        make_float4(acc[i][4 * j], acc[i][4 * j + 1], acc[i][4 * j + 2], acc[i][4 * j + 3]);
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < TN1 / 2; ++j)
+                                    reinterpret_cast<float2 *>(dst)[j] = make_float2(acc[i][2 * j], acc[i][2 * j + 1]);
+                            }
+                        }
+                    }
+                }
+                csync();  // T rows are at their owners
+
+                // ---------------- stage 2: C[m][n] = sum_k T[m][k] * AxT[k][n], streamed into the argmax
+                {
+                    const int mrow0 = mb + rank * MS;  // global m of my T row 0
+                    const int nrows = max(0, min(MS, mend - mrow0));
+                    for (int rc = 0; rc < nrows; rc += TPM2 * TM2) {
+                        for (int nc = 0; nc < M; nc += TPN2 * TN2) {
+                            float acc[TM2][TN2];
+#pragma unroll
+                            for (int i = 0; i < TM2; ++i)
+#pragma unroll
+                                for (int j = 0; j < TN2; ++j) acc[i][j] = 0.f;
+                            constexpr int NKT = W / BK;
+                            const float *Bsrc = p.AxT + nc;
+                            const bool active = tm2 < TPM2;
+                            const float *Arow[TM2];
+#pragma unroll
+                            for (int i = 0; i < TM2; ++i) Arow[i] = Tb + (size_t)min(rc + tm2 * TM2 + i, MS - 1) * LDT;
+                            if (tid == 0)
+                                for (int t = 0; t < NSTG - 1 && t < NKT; ++t) stage_issue(t % NSTG, Bsrc, t, p.Np2, NCH2);
+                            for (int kt = 0; kt < NKT; ++kt) {
+                                const int slot = kt % NSTG;
+                                if (tid == 0 && kt + NSTG - 1 < NKT)
+                                    stage_issue((kt + NSTG - 1) % NSTG, Bsrc, kt + NSTG - 1, p.Np2, NCH2);
+                                bar_wait(slot);
+                                if (active) {
+                                    const float *Bt = stg + (size_t)slot * p.stg_floats + tn2 * TN2;
+#pragma unroll
+                                    for (int k4 = 0; k4 < BK / 4; ++k4) {
+                                        float4 a4[TM2];
+#pragma unroll
+                                        for (int i = 0; i < TM2; ++i)
+                                            a4[i] = *reinterpret_cast<const float4 *>(Arow[i] + kt * BK + k4 * 4);
+#pragma unroll
+                                        for (int kk = 0; kk < 4; ++kk) {
+                                            float b[TN2];
+                                            load_vec<TN2>(b, Bt + (k4 * 4 + kk) * NCH2);
+#pragma unroll
+                                            for (int i = 0; i < TM2; ++i) {
+                                                const float av = kk == 0 ? a4[i].x : kk == 1 ? a4[i].y : kk == 2 ? a4[i].z : a4[i].w;
+#pragma unroll
+                                                for (int j = 0; j < TN2; ++j) acc[i][j] = fmaf(av, b[j], acc[i][j]);
+                                            }
+                                        }
+                                    }
+                                }
+                                __syncthreads();
+                            }
+                            if (active) {
+#pragma unroll
+                                for (int i = 0; i < TM2; ++i) {
+                                    const int r = rc + tm2 * TM2 + i;
+                                    const int m = mrow0 + r;
+#pragma unroll
+                                    for (int j = 0; j < TN2; ++j) {
+                                        const int n = nc + tn2 * TN2 + j;
+                                        if (r < nrows && n < M && better(acc[i][j], m * M + n, sub.v, sub.i))
+                                            sub.v = acc[i][j], sub.i = m * M + n;
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+                if (mb + MSB < M) csync();  // T is overwritten by the next super-block
+            }
+        }
+        int ms, ns;
+        {
+            sub = block_best(sub);
+            if (tid == 0) {
+                xsrc[0] = (double)sub.v;
+                xsrc[1] = (double)sub.i;
+            }
+            const double *res = exchange(2);
+            Best g{(float)res[0], (int)res[1]};
+            for (int r = 1; r < CS; ++r) {
+                const float v = (float)res[r * XN];
+                const int i = (int)res[r * XN + 1];
+                if (better(v, i, g.v, g.i)) g.v = v, g.i = i;
+            }
+            ms = g.i / M;
+            ns = g.i % M;
+        }
+
+        // ---------------- fp64 3x3 hill-climb on the 1/u grid, from the fp32 Q
+        double up_peak = 0.0;
+        {
+            constexpr int NSL = (NT / NC) > 0 ? (NT / NC) : 1;  // j-slices per column
+            double *dtab = reinterpret_cast<double *>(U);                      // [3][H]
+            double2 *part = reinterpret_cast<double2 *>(dtab + 3 * H);         // [3][NSL][NC]
+            double2 *R64 = part + 3 * NSL * NC;                                // [3][NC]
+            double *terms = reinterpret_cast<double *>(R64 + 3 * NC);          // [9][NC]
+            for (int iter = 0; iter < 8; ++iter) {
+                for (int e = tid; e < 3 * H; e += NT) {
+                    const int a = e / H, j = e % H;
+                    const int mm = ms - 1 + a;
+                    dtab[e] = (mm >= 0 && mm < M) ? dirichlet64((long long)(mm - cM) - (long long)j * u, u, H) : 0.0;
+                }
+                __syncthreads();
+                for (int e = tid; e < NSL * NC; e += NT) {
+                    const int ql = e % NC, sl = e / NC;
+                    double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
+                    for (int j = sl; j < H; j += NSL) {
+                        const float2 v = Sl[(size_t)((y0 + j) & (H - 1)) * NC + ql];
+                        const double vx = (double)v.x, vy = (double)v.y;
+                        const double d0 = dtab[j], d1 = dtab[H + j], d2 = dtab[2 * H + j];
+                        s0.x = fma(d0, vx, s0.x), s0.y = fma(d0, vy, s0.y);
+                        s1.x = fma(d1, vx, s1.x), s1.y = fma(d1, vy, s1.y);
+                        s2.x = fma(d2, vx, s2.x), s2.y = fma(d2, vy, s2.y);
+                    }
+                    part[(0 * NSL + sl) * NC + ql] = s0;
+                    part[(1 * NSL + sl) * NC + ql] = s1;
+                    part[(2 * NSL + sl) * NC + ql] = s2;
+                }
+                __syncthreads();
+                for (int e = tid; e < 3 * NC; e += NT) {
+                    const int a = e / NC, ql = e % NC;
+                    double2 s = make_double2(0.0, 0.0);
+                    for (int sl = 0; sl < NSL; ++sl) {
+                        const double2 t = part[(a * NSL + sl) * NC + ql];
+                        s.x += t.x, s.y += t.y;
+                    }
+                    R64[e] = s;
+                }
+                long long xnum[3];
+                double nyq[3], c9[9];
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    const long long xn = (long long)x0 * u + (ns - 1 + b - cM);
+                    xnum[b] = xn;
+                    long long r2 = xn % (2LL * u);
+                    if (r2 < 0) r2 += 2LL * u;
+                    nyq[b] = cospi((double)r2 / (double)u);
+                }
+                __syncthreads();
+                xeval9(R64, xnum, (long long)u * W, nyq, terms, c9);
+                double bv = -INFINITY;
+                int ba = 1, bb = 1, bi = 0x7fffffff;
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) {
+                        const int mm = ms - 1 + a, nn = ns - 1 + b;
+                        if (mm < 0 || mm >= M || nn < 0 || nn >= M) continue;
+                        const int idx = mm * M + nn;
+                        const double v = c9[a * 3 + b];
+                        if (v > bv || (v == bv && idx < bi)) bv = v, bi = idx, ba = a, bb = b;
+                    }
+                up_peak = bv;
+                if (ba == 1 && bb == 1) break;
+                ms += ba - 1;
+                ns += bb - 1;
+                __syncthreads();
+            }
+        }
+        if (rank == 0 && tid == 0) {
+            p.dy[f] = (float)((double)wy + (double)(ms - cM) / (double)u);
+            p.dx[f] = (float)((double)wx + (double)(ns - cM) / (double)u);
+            if (p.peak) p.peak[f] = (float)(up_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean);
+            if (p.iy) p.iy[f] = wy;
+            if (p.ix) p.ix[f] = wx;
+        }
+        __syncthreads();  // U (polish scratch) is reused by the next frame's raw ring
+    }
+    csync();  // no CTA of the cluster exits while peers may still address its shared memory
+}
+
+// ------------------------------------------------------------------ host-side launcher glue
+template <class C>
+struct Launcher {
+    static size_t fixed_smem() { return C::FIXED_BYTES; }
+    static int raw_scratch_bytes() { return C::RAWB + C::SCRB; }
+    static cudaError_t prepare(int smem_bytes)
+    {
+        cudaError_t e = cudaFuncSetAttribute(cc_fused_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+        if (e != cudaSuccess) return e;
+        if (C::CS > 8) e = cudaFuncSetAttribute(cc_fused_kernel<C>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        return e;
+    }
+    static void fill(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, int n_clusters, int smem_bytes, cudaStream_t st)
+    {
+        cfg = cudaLaunchConfig_t{};
+        cfg.gridDim = dim3((unsigned)(n_clusters * C::CS), 1, 1);
+        cfg.blockDim = dim3(C::NT, 1, 1);
+        cfg.dynamicSmemBytes = (size_t)smem_bytes;
+        cfg.stream = st;
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = C::CS;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    static cudaError_t max_clusters(int smem_bytes, int *n)
+    {
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute attr[1];
+        fill(cfg, attr, 1, smem_bytes, 0);
+        return cudaOccupancyMaxActiveClusters(n, cc_fused_kernel<C>, &cfg);
+    }
+    static cudaError_t launch(const CcParams &p, int n_clusters, int smem_bytes, cudaStream_t st)
+    {
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute attr[1];
+        fill(cfg, attr, n_clusters, smem_bytes, st);
+        return cudaLaunchKernelEx(&cfg, cc_fused_kernel<C>, p);
+    }
+    static CcVariant variant()
+    {
+        CcVariant v{};
+        v.H = C::H, v.W = C::W, v.CS = C::CS, v.NT = C::NT, v.dtype = sizeof(typename C::PIX) == 1 ? 0 : 1;
+        v.TM1 = C::TM1, v.TN1 = C::TN1, v.TM2 = C::TM2, v.TN2 = C::TN2;
+        v.s_global = C::SG ? 1 : 0;
+        v.BK = BK, v.NSTG = NSTG;
+        v.fixed_smem = &fixed_smem;
+        v.raw_scratch_bytes = &raw_scratch_bytes;
+        v.prepare = &prepare;
+        v.max_clusters = &max_clusters;
+        v.launch = &launch;
+        return v;
+    }
+};
+
+}  // namespace ccf

@@ -1,0 +1,10 @@
+// cc_variant.cu -- one translation unit per kernel variant; build.py defines
+// CCV_NAME and the template arguments on the nvcc command line.
+#include "cc_fused.cuh"
+
+using VariantCfg = ccf::Cfg<CCV_H, CCV_W, CCV_CS, CCV_PIX, CCV_NT, CCV_TM1, CCV_TN1, CCV_TM2, CCV_TN2, CCV_SG>;
+
+#define CCV_CAT2(a, b) a##b
+#define CCV_CAT(a, b) CCV_CAT2(a, b)
+
+CcVariant CCV_CAT(cc_variant_, CCV_NAME)() { return ccf::Launcher<VariantCfg>::variant(); }
