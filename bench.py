@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- frames/s of the fused cross-correlation tracker on B200.
+
+One "step" = one cc_track() pass of the whole hot path (ingest, FFTs, product,
+argmax, upsampled DFT, sub-pixel argmax) over one batch of seeded synthetic
+frames (BASELINE.json configs[2]: 256x256 uint16, batch 10,000, u = 100 --
+the configuration the roofline target is quoted on).  Also reports the
+single-frame latency of configs[1] (128x128 uint8, u = 20, batch-1 streaming).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Under torchrun (N > 1) every rank runs the same workload on its own frames
+(weak scaling, no data-path collective); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2310_08770_b200 import workloads as wl  # noqa: E402
+
+NOMINAL_SM_MHZ = 1965.0
+FP32_LANES_PER_SM = 128
+
+
+def flops_per_frame(H, W, u):
+    """Algorithmic flop count of SURVEY.md 8(d): FFT pair + product + upsampled DFT stages 1 and 2."""
+    Wh, M = W // 2 + 1, (3 * u + 1) // 2
+    fft = 5.0 * H * W * np.log2(H * W)
+    prod = 6.0 * H * Wh
+    s1 = 8.0 * M * H * Wh
+    s2 = 4.0 * M * M * Wh
+    return fft + prod + s1 + s2
+
+
+def executed_flops_per_frame(H, W, u):
+    """Flops of the formulation the kernel executes (real Dirichlet stage 1: 4*M*H*W/2... see DESIGN.md)."""
+    M = (3 * u + 1) // 2
+    fft = 5.0 * H * W * np.log2(H * W)
+    return fft + 6.0 * H * (W // 2) + 2.0 * M * H * W + 2.0 * M * M * W
+
+
+class ClockSampler:
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])), mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(cfg, n_frames: int):
+    """Frames/s of the float64 CPU oracle, as it stands, on the first n parity-subset frames."""
+    import oracle
+    idx = wl.oracle_subset(cfg)[:n_frames]
+    fr = wl.frames(cfg, idx)
+    ref = wl.reference(cfg)
+    oracle.track(fr[:1], ref, cfg.upsample)  # build + warm
+    t0 = time.perf_counter()
+    oracle.track(fr, ref, cfg.upsample)
+    dt = time.perf_counter() - t0
+    return len(idx) / dt, oracle.num_threads(), len(idx), dt
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    n = args.ref_frames
+    idx = wl.oracle_subset(cfg)[:n]
+    fr = wl.frames(cfg, idx)
+    ref = wl.reference(cfg)
+    oracle.track(fr[:1], ref, cfg.upsample)
+    for _ in range(args.warmup):
+        oracle.track(fr, ref, cfg.upsample)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.track(fr, ref, cfg.upsample)
+    dt = (time.perf_counter() - t0) / max(1, args.steps)
+    val = len(idx) / dt
+    sample = "first %d frames of the cfg-3 parity subset per step (bounded sample of the 10,000-frame batch)" % len(idx)
+    line = {
+        "impl": "reference", "metric": "frames_per_s", "value": val, "unit": "frames/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "H": cfg.H, "W": cfg.W, "pixel": cfg.dtype, "upsample": cfg.upsample,
+                   "frames_per_step": len(idx)},
+        "cpu_baseline": {"value": val, "unit": "frames/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--batch", type=int, default=0, help="frames per step (default: the config's 10,000)")
+    ap.add_argument("--ref-frames", type=int, default=256, help="frames per step of the --impl reference arm")
+    ap.add_argument("--cpu-frames", type=int, default=512, help="sample size of the cpu_baseline leg")
+    ap.add_argument("--latency-frames", type=int, default=10000)
+    ap.add_argument("--no-latency", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    cfg = wl.config(3)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2310_08770_b200 import Plan, fp32_peak_probe
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    B = args.batch or cfg.n_frames
+    # every rank draws its own frames: same recipe, frame indices offset by rank (weak scaling)
+    t_gen = time.perf_counter()
+    uniq = min(B, cfg.n_frames)
+    idx = (np.arange(uniq) + rank * 7919) % cfg.n_frames
+    frames = wl.frames(cfg, idx)
+    if uniq < B:
+        frames = np.concatenate([frames] * ((B + uniq - 1) // uniq))[:B]
+    ref = wl.reference(cfg)
+    t_gen = time.perf_counter() - t_gen
+    plan = Plan(cfg.H, cfg.W, frames.dtype, cfg.upsample, ref)
+    info = plan.info()
+    dfr = plan.device_frames(frames)
+    out = (torch.empty(B, dtype=torch.float32, device="cuda"), torch.empty(B, dtype=torch.float32, device="cuda"),
+           torch.empty(B, dtype=torch.float32, device="cuda"))
+
+    for _ in range(args.warmup):
+        plan.track(dfr, B, out=out)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t0 = time.perf_counter()
+    for a, b in ev:
+        a.record()
+        plan.track(dfr, B, out=out)
+        b.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop() if rank == 0 else None
+    kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms = ev[0][0].elapsed_time(ev[-1][1]) / args.steps
+    t = torch.tensor([step_ms, float(np.mean(kernel_ms))], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms, kern_ms = float(t[0]), float(t[1])
+    value = world * B / (step_ms * 1e-3)
+
+    # ---- end to end: pinned host frames -> cc_track_host -> host results
+    e2e = None
+    if not args.no_e2e:
+        hfr = torch.from_numpy(frames.view(np.uint8).reshape(B, -1)).pin_memory()
+        hnp = hfr.numpy().view(frames.dtype).reshape(frames.shape)
+        hdx = torch.empty(B, dtype=torch.float32).pin_memory()
+        hdy = torch.empty(B, dtype=torch.float32).pin_memory()
+        hpk = torch.empty(B, dtype=torch.float32).pin_memory()
+        plan.track_host(hnp, hdx.numpy(), hdy.numpy(), hpk.numpy())
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            plan.track_host(hnp, hdx.numpy(), hdy.numpy(), hpk.numpy())
+        barrier()
+        dt = (time.perf_counter() - t0) / args.steps
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * B / float(tt[0]), "unit": "frames/s", "h2d_bytes_per_step": int(frames.nbytes),
+               "d2h_bytes_per_step": int(3 * 4 * B), "ms_per_step": float(tt[0]) * 1e3,
+               "api": "cc_track_host (pinned host frames in, host dx/dy/peak out)"}
+        same = bool(np.array_equal(hdx.numpy(), out[0].cpu().numpy()) and np.array_equal(hdy.numpy(), out[1].cpu().numpy()))
+        e2e["matches_device_path"] = same
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the (single) fused kernel
+    flop = flops_per_frame(cfg.H, cfg.W, cfg.upsample)
+    peak_tf = 148 * FP32_LANES_PER_SM * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
+    achieved_tf = flop * B / (kern_ms * 1e-3) / 1e12
+    probe_tf = fp32_peak_probe()
+    hbm_gbs = None
+    try:
+        hbm_gbs = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_gbs = 6650.0
+    t_alu = flop / (peak_tf * 1e12)
+    t_hbm = (frames[0].nbytes + 12) / (hbm_gbs * 1e9)
+    roofline = {
+        "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+        "traffic": None, "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
+        "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
+        "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
+        "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,
+        "ffma_probe_tflops": probe_tf,
+        "roofline_frames_per_s": 1.0 / max(t_alu, t_hbm), "hbm_leg_frames_per_s": 1.0 / t_hbm,
+        "hbm_achieved_gbs": (frames[0].nbytes + 12) * B / (kern_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs,
+    }
+
+    # ---- single-frame latency, configs[1]: 128x128 u8, u = 20, sequential batch-1 calls
+    latency = None
+    if not args.no_latency:
+        c2 = wl.config(2)
+        nlat = min(args.latency_frames, c2.n_frames)
+        f2 = wl.frames(c2, np.arange(nlat))
+        p2 = Plan(c2.H, c2.W, f2.dtype, c2.upsample, wl.reference(c2))
+        d2 = p2.device_frames(f2)
+        o2 = (torch.empty(1, dtype=torch.float32, device="cuda"), torch.empty(1, dtype=torch.float32, device="cuda"),
+              torch.empty(1, dtype=torch.float32, device="cuda"))
+        lib_track = p2.track
+        for i in range(50):
+            lib_track(d2[i], 1, out=o2)
+        torch.cuda.synchronize()
+        lat = np.empty(nlat)
+        for i in range(nlat):
+            t0 = time.perf_counter_ns()
+            lib_track(d2[i], 1, out=o2)
+            torch.cuda.synchronize()
+            lat[i] = (time.perf_counter_ns() - t0) * 1e-3
+        # GPU-only time of the same launches (events around 200 back-to-back calls)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for i in range(200):
+            lib_track(d2[i], 1, out=o2)
+        b.record()
+        torch.cuda.synchronize()
+        latency = {"workload": c2.name, "calls": nlat, "median_us": float(np.median(lat)), "p99_us": float(np.percentile(lat, 99)),
+                   "max_us": float(lat.max()), "gpu_only_us_per_call_back_to_back": a.elapsed_time(b) * 1e3 / 200,
+                   "cluster_size": p2.info()["lat_cluster_size"] or p2.info()["cluster_size"],
+                   "note": "host clock around cc_track(batch=1) + stream sync, frame resident in HBM, through the Python binding"}
+        p2.close()
+
+    # ---- CPU oracle beside it
+    cpu = None
+    if not args.no_cpu:
+        v, cores, n, dt = oracle_rate(cfg, args.cpu_frames)
+        cpu = {"value": v, "unit": "frames/s", "cores": cores, "kind": "oracle",
+               "sample": "first %d frames of the cfg-3 parity subset, %.1f s wall" % (n, dt)}
+
+    line = {
+        "metric": "frames_per_s", "value": value, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "H": cfg.H, "W": cfg.W, "pixel": cfg.dtype, "upsample": cfg.upsample,
+                   "frames_per_step_per_gpu": B, "unique_frames": int(uniq), "parallelism": "replicas x%d" % world,
+                   "l2": "inputs (%.2f GB per step) larger than L2" % (frames.nbytes / 1e9),
+                   "cluster_size": info["cluster_size"], "clusters_resident": info["max_clusters"],
+                   "threads": info["threads"], "smem_bytes": info["smem_bytes"], "gen_s": round(t_gen, 1)},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu,
+        "latency": latency, "wall_s_timed_region": wall,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,224 @@
+"""GPU parity: the fused CUDA path (through the C-ABI) against the float64 CPU
+oracle, element by element on the same seeded inputs.
+
+Bar (BASELINE.json north_star): integer peaks bit-exact; sub-pixel
+displacements within 2e-3 px (outputs are multiples of 1/u >= 0.01, so this
+means "the same grid point"); peak value relative error <= 1e-4.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_PX = 2e-3       # north_star
+TOL_PEAK = 1e-4     # SURVEY.md 8(c), informational bound kept as a gate
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2310_08770_b200 import build as cuda_build
+    cuda_build.build()
+    import paper_2310_08770_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+def _run(pkg, frames, ref, u, debug=True):
+    import torch
+    plan = pkg.Plan(frames.shape[1], frames.shape[2], frames.dtype, u, ref)
+    out = plan.track(plan.device_frames(frames), debug=debug)
+    torch.cuda.synchronize()
+    res = [t.cpu().numpy() for t in out]
+    plan.close()
+    return res
+
+
+def _compare(o, dx, dy, pk, iy, ix, label):
+    bad_i = np.nonzero((iy != o.wy) | (ix != o.wx))[0]
+    bad_s = np.nonzero((np.abs(dx - o.dx) > TOL_PX) | (np.abs(dy - o.dy) > TOL_PX))[0]
+    msg = []
+    for i in list(bad_i[:8]) + list(bad_s[:8]):
+        margin = (o.up_top1[i] - o.up_top2[i]) / max(abs(o.up_top1[i]), 1e-300)
+        msg.append("frame %d: gpu int (%d,%d) sub (%.4f,%.4f) | oracle int (%d,%d) sub (%.4f,%.4f) | oracle sub margin %.2e"
+                   % (i, iy[i], ix[i], dy[i], dx[i], o.wy[i], o.wx[i], o.dy[i], o.dx[i], margin))
+    assert len(bad_i) == 0 and len(bad_s) == 0, "%s: %d integer / %d sub-pixel mismatches\n%s" % (
+        label, len(bad_i), len(bad_s), "\n".join(msg))
+    rel = np.max(np.abs(pk / o.peak - 1.0))
+    assert rel <= TOL_PEAK, "%s: peak relative error %.2e" % (label, rel)
+
+
+# (config, number of parity-subset frames the oracle is run on)
+SUBSETS = [(1, 1000), (2, 1000), (3, 400), (4, 64), (5, 24)]
+
+
+@pytest.mark.parametrize("ci,n", SUBSETS)
+def test_config_parity_subset(gpu, oracle_mod, ci, n):
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    idx = wl.oracle_subset(cfg)[:n]
+    fr = wl.frames(cfg, idx)
+    ref = wl.reference(cfg)
+    o = oracle_mod.track(fr, ref, cfg.upsample)
+    dx, dy, pk, iy, ix = _run(gpu, fr, ref, cfg.upsample)
+    _compare(o, dx, dy, pk, iy, ix, cfg.name)
+
+
+def test_cfg3_full_batch_in_bench_configuration(gpu, oracle_mod):
+    """10,000 frames in ONE cc_track call (the launch bench.py times); sampled outputs against the oracle,
+    every output checked for the properties that hold at any size."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(3)
+    fr = wl.frames(cfg)
+    ref = wl.reference(cfg)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    d = plan.device_frames(fr)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(d, debug=True)]
+    dx2, dy2, pk2 = [t.cpu().numpy() for t in plan.track(d)]
+    torch.cuda.synchronize()
+    assert np.array_equal(dx, dx2) and np.array_equal(dy, dy2) and np.array_equal(pk, pk2)   # deterministic
+    sample = np.arange(7, cfg.n_frames, 97)[:96]                  # frames NOT on the stride-10 subset too
+    o = oracle_mod.track(fr[sample], ref, cfg.upsample)
+    _compare(o, dx[sample], dy[sample], pk[sample], iy[sample], ix[sample], "cfg3 full batch (sampled)")
+    u = cfg.upsample
+    for v, w in ((dx, ix), (dy, iy)):
+        k = np.rint(v.astype(np.float64) * u)
+        assert np.max(np.abs(k / u - v)) < 1e-5                    # multiples of 1/u
+        off = k - w.astype(np.float64) * u
+        assert off.min() >= -(cfg.upsample * 3 // 2 // 2) and off.max() <= (3 * u + 1) // 2 - 1 - (3 * u + 1) // 2 // 2
+    truth = wl.shifts(cfg)
+    err = np.hypot(dx - truth[:, 1], dy - truth[:, 0])
+    assert np.median(err) < 0.5 and err.max() < 3.0               # tracks the spot (fringe/gradient bias allowed)
+    plan.close()
+
+
+def test_streaming_batch1_matches_batched(gpu, oracle_mod):
+    """configs[1] mode: sequential cc_track(batch=1) calls (the small-batch cluster variant) give the
+    same displacements as one batched call and as the oracle; frame 0 == reference -> exactly (0, 0)."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(2)
+    idx = np.arange(64)
+    fr = wl.frames(cfg, idx)
+    ref = wl.reference(cfg)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    assert plan.info()["lat_cluster_size"] > 1
+    d = plan.device_frames(fr)
+    bx, by, _ = [t.cpu().numpy() for t in plan.track(d)]
+    sx, sy = np.empty(64, np.float32), np.empty(64, np.float32)
+    for i in range(64):
+        x, y, _ = plan.track(d[i], 1)
+        sx[i], sy[i] = x.item(), y.item()
+    torch.cuda.synchronize()
+    o = oracle_mod.track(fr, ref, cfg.upsample)
+    assert np.array_equal(sx, bx) and np.array_equal(sy, by)
+    assert np.max(np.abs(sx - o.dx)) <= TOL_PX and np.max(np.abs(sy - o.dy)) <= TOL_PX
+    assert sx[0] == 0.0 and sy[0] == 0.0
+    plan.close()
+
+
+@pytest.mark.parametrize("H,W,dt", [(64, 64, np.uint16), (128, 128, np.uint8), (256, 256, np.uint16)])
+def test_integer_circular_shifts_recovered_exactly(gpu, oracle_mod, H, W, dt):
+    """Periodic boundaries: frame = circshift(ref, (a, b)) -> d = wrap(a, b), offset exactly 0."""
+    rng = np.random.default_rng(11)
+    hi = 200 if dt == np.uint8 else 4000
+    ref = rng.integers(0, hi, size=(H, W)).astype(dt)
+    shifts = [(0, 0), (1, 0), (0, 1), (H // 2 - 1, W // 2 - 1), (H // 2, W // 2), (H - 1, W - 1), (5, W - 7), (H - 3, 2)]
+    fr = np.stack([np.roll(ref, s, axis=(0, 1)) for s in shifts])
+    dx, dy, pk, iy, ix = _run(gpu, fr, ref.astype(np.float32), 10)
+    for k, (a, b) in enumerate(shifts):
+        wa = a - H if 2 * a >= H else a
+        wb = b - W if 2 * b >= W else b
+        assert (iy[k], ix[k]) == (wa, wb)
+        assert dy[k] == float(wa) and dx[k] == float(wb)
+    assert np.max(np.abs(pk / np.sum(ref.astype(np.float64) ** 2) - 1)) < 1e-5
+    o = oracle_mod.track(fr, ref.astype(np.float32), 10)
+    _compare(o, dx, dy, pk, iy, ix, "circular shifts")
+
+
+def test_degenerate_constant_frame_and_ties(gpu, oracle_mod):
+    """Constant frame -> cc constant -> smallest index (0,0) in both argmaxes -> d = (-c/u, -c/u) (R6)."""
+    H = W = 64
+    u = 10
+    ref = np.random.default_rng(3).integers(0, 1000, size=(H, W)).astype(np.float32)
+    fr = np.stack([np.full((H, W), 777, np.uint16), np.zeros((H, W), np.uint16), np.full((H, W), 65535, np.uint16)])
+    dx, dy, pk, iy, ix = _run(gpu, fr, ref, u)
+    M = (3 * u + 1) // 2
+    c = M // 2
+    assert np.all(iy == 0) and np.all(ix == 0)
+    assert np.allclose(dx, -c / u) and np.allclose(dy, -c / u)
+    o = oracle_mod.track(fr, ref, u)
+    assert np.all(o.wy == 0) and np.all(o.wx == 0) and np.allclose(o.dx, -c / u)
+    assert np.max(np.abs(pk - o.peak) / np.maximum(1.0, np.abs(o.peak))) < 1e-5
+
+
+@pytest.mark.parametrize("u", [1, 2, 7, 33, 256])
+def test_other_upsample_factors(gpu, oracle_mod, u):
+    """u = 1 (integer peak only), odd/even M, and a factor large enough to need several T super-blocks."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(24))
+    ref = wl.reference(cfg)
+    o = oracle_mod.track(fr, ref, u)
+    dx, dy, pk, iy, ix = _run(gpu, fr, ref, u)
+    _compare(o, dx, dy, pk, iy, ix, "u=%d" % u)
+
+
+def test_full_range_random_pixels_u8_u16(gpu, oracle_mod):
+    """Maximum-size pixel values and no structure at all: parity must still hold."""
+    rng = np.random.default_rng(5)
+    for dt, hi, H in ((np.uint16, 65536, 128), (np.uint8, 256, 64)):
+        ref = rng.integers(0, hi, size=(H, H)).astype(np.float32)
+        fr = rng.integers(0, hi, size=(6, H, H)).astype(dt)
+        fr[0] = ref.astype(dt)
+        o = oracle_mod.track(fr, ref, 20)
+        dx, dy, pk, iy, ix = _run(gpu, fr, ref, 20)
+        _compare(o, dx, dy, pk, iy, ix, "random %s" % dt.__name__)
+        assert dx[0] == 0 and dy[0] == 0
+
+
+def test_ragged_batches_and_empty(gpu, oracle_mod):
+    """Batch sizes around the number of resident clusters (ragged last wave), and batch 0."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(301))
+    ref = wl.reference(cfg)
+    o = oracle_mod.track(fr, ref, cfg.upsample)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    nres = plan.info()["max_clusters"]
+    d = plan.device_frames(fr)
+    for b in sorted({1, 2, nres - 1, nres, nres + 1, 2 * nres + 3, 301} & set(range(1, 302))):
+        dx, dy, pk = [t.cpu().numpy() for t in plan.track(d, b)]
+        assert np.max(np.abs(dx - o.dx[:b])) <= TOL_PX and np.max(np.abs(dy - o.dy[:b])) <= TOL_PX, b
+    lib = gpu.load_library()
+    assert lib.cc_track(plan._h, None, 0, None, None, None, None) == 0       # batch 0: CC_OK, no launch
+    assert lib.cc_track(plan._h, ctypes.c_void_p(d.data_ptr() + 2), 1,
+                        ctypes.c_void_p(8), ctypes.c_void_p(8), None, None) == 1   # misaligned frames
+    torch.cuda.synchronize()
+    plan.close()
+
+
+def test_host_path_matches_device_path(gpu):
+    """cc_track_host (H2D/D2H inside the call) returns exactly what cc_track returns."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(500))
+    ref = wl.reference(cfg)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    dx, dy, pk = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr))]
+    hx, hy, hp = plan.track_host(fr)
+    torch.cuda.synchronize()
+    assert np.array_equal(hx, dx) and np.array_equal(hy, dy) and np.array_equal(hp, pk)
+    plan.close()
+
+
+def test_fp32_probe_reports_sane_rate(gpu):
+    tf = gpu.fp32_peak_probe()
+    assert 30.0 < tf < 80.0
