@@ -273,8 +273,7 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
         // packed column: DC bin of the reference zeroed (shift-independent constant; R10)
         std::complex<double> g0 = (ky == 0) ? std::complex<double>(0.0, 0.0) : std::conj(G[(size_t)ky * W]) / HW;
         std::complex<double> gn = std::conj(G[(size_t)ky * W + Wh]) / HW;
-        const std::complex<double> al = 0.5 * (g0 + gn), be = 0.5 * (g0 - gn);
-        ab[p] = make_float4((float)al.real(), (float)al.imag(), (float)be.real(), (float)be.imag());
+        ab[p] = make_float4((float)g0.real(), (float)g0.imag(), (float)gn.real(), (float)gn.imag());
     }
 
     int maxMC1 = pl->thr.MC1, np2 = pl->thr.np2_need;

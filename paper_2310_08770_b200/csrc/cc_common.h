@@ -45,7 +45,7 @@ struct CcParams {
     const float2 *tw;             // [NTW] (cos, -sin)(2 pi j / NTW), NTW = max(H, W)
     const uint16_t *row_slot;     // [W] slot holding row frequency k
     const float2 *Gt;             // [H][W/2]: conj(G[ky(p)][q]) / (H W), p = column slot; q = 0 unused
-    const float4 *ab;             // [H]: (alpha, beta) of the packed DC/Nyquist column, by slot
+    const float4 *ab;             // [H]: conj(G)/(HW) of columns kx = 0 (DC bin zeroed) and kx = W/2, by slot
     const uint16_t *col_partner;  // [H]: slot of -ky for the frequency at slot p
     const float *Dt;              // [H][Mp1]: Dirichlet interpolation matrix, j-major
     const float *AxT;             // [W][Np2]: x-axis upsampling matrix, k-major (re, -im interleaved along k)

@@ -530,7 +530,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
             __syncthreads();
             if (rank == 0) {
-                // P'[p] = alpha[p] Z[p] + beta[p] conj(Z[partner(p)])   (two real columns in one complex FFT)
+                // two real columns (kx = 0 and kx = W/2) ride in one complex FFT: split them with the -ky
+                // partner, multiply each by its conj(G) column, re-pack as PA + i PB.  The split is done
+                // first so that exact zeros stay exact (a constant frame must give P = 0, not rounding noise).
                 constexpr int PER = (H + NT - 1) / NT;
                 float2 o[PER];
 #pragma unroll
@@ -538,9 +540,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     const int s = tid + e * NT;
                     if (s < H) {
                         const float2 z = Sl[(size_t)s * NC], zp = Sl[(size_t)p.col_partner[s] * NC];
-                        const float4 ab = p.ab[s];
-                        o[e] = make_float2(ab.x * z.x - ab.y * z.y + ab.z * zp.x + ab.w * zp.y,
-                                           ab.x * z.y + ab.y * z.x - ab.z * zp.y + ab.w * zp.x);
+                        const float4 g = p.ab[s];  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
+                        const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
+                        const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
+                        const float2 pa = cmul(fa, make_float2(g.x, g.y)), pb = cmul(fb, make_float2(g.z, g.w));
+                        o[e] = make_float2(pa.x - pb.y, pa.y + pb.x);
                         if (s == 0) *f00 = z.x;  // sum of (I - c0): DC add-back for `peak`
                     }
                 }
