@@ -105,6 +105,20 @@ cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch,
                          float *dx, float *dy, float *peak, int *iy, int *ix, void *stream);
 
 /*
+ * cc_track_profile -- cc_track that additionally records, per frame, the SM
+ * clock cycles spent in each phase of the fused kernel (the per-frame latency
+ * breakdown).  Phases: 0 ingest + row FFT, 1 column FFT (x) conj(F[E]) +
+ * column inverse, 2 row inverse FFT + integer argmax, 3 fp64 integer polish,
+ * 4 upsampled-DFT stage 1, 5 stage 2, 6 sub-pixel argmax reduction, 7 fp64
+ * sub-pixel polish.
+ *   phase_cycles   DEVICE pointer, batch * CC_NUM_PHASES uint64
+ */
+#define CC_NUM_PHASES 8
+cc_status cc_track_profile(const cc_plan *plan, const void *frames, int batch,
+                           float *dx, float *dy, float *peak,
+                           unsigned long long *phase_cycles, void *stream);
+
+/*
  * cc_track_host -- the same path for HOST buffers (pageable or pinned): frames
  * are copied host->device in chunks overlapped with compute, results are
  * copied back, and the call returns after everything has completed.

@@ -19,7 +19,7 @@ CC_U8, CC_U16 = 0, 1
 _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
-EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_host", "cc_plan_destroy",
+EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
            "cc_plan_info", "cc_fp32_peak_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -55,6 +55,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_track.restype = ci
         lib.cc_track_debug.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.cc_track_debug.restype = ci
+        lib.cc_track_profile.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp]
+        lib.cc_track_profile.restype = ci
         lib.cc_track_host.argtypes = [vp, vp, ci, vp, vp, vp]
         lib.cc_track_host.restype = ci
         lib.cc_plan_destroy.argtypes = [vp]
@@ -153,6 +155,21 @@ class Plan:
             return dx, dy, pk, iy, ix
         _check(lib.cc_track(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(), pkp, s))
         return dx, dy, pk
+
+    def track_profile(self, frames_dev, batch: int | None = None):
+        """cc_track_profile: returns (dx, dy, peak, cycles[batch, 8]) device tensors."""
+        torch = _torch()
+        fb = self.H * self.W * self.np_dtype.itemsize
+        if batch is None:
+            batch = frames_dev.numel() * frames_dev.element_size() // fb
+        dev = frames_dev.device
+        dx = torch.empty(batch, dtype=torch.float32, device=dev)
+        dy = torch.empty(batch, dtype=torch.float32, device=dev)
+        pk = torch.empty(batch, dtype=torch.float32, device=dev)
+        cyc = torch.zeros((batch, 8), dtype=torch.int64, device=dev)
+        _check(load_library().cc_track_profile(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(),
+                                               pk.data_ptr(), cyc.data_ptr(), torch.cuda.current_stream(dev).cuda_stream))
+        return dx, dy, pk, cyc
 
     def track_host(self, frames_np, dx=None, dy=None, peak=None):
         """cc_track_host: host numpy frames in, host numpy results out (H2D/D2H inside)."""

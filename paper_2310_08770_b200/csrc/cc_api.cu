@@ -358,8 +358,8 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.stg_floats = vp.stg_floats, p.Emean = pl->Emean;
 }
 
-extern "C" cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
-                                    int *iy, int *ix, void *stream)
+static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                            int *iy, int *ix, unsigned long long *phase_clk, void *stream)
 {
     if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track: bad plan or batch");
     if (batch == 0) return CC_OK;
@@ -370,17 +370,30 @@ extern "C" cc_status cc_track_debug(const cc_plan *plan, const void *frames, int
         vp = &plan->lat;
     CcParams p{};
     fill_params(plan, *vp, p);
-    p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix;
+    p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix, p.phase_clk = phase_clk;
     const int ncl = std::min(batch, vp->max_clusters);
     cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
     return CC_OK;
 }
 
+extern "C" cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                                    int *iy, int *ix, void *stream)
+{
+    return track_impl(plan, frames, batch, dx, dy, peak, iy, ix, nullptr, stream);
+}
+
+extern "C" cc_status cc_track_profile(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy,
+                                      float *peak, unsigned long long *phase_cycles, void *stream)
+{
+    if (!phase_cycles) return fail(CC_ERR_INVALID_ARG, "cc_track_profile: null pointer");
+    return track_impl(plan, frames, batch, dx, dy, peak, nullptr, nullptr, phase_cycles, stream);
+}
+
 extern "C" cc_status cc_track(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
                               void *stream)
 {
-    return cc_track_debug(plan, frames, batch, dx, dy, peak, nullptr, nullptr, stream);
+    return track_impl(plan, frames, batch, dx, dy, peak, nullptr, nullptr, nullptr, stream);
 }
 
 extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak)

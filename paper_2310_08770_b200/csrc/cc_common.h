@@ -34,6 +34,11 @@ static inline int cc_freq_of_slot(int N, int p)
     return k;
 }
 
+// Phases of the per-frame breakdown (cc_track_profile): 0 ingest + row FFT, 1 column FFT (x) conj(G) +
+// column inverse, 2 row C2R + integer argmax, 3 fp64 integer polish, 4 upsampled stage 1 (sum over
+// super-blocks: last one), 5 upsampled stage 2, 6 sub-pixel argmax reduction, 7 fp64 sub-pixel polish.
+#define CC_NPHASE 8
+
 // Kernel parameters (passed by value).  All table pointers are device memory
 // owned by the plan.
 struct CcParams {
@@ -41,6 +46,7 @@ struct CcParams {
     int batch;
     float *dx, *dy, *peak;  // peak may be null
     int *iy, *ix;           // may be null
+    unsigned long long *phase_clk;  // optional [batch][CC_NPHASE] SM-clock cycles per phase, else null
 
     const float2 *tw;             // [NTW] (cos, -sin)(2 pi j / NTW), NTW = max(H, W)
     const uint16_t *row_slot;     // [W] slot holding row frequency k

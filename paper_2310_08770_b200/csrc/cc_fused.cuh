@@ -428,7 +428,17 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
     };
 
+    long long tph = 0;
+    auto stamp = [&](int k, int f) {  // optional per-phase cycle counts (rank 0, thread 0)
+        if (p.phase_clk && rank == 0 && tid == 0) {
+            const long long now = clock64();
+            p.phase_clk[(size_t)f * CC_NPHASE + k] = (unsigned long long)(now - tph);
+            tph = now;
+        }
+    };
+
     for (int f = cid; f < p.batch; f += ncl) {
+        if (p.phase_clk && rank == 0 && tid == 0) tph = clock64();
         // =============================================================== a1 + a2: ingest and row FFTs
         {
             const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
@@ -484,6 +494,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
         }
         csync();  // every F_row[y][kx] is at its column owner
+        stamp(0, f);
 
         // =============================================================== a2/a3/a4: column FFT (x) Gc, column inverse
         {
@@ -576,6 +587,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
         }
         csync();  // Q[y][kx] complete everywhere
+        stamp(1, f);
 
         // =============================================================== a4/a5: row C2R streamed into the integer argmax
         int y0, x0;
@@ -618,6 +630,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
             y0 = g.i / W;
             x0 = g.i % W;
+            stamp(2, f);
 
             // fp64 re-evaluation of the 3x3 neighbourhood of the fp32 winner
             double2 *R64 = reinterpret_cast<double2 *>(U);
@@ -652,6 +665,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             x0 = bi % W;
             cc_peak = bv;
         }
+        stamp(3, f);
         const int wy = (2 * y0 >= H) ? y0 - H : y0;
         const int wx = (2 * x0 >= W) ? x0 - W : x0;
 
@@ -746,6 +760,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                 }
                 csync();  // T rows are at their owners
+                stamp(4, f);
 
                 // ---------------- stage 2: C[m][n] = sum_k T[m][k] * AxT[k][n], streamed into the argmax
                 {
@@ -810,6 +825,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         }
                     }
                 }
+                stamp(5, f);
                 if (mb + MSB < M) csync();  // T is overwritten by the next super-block
             }
         }
@@ -830,6 +846,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             ms = g.i / M;
             ns = g.i % M;
         }
+        stamp(6, f);
 
         // ---------------- fp64 3x3 hill-climb on the 1/u grid, from the fp32 Q
         double up_peak = 0.0;
@@ -902,6 +919,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 __syncthreads();
             }
         }
+        stamp(7, f);
         if (rank == 0 && tid == 0) {
             p.dy[f] = (float)((double)wy + (double)(ms - cM) / (double)u);
             p.dx[f] = (float)((double)wx + (double)(ns - cM) / (double)u);
