@@ -17,13 +17,13 @@
 #include "cc_common.h"
 
 // ------------------------------------------------------------------ variants
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG) CcVariant cc_variant_##name();
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2) CcVariant cc_variant_##name();
 #include "cc_variant_list.h"
 #undef CCV
 
 typedef CcVariant (*cc_variant_fn)();
 static const cc_variant_fn g_variant_fns[] = {
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG) &cc_variant_##name,
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2) &cc_variant_##name,
 #include "cc_variant_list.h"
 #undef CCV
 };
@@ -47,26 +47,28 @@ static cc_status fail_cuda(cudaError_t e, const char *what)
 
 static const int SMEM_LIMIT = 232448;  // 227 KB per CTA on sm_100
 
-// Per-variant launch geometry derived from the plan (M etc.).
+// Per-variant launch geometry and operand tiles derived from the plan (M etc.).
 struct VarPlan {
     CcVariant v;
     int smem_bytes = 0, max_clusters = 0;
-    int MS = 0, nsb = 0, NCH2 = 0, TPN2 = 0, u_bytes = 0, stg_floats = 0;
-    int MC1 = 0, np2_need = 0;
-    float2 *Sg = nullptr;  // global spectrum scratch (s_global variants)
+    int DS = 0, nsb = 0, DSBp = 0, nch1 = 0, KT1 = 0, nrc2 = 0, nnc2 = 0, KT2 = 0;
+    int ntiles_frame = 0, tile_floats = 0, u_bytes = 0;
+    float *blob = nullptr;      // device: staged operand tiles
+    uint32_t *sched = nullptr;  // device: per-frame tile order
+    float *nyqc = nullptr;      // device: cos(pi e / u)
+    float2 *Sg = nullptr;       // global spectrum scratch (s_global variants)
     size_t sg_bytes = 0;
     bool ready = false;
 };
 
 struct cc_plan {
     int H = 0, W = 0, u = 0, M = 0, c = 0, dtype = 0;
-    int Mp1 = 0, Np2 = 0, c0 = 0;
+    int c0 = 0;
     double Emean = 0.0;
     // device tables
     float2 *tw = nullptr, *Gt = nullptr;
     uint16_t *row_slot = nullptr, *col_partner = nullptr;
     float4 *ab = nullptr;
-    float *Dt = nullptr, *AxT = nullptr;
     size_t table_bytes = 0;
     VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
     bool has_lat = false;
@@ -131,36 +133,133 @@ static bool plan_variant(VarPlan &vp, int M, int W, int H)
 {
     const CcVariant &v = vp.v;
     const int NC = W / 2 / v.CS;
-    const int TPN1 = 2 * NC / v.TN1, TPM1 = v.NT / TPN1;
-    vp.MC1 = TPM1 * v.TM1;
-    const int want = (M + v.TN2 - 1) / v.TN2;
-    vp.TPN2 = std::min(v.NT, std::max(1, want));
-    if (want > v.NT) {  // several n-chunks: chunk starts must stay 16-byte aligned
-        while ((vp.TPN2 * v.TN2) % 4) --vp.TPN2;
-    }
-    vp.NCH2 = round_up(vp.TPN2 * v.TN2, 4);
-    const int nch = (M + vp.TPN2 * v.TN2 - 1) / (vp.TPN2 * v.TN2);
-    vp.np2_need = round_up((nch - 1) * vp.TPN2 * v.TN2 + vp.NCH2, 4);
-    vp.stg_floats = v.BK * std::max(vp.MC1, vp.NCH2);
+    const int nd = M / 2 + 1;  // offsets d = 0..c (and e = 0..c)
+    const int MC1 = v.R1 * v.TM1;
+    const int T1F = v.BK1 * MC1, T2F = v.G2 * v.Cn2 * (16 + 4 * (v.TN2 - 4));
+    vp.tile_floats = std::max(T1F, T2F);
     const int NSL = std::max(1, v.NT / NC);
     const int polish = 3 * H * 8 + 3 * NSL * NC * 16 + 3 * NC * 16 + 9 * NC * 8;
     const int lower = std::max(v.raw_scratch_bytes(), polish);
-    const long avail = (long)SMEM_LIMIT - (long)v.fixed_smem() - (long)v.NSTG * vp.stg_floats * 4 - 32;
+    const int red_bytes = (v.KS2 - 1) * v.R2 * v.Cn2 * 2 * v.TM2 * v.TN2 * 4;
+    const long avail = (long)SMEM_LIMIT - (long)v.fixed_smem() - 32;
     if (avail < lower) return false;
     const int LDT = W + 4;
-    const int ms_cap = (int)(avail / ((long)LDT * 4));
-    if (ms_cap < 1) return false;
-    int nsb = 1, MS;
+    const int ds_cap = (int)((avail - red_bytes) / ((long)LDT * 4)) / 2;
+    if (ds_cap < 1) return false;
+    int nsb = 1, DS;
     for (;; ++nsb) {
-        const int msb = (M + nsb - 1) / nsb;
-        MS = (msb + v.CS - 1) / v.CS;
-        if (MS <= ms_cap) break;
+        const int per_sb = (nd + nsb - 1) / nsb;
+        DS = (per_sb + v.CS - 1) / v.CS;
+        if (DS <= ds_cap) break;
     }
-    vp.MS = MS;
-    vp.nsb = (M + MS * v.CS - 1) / (MS * v.CS);
-    vp.u_bytes = round_up(std::max(lower, MS * LDT * 4), 16);
-    vp.smem_bytes = (int)v.fixed_smem() + vp.u_bytes + v.NSTG * vp.stg_floats * 4 + 32;
+    vp.DS = DS;
+    vp.nsb = (nd + DS * v.CS - 1) / (DS * v.CS);
+    vp.DSBp = round_up(DS * v.CS, v.TM1);
+    vp.nch1 = (2 * vp.DSBp + MC1 - 1) / MC1;
+    vp.KT1 = (H / 2 + 1 + v.BK1 - 1) / v.BK1;
+    vp.nrc2 = (2 * DS + v.R2 * v.TM2 - 1) / (v.R2 * v.TM2);
+    vp.nnc2 = (nd + v.Cn2 * v.TN2 - 1) / (v.Cn2 * v.TN2);
+    vp.KT2 = W / (4 * v.G2);
+    vp.ntiles_frame = vp.nsb * (vp.nch1 * vp.KT1 + vp.nrc2 * vp.nnc2 * vp.KT2);
+    vp.u_bytes = round_up(std::max(lower, 2 * DS * LDT * 4 + red_bytes), 16);
+    vp.smem_bytes = (int)v.fixed_smem() + vp.u_bytes + 32;
     return vp.smem_bytes <= SMEM_LIMIT;
+}
+
+// D_H(t) = sin(pi t) cot(pi t / H) / H at t = tnum / u (periodic-sinc weight, Nyquist bin split half/half)
+static double dirichlet_host(long long tnum, int u, int H)
+{
+    const long long den = (long long)u * H;
+    const long long r = ((tnum % den) + den) % den;
+    if (r == 0) return 1.0;
+    const long long r2 = ((tnum % (2LL * u)) + 2LL * u) % (2LL * u);
+    if (r2 == 0 || r2 == u) return 0.0;
+    const double s1 = sin(M_PI * (double)r2 / (double)u);
+    const double x = M_PI * (double)r / (double)den;
+    return s1 * cos(x) / ((double)H * sin(x));
+}
+
+// operand tiles of one variant: stage-1 even/odd Dirichlet tiles, stage-2 cos/sin tiles, the tile schedule
+static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *acc)
+{
+    const CcVariant &v = vp.v;
+    const int c = M / 2, nd = c + 1;
+    const int TF = vp.tile_floats, MC1 = v.R1 * v.TM1, DSB = vp.DS * v.CS;
+    const int n1 = vp.nsb * vp.nch1 * vp.KT1, n2 = vp.nnc2 * vp.KT2;
+    std::vector<float> blob((size_t)(n1 + n2) * TF, 0.f);
+    // position inside a staged k-row -> logical [U|V] column of the chunk (cc_tm1_* chunk layout)
+    std::vector<int> col_of_pos(MC1);
+    for (int tm1 = 0; tm1 < v.R1; ++tm1)
+        for (int ci = 0; ci < cc_tm1_nchunks(v.TM1); ++ci) {
+            const int w = cc_tm1_width(v.TM1, ci), st = cc_tm1_start(v.TM1, ci);
+            for (int i = 0; i < w; ++i) col_of_pos[v.R1 * st + tm1 * w + i] = tm1 * v.TM1 + st + i;
+        }
+    for (int sb = 0; sb < vp.nsb; ++sb)
+        for (int ch = 0; ch < vp.nch1; ++ch)
+            for (int kt = 0; kt < vp.KT1; ++kt) {
+                float *tile = blob.data() + (size_t)((sb * vp.nch1 + ch) * vp.KT1 + kt) * TF;
+                for (int kk = 0; kk < v.BK1; ++kk) {
+                    const int j = kt * v.BK1 + kk;
+                    if (j > H / 2) continue;
+                    for (int pos = 0; pos < MC1; ++pos) {
+                        const int gc = ch * MC1 + col_of_pos[pos];
+                        const bool isV = gc >= vp.DSBp;
+                        const int dsb = gc - (isV ? vp.DSBp : 0);
+                        const int d = sb * DSB + dsb;
+                        if (dsb >= DSB || d >= nd) continue;
+                        double val;
+                        if (j == 0 || j == H / 2) {
+                            val = isV ? 0.0 : dirichlet_host((long long)d - (long long)j * u, u, H);
+                        } else {
+                            const double dm = dirichlet_host((long long)d - (long long)j * u, u, H);
+                            const double dp = dirichlet_host((long long)d + (long long)j * u, u, H);
+                            val = isV ? 0.5 * (dm - dp) : 0.5 * (dm + dp);
+                        }
+                        tile[kk * MC1 + pos] = (float)val;
+                    }
+                }
+            }
+    const int X2 = v.TN2 - 4, GF2 = v.Cn2 * (16 + 4 * X2), NCOL2 = v.Cn2 * v.TN2;
+    const long long denx = (long long)u * W;
+    auto val2 = [&](int k, int e) -> float {
+        if (e >= nd) return 0.f;
+        if (k == 0) return 1.f;
+        if (k == 1) return 0.f;  // Nyquist column: added in the stage-2 epilogue with nyqc
+        const int q = k / 2;
+        const long long num = ((long long)q * e) % denx;
+        const double th = 2.0 * M_PI * (double)num / (double)denx;
+        return (float)((k & 1) ? 2.0 * sin(th) : 2.0 * cos(th));
+    };
+    for (int nc2 = 0; nc2 < vp.nnc2; ++nc2)
+        for (int kt = 0; kt < vp.KT2; ++kt) {
+            float *tile = blob.data() + (size_t)(n1 + nc2 * vp.KT2 + kt) * TF;
+            for (int g = 0; g < v.G2; ++g)
+                for (int kk = 0; kk < 4; ++kk) {
+                    const int k = (kt * v.G2 + g) * 4 + kk;
+                    for (int col = 0; col < v.Cn2 * 4; ++col)
+                        tile[g * GF2 + kk * v.Cn2 * 4 + col] = val2(k, nc2 * NCOL2 + col);
+                    if (X2)
+                        for (int tn = 0; tn < v.Cn2; ++tn)
+                            tile[g * GF2 + 16 * v.Cn2 + tn * 4 + kk] = val2(k, nc2 * NCOL2 + 4 * v.Cn2 + tn);
+                }
+        }
+    std::vector<uint32_t> sched;
+    for (int sb = 0; sb < vp.nsb; ++sb) {
+        for (int ch = 0; ch < vp.nch1; ++ch)
+            for (int kt = 0; kt < vp.KT1; ++kt) sched.push_back((uint32_t)((sb * vp.nch1 + ch) * vp.KT1 + kt));
+        for (int rc = 0; rc < vp.nrc2; ++rc)
+            for (int nc2 = 0; nc2 < vp.nnc2; ++nc2)
+                for (int kt = 0; kt < vp.KT2; ++kt) sched.push_back((uint32_t)(n1 + nc2 * vp.KT2 + kt));
+    }
+    std::vector<float> nyq((size_t)vp.nnc2 * NCOL2, 0.f);
+    for (int e = 0; e < nd; ++e) {
+        const long long r2 = (long long)e % (2LL * u);
+        nyq[e] = (float)cos(M_PI * (double)r2 / (double)u);
+    }
+    cudaError_t e = upload(&vp.blob, blob, acc);
+    if (e == cudaSuccess) e = upload(&vp.sched, sched, acc);
+    if (e == cudaSuccess) e = upload(&vp.nyqc, nyq, acc);
+    return e;
 }
 
 static cc_status check_device()
@@ -179,8 +278,8 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
 {
     if (!plan) return CC_OK;
     cudaFree(plan->tw), cudaFree(plan->Gt), cudaFree(plan->row_slot), cudaFree(plan->col_partner);
-    cudaFree(plan->ab), cudaFree(plan->Dt), cudaFree(plan->AxT);
-    cudaFree(plan->thr.Sg), cudaFree(plan->lat.Sg);
+    cudaFree(plan->ab);
+    for (VarPlan *vp : {&plan->thr, &plan->lat}) cudaFree(vp->Sg), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
         if (plan->hev[i]) cudaEventDestroy(plan->hev[i]);
@@ -276,52 +375,16 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
         ab[p] = make_float4((float)g0.real(), (float)g0.imag(), (float)gn.real(), (float)gn.imag());
     }
 
-    int maxMC1 = pl->thr.MC1, np2 = pl->thr.np2_need;
-    if (pl->has_lat) maxMC1 = std::max(maxMC1, pl->lat.MC1), np2 = std::max(np2, pl->lat.np2_need);
-    pl->Mp1 = round_up(M, 4) + round_up(maxMC1, 4);
-    pl->Np2 = np2;
-    std::vector<float> Dt((size_t)H * pl->Mp1, 0.f), AxT((size_t)W * pl->Np2, 0.f);
-    if (u > 1) {
-        // Dt[j][m] = D_H((m - c)/u - j),  D_H(t) = sin(pi t) cot(pi t / H) / H   (Nyquist bin split half/half)
-        for (int j = 0; j < H; ++j)
-            for (int m = 0; m < M; ++m) {
-                const long long tnum = (long long)(m - c) - (long long)j * u;  // t = tnum / u
-                const long long den = (long long)u * H;
-                long long r = ((tnum % den) + den) % den;
-                double d;
-                if (r == 0) d = 1.0;
-                else {
-                    long long r2 = ((tnum % (2LL * u)) + 2LL * u) % (2LL * u);
-                    const double s1 = sin(M_PI * (double)r2 / (double)u);
-                    const double x = M_PI * (double)r / (double)den;
-                    d = (r2 == 0 || r2 == u) ? 0.0 : s1 * cos(x) / ((double)H * sin(x));
-                }
-                Dt[(size_t)j * pl->Mp1 + m] = (float)d;
-            }
-        // AxT[2q][n] = w_q cos(theta), AxT[2q+1][n] = -w_q sin(theta), theta = 2 pi q (n - c) / (u W);
-        // packed column q = 0: (1, cos(pi (n - c) / u))
-        const long long denx = (long long)u * W;
-        for (int n = 0; n < M; ++n) {
-            AxT[(size_t)0 * pl->Np2 + n] = 1.f;
-            long long r2 = (((long long)(n - c) % (2LL * u)) + 2LL * u) % (2LL * u);
-            AxT[(size_t)1 * pl->Np2 + n] = (float)cos(M_PI * (double)r2 / (double)u);
-            for (int q = 1; q < Wh; ++q) {
-                long long num = (((long long)q * (n - c)) % denx + denx) % denx;
-                const double th = 2.0 * M_PI * (double)num / (double)denx;
-                AxT[(size_t)(2 * q) * pl->Np2 + n] = (float)(2.0 * cos(th));
-                AxT[(size_t)(2 * q + 1) * pl->Np2 + n] = (float)(-2.0 * sin(th));
-            }
-        }
-    }
-
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = upload(&pl->tw, tw, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->row_slot, row_slot, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->col_partner, col_partner, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->Gt, Gt, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->ab, ab, &pl->table_bytes);
-    if (e == cudaSuccess) e = upload(&pl->Dt, Dt, &pl->table_bytes);
-    if (e == cudaSuccess) e = upload(&pl->AxT, AxT, &pl->table_bytes);
+    if (u > 1) {
+        if (e == cudaSuccess) e = build_tiles(pl->thr, H, W, u, M, &pl->table_bytes);
+        if (e == cudaSuccess && pl->has_lat) e = build_tiles(pl->lat, H, W, u, M, &pl->table_bytes);
+    }
 
     // ---- kernel attributes, occupancy, scratch
     VarPlan *vps[2] = {&pl->thr, pl->has_lat ? &pl->lat : nullptr};
@@ -352,10 +415,11 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
 static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
 {
     p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
-    p.Dt = pl->Dt, p.AxT = pl->AxT, p.Sg = vp.Sg;
-    p.u = pl->u, p.M = pl->M, p.c = pl->c, p.Mp1 = pl->Mp1, p.Np2 = pl->Np2;
-    p.MS = vp.MS, p.nsb = vp.nsb, p.NCH2 = vp.NCH2, p.TPN2 = vp.TPN2;
-    p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.stg_floats = vp.stg_floats, p.Emean = pl->Emean;
+    p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg;
+    p.u = pl->u, p.M = pl->M, p.c = pl->c, p.nd = pl->c + 1;
+    p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
+    p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
+    p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.Emean = pl->Emean;
 }
 
 static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,

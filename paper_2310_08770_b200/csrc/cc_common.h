@@ -34,9 +34,21 @@ static inline int cc_freq_of_slot(int N, int p)
     return k;
 }
 
+// TM1 split into vector chunks: widths 4,4,2 / 4,1 / ... ; chunk ci of thread-row tm1 sits at
+// R1 * start(ci) + tm1 * width(ci) inside a staged k-row of MC1 floats.
+__host__ __device__ constexpr int cc_tm1_nchunks(int tm1) { return tm1 == 10 ? 3 : (tm1 == 5 || tm1 == 8 || tm1 == 3) ? 2 : 1; }
+__host__ __device__ constexpr int cc_tm1_width(int tm1, int ci)
+{
+    return tm1 == 10 ? (ci < 2 ? 4 : 2) : tm1 == 8 ? 4 : tm1 == 5 ? (ci == 0 ? 4 : 1) : tm1 == 3 ? (ci == 0 ? 2 : 1) : tm1;
+}
+__host__ __device__ constexpr int cc_tm1_start(int tm1, int ci)
+{
+    return ci == 0 ? 0 : ci == 1 ? cc_tm1_width(tm1, 0) : cc_tm1_width(tm1, 0) + cc_tm1_width(tm1, 1);
+}
+
 // Phases of the per-frame breakdown (cc_track_profile): 0 ingest + row FFT, 1 column FFT (x) conj(G) +
-// column inverse, 2 row C2R + integer argmax, 3 fp64 integer polish, 4 upsampled stage 1 (sum over
-// super-blocks: last one), 5 upsampled stage 2, 6 sub-pixel argmax reduction, 7 fp64 sub-pixel polish.
+// column inverse, 2 row C2R + integer argmax, 3 fp64 integer polish, 4 upsampled stage 1 (last
+// super-block), 5 upsampled stage 2, 6 sub-pixel argmax reduction, 7 fp64 sub-pixel polish.
 #define CC_NPHASE 8
 
 // Kernel parameters (passed by value).  All table pointers are device memory
@@ -53,29 +65,35 @@ struct CcParams {
     const float2 *Gt;             // [H][W/2]: conj(G[ky(p)][q]) / (H W), p = column slot; q = 0 unused
     const float4 *ab;             // [H]: conj(G)/(HW) of columns kx = 0 (DC bin zeroed) and kx = W/2, by slot
     const uint16_t *col_partner;  // [H]: slot of -ky for the frequency at slot p
-    const float *Dt;              // [H][Mp1]: Dirichlet interpolation matrix, j-major
-    const float *AxT;             // [W][Np2]: x-axis upsampling matrix, k-major (re, -im interleaved along k)
+    const float *blob;            // staged GEMM operand tiles (stage-1 even/odd Dirichlet tiles, stage-2 cos/sin tiles),
+                                  // tile t at blob + t * tile_floats
+    const uint32_t *sched;        // [ntiles_frame] blob tile index of the i-th tile a frame consumes
+    const float *nyqc;            // [ne_pad] cos(pi e / u): Nyquist-column weight of stage 2
     float2 *Sg;                   // global spectrum scratch (variants with S in L2), else null
 
-    int u, M, c;  // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
-    int Mp1;      // padded row length of Dt
-    int Np2;      // padded row length of AxT
-    int MS;       // rows of T held per CTA per super-block
-    int nsb;      // number of super-blocks
-    int NCH2;     // staged width (floats) of an AxT tile
-    int TPN2;     // threads across n in stage 2
-    int c0;       // integer constant subtracted from every pixel before the FFT
-    int u_bytes;  // bytes of the raw/scratch/T union region
-    int stg_floats;  // floats per staging buffer
-    double Emean;    // mean of the reference image (DC add-back for `peak`)
+    int u, M, c;        // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
+    int nd;             // c + 1: number of |offsets| d (and e) evaluated per axis
+    int DS;             // offsets d owned per CTA per super-block (T holds 2*DS rows)
+    int nsb;            // number of super-blocks
+    int DSBp;           // DS*CS rounded up to a multiple of TM1: U columns of a stage-1 super-block
+    int nch1;           // stage-1 column chunks per super-block
+    int KT1;            // stage-1 k-tiles (of BK1 rows j)
+    int nrc2, nnc2;     // stage-2 row chunks / e-column chunks
+    int ntiles_frame;   // tiles consumed per frame
+    int tile_floats;    // floats per staging slot
+    int c0;             // integer constant subtracted from every pixel before the FFT
+    int u_bytes;        // bytes of the raw/scratch/T union region
+    double Emean;       // mean of the reference image (DC add-back for `peak`)
 };
 
 // Launcher interface of one compiled kernel variant.
 struct CcVariant {
     int H, W, CS, NT, dtype;  // dtype: 0 = u8, 1 = u16
     int TM1, TN1, TM2, TN2;
+    int R1, Cn1, R2, Cn2, KS2;  // thread grids of the two GEMM stages (rows x cols [x k-split])
+    int BK1, G2;                // stage-1 k-rows per tile; stage-2 groups of 4 k-rows per tile
     int s_global;  // 1: spectrum array lives in global memory (L2), 0: shared memory / DSMEM
-    int BK, NSTG;
+    int NSTG;
     size_t (*fixed_smem)();                 // bytes that do not depend on M (S, tables, misc), before U/stg
     int (*raw_scratch_bytes)();             // raw ring + FFT scratch (lower bound of the U region)
     cudaError_t (*prepare)(int smem_bytes);  // sets func attributes

@@ -9,8 +9,11 @@
 //   a3 product   : fused into the last forward / first inverse column pass
 //   a4 inv FFT   : column inverse -> Q[y][kx] (kept: it feeds a6), row C2R
 //   a5 argmax    : streamed out of the row C2R, never stored; fp64 3x3 polish
-//   a6 upsampled : stage 1  T = D(real Dirichlet) * Q      (FP32 register-tiled GEMM)
-//                  stage 2  C = T' * AxT                   (FP32 register-tiled GEMM)
+//   a6 upsampled : both upsampling matrices are even/odd-symmetric about the window centre, so
+//                  stage 1  [T(c+d) + T(c-d), T(c+d) - T(c-d)] = [Ee, Eo] * [Q(y0+j) + Q(y0-j), Q(y0+j) - Q(y0-j)]
+//                  stage 2  [C(m,c+e) + C(m,c-e), C(m,c-e) - C(m,c+e)] / 2 = [T_re * cos, T_im * sin]
+//                  (FP32 register-tiled GEMMs with half the multiply-adds of the plain products);
+//                  operand tiles stream L2 -> smem through a TMA ring with full/empty mbarriers
 //   a7 argmax    : streamed out of stage 2, fp64 3x3 hill-climb polish, compose
 // Product code: shares nothing with oracle/.
 #pragma once
@@ -24,10 +27,10 @@
 namespace ccf {
 namespace cg = cooperative_groups;
 
-constexpr int BK = 8;     // k-depth of a staged GEMM tile
-constexpr int NSTG = 3;   // staging ring depth
+constexpr int NSTG = 6;   // staging ring depth
+constexpr int PFD = 4;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
 constexpr int XN = 10;    // doubles per cluster-exchange record
-constexpr int NBARS = NSTG + 2;
+constexpr int NBARS = 2 * NSTG + 2;  // full[NSTG], empty[NSTG], raw ring [2]
 
 // ------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -38,6 +41,10 @@ __device__ __forceinline__ void mbar_init(uint64_t *b, uint32_t cnt)
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity)
 {
@@ -242,11 +249,33 @@ __device__ __forceinline__ double dirichlet64(long long tnum, int u, int Hn)
     return s1 * cospi(x) / ((double)Hn * sinpi(x));
 }
 
+// Even / odd parts of the Dirichlet weight about row offset j (0 < j < H/2), t = tnum / u, |t| < 1:
+//   we = (D_H(t-j) + D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2x) / (2 H sin(x-y) sin(x+y)),
+//   wo = (D_H(t-j) - D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2y) / (2 H sin(x-y) sin(x+y)),
+// x = pi t / H, y = pi j / H; every sine gets an exactly reduced integer phase numerator.
+__device__ __forceinline__ double sinpi_frac(long long num, long long den)  // sin(pi num / den)
+{
+    long long r = num % (2 * den);
+    if (r < 0) r += 2 * den;
+    return sinpi((double)r / (double)den);
+}
+__device__ __forceinline__ void dirichlet_pair64(long long tnum, int j, int u, int Hn, double *we, double *wo)
+{
+    const long long den = (long long)u * Hn;
+    const double s = sinpi_frac(tnum, u);
+    const double sa = sinpi_frac(tnum - (long long)j * u, den), sb = sinpi_frac(tnum + (long long)j * u, den);
+    const double pref = ((j & 1) ? -s : s) / (2.0 * (double)Hn * sa * sb);
+    *we = pref * sinpi_frac(2 * tnum, den);
+    *wo = pref * sinpi_frac(2LL * j, Hn);
+}
+
 // ------------------------------------------------------------------ the kernel
-template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_>
+template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
+          int R2_, int KS2_>
 struct Cfg {
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
+    static constexpr int BK1 = BK1_, G2 = G2_, R2 = R2_, KS2 = KS2_;
     static constexpr bool SG = SG_;
     using PIX = PIX_;
     static constexpr int NC = W / 2 / CS;   // spectrum columns per CTA (column 0 of rank 0 packs DC + Nyquist)
@@ -261,17 +290,40 @@ struct Cfg {
     static constexpr int CHB = RCH * W * (int)sizeof(PIX);
     static constexpr int RAWB = (NCHK > 1 ? 2 : 1) * CHB;
     static constexpr int SCRB = NWARP * PADW * 8;
-    static constexpr int TPN1 = 2 * NC / TN1;
-    static constexpr int TPM1 = NT / TPN1;
-    static constexpr int MC1 = TPM1 * TM1;
+    // stage 1: thread grid R1 (rows of [U|V]) x Cn1 (groups of TN1 spectrum floats); a warp covers WR1 x WC1 threads
+    static constexpr int Cn1 = 2 * NC / TN1;
+    static constexpr int R1 = NT / Cn1;
+    static constexpr int WC1 = Cn1 < 8 ? Cn1 : 8;
+    static constexpr int WR1 = 32 / WC1;
+    static constexpr int WG1C = Cn1 / WC1;
+    static constexpr int MC1 = R1 * TM1;          // [U|V] columns per stage-1 chunk
+    static constexpr int T1F = BK1 * MC1;         // floats of a stage-1 tile
+    // stage 2: thread grid R2 x Cn2 x KS2 (k-split); a warp covers WR2 x WC2 threads of one k-slice
+    static constexpr int Cn2 = NT / (R2 * KS2);
+    static constexpr int WC2 = Cn2 < 8 ? Cn2 : 8;
+    static constexpr int WR2 = 32 / WC2;
+    static constexpr int WG2C = Cn2 / WC2;
+    static constexpr int WG2R = R2 / WR2;
+    static constexpr int X2 = TN2 - 4;                  // 0 or 1 extra e-column per thread
+    static constexpr int GF2 = Cn2 * (16 + 4 * X2);      // floats of one group of 4 k-rows
+    static constexpr int T2F = G2 * GF2;                 // floats of a stage-2 tile
+    static constexpr int NCOL2 = Cn2 * TN2;              // e-columns per stage-2 chunk
+    static constexpr int TILEF = T1F > T2F ? T1F : T2F;  // floats per staging slot
+    static constexpr int RED_FLOATS = (KS2 - 1) * R2 * Cn2 * 2 * TM2 * TN2;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
     static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64;
-    static constexpr size_t FIXED_BYTES = S_BYTES + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES;
+    static constexpr size_t FIXED_BYTES = S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES;
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
     static_assert(NR % RCH == 0 && RCH % 2 == 0, "bad raw chunking");
-    static_assert((2 * NC) % TN1 == 0 && NT % TPN1 == 0 && TN1 % 2 == 0 && MC1 % 4 == 0, "bad stage-1 tiling");
+    static_assert((2 * NC) % TN1 == 0 && NT % Cn1 == 0 && TN1 % 4 == 0 && Cn1 % WC1 == 0 && 32 % WC1 == 0, "bad stage-1 tiling");
+    static_assert(R1 % 4 == 0 && R1 % WR1 == 0 && (R1 / WR1) * WG1C == NWARP, "bad stage-1 warp grid");
+    static_assert(TM1 == 1 || TM1 == 2 || TM1 == 3 || TM1 == 4 || TM1 == 5 || TM1 == 8 || TM1 == 10, "TM1 chunking");
+    static_assert(R2 * Cn2 * KS2 == NT && Cn2 % WC2 == 0 && 32 % WC2 == 0 && R2 % WR2 == 0, "bad stage-2 tiling");
+    static_assert(WG2R * WG2C * KS2 == NWARP && (TN2 == 4 || TN2 == 5) && G2 % KS2 == 0 && W % (4 * G2) == 0, "bad stage-2 tiling");
+    static_assert(TILEF % 4 == 0 && MC1 % 4 == 0, "tile alignment");
     static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
+    static_assert(NSTG - PFD >= 2, "ring");
 };
 
 template <class C>
@@ -279,7 +331,6 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 {
     constexpr int H = C::H, W = C::W, CS = C::CS, NT = C::NT, NC = C::NC, NR = C::NR;
     constexpr int NWARP = C::NWARP, NTW = C::NTW, PADW = C::PADW;
-    constexpr int TM1 = C::TM1, TN1 = C::TN1, TM2 = C::TM2, TN2 = C::TN2;
     constexpr int LDT = C::LDT;
     constexpr bool SG = C::SG;
     using PIX = typename C::PIX;
@@ -292,13 +343,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     // ---- shared memory carve-up
     float2 *const Ssm = reinterpret_cast<float2 *>(smem);
-    unsigned char *const U = smem + C::S_BYTES;
-    float *const stg = reinterpret_cast<float *>(U + p.u_bytes);
-    float2 *const tw = reinterpret_cast<float2 *>(stg + NSTG * p.stg_floats);
+    float *const stg = reinterpret_cast<float *>(smem + C::S_BYTES);        // [NSTG][TILEF] operand ring
+    unsigned char *const U = reinterpret_cast<unsigned char *>(stg + NSTG * C::TILEF);
+    float2 *const tw = reinterpret_cast<float2 *>(U + p.u_bytes);
     uint16_t *const rslot = reinterpret_cast<uint16_t *>(tw + NTW);
     unsigned char *misc = reinterpret_cast<unsigned char *>(rslot + W);
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
-    uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // [NSTG] staging, [NSTG..NSTG+1] raw ring
+    uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
+    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
     float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
@@ -325,12 +377,42 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     for (int i = tid; i < NTW; i += NT) tw[i] = p.tw[i];
     for (int i = tid; i < W; i += NT) rslot[i] = p.row_slot[i];
     if (tid == 0) {
-        for (int i = 0; i < NBARS; ++i) mbar_init(&bars[i], 1);
+        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
+        mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
         fence_mbar_init();
     }
-    uint32_t ph = 0;   // mbarrier phase parity bits, one per barrier
+    uint32_t ph = 0;   // phase parity bits of the raw ring
     int xpar = 0;      // exchange buffer parity
     csync();
+
+    // ---- operand ring: every frame consumes the same p.ntiles_frame tiles of p.blob in the order of
+    // p.sched.  Thread 0 keeps PFD tiles in flight (also across frames and phases); a slot is refilled
+    // once all NWARP warps have released it (empty mbarrier) -- no CTA barrier inside the GEMM loops.
+    const uint32_t my_frames = p.batch > cid ? (uint32_t)((p.batch - cid + ncl - 1) / ncl) : 0u;
+    const uint32_t total_tiles = my_frames * (uint32_t)p.ntiles_frame;
+    uint32_t g_cons = 0, g_load = 0, s_idx = 0;
+    auto ring_produce = [&]() {  // thread 0 only
+        const uint32_t slot = g_load % NSTG;
+        mbar_wait(&bempty[slot], ((g_load / NSTG) & 1u) ^ 1u);
+        const uint32_t ti = __ldg(&p.sched[s_idx]);
+        mbar_expect_tx(&bfull[slot], (uint32_t)C::TILEF * 4u);
+        bulk_g2s(stg + (size_t)slot * C::TILEF, p.blob + (size_t)ti * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[slot]);
+        ++g_load;
+        if (++s_idx == (uint32_t)p.ntiles_frame) s_idx = 0;
+    };
+    auto ring_acquire = [&]() -> const float * {
+        if (tid == 0 && g_load < total_tiles) ring_produce();
+        const uint32_t slot = g_cons % NSTG;
+        mbar_wait(&bfull[slot], (g_cons / NSTG) & 1u);
+        return stg + (size_t)slot * C::TILEF;
+    };
+    auto ring_release = [&]() {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bempty[g_cons % NSTG]);
+        ++g_cons;
+    };
+    if (tid == 0)
+        for (int i = 0; i < PFD && g_load < total_tiles; ++i) ring_produce();
 
     const int u = p.u, M = p.M, cM = p.c;
 
@@ -369,20 +451,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         return r;
     };
 
-    // staged GEMM operand tiles: BK rows of `rowlen` floats, row r of tile t at src + (t*BK + r)*ld
-    auto stage_issue = [&](int slot, const float *src, int t, int ld, int rowlen) {
-        // called by thread 0 only
-        mbar_expect_tx(&bars[slot], (uint32_t)(BK * rowlen * 4));
-        float *dst = stg + (size_t)slot * p.stg_floats;
-        if (ld == rowlen) {
-            bulk_g2s(dst, src + (size_t)t * BK * ld, (uint32_t)(BK * rowlen * 4), &bars[slot]);
-        } else {
-            for (int r = 0; r < BK; ++r)
-                bulk_g2s(dst + r * rowlen, src + ((size_t)t * BK + r) * ld, (uint32_t)(rowlen * 4), &bars[slot]);
-        }
-    };
-    auto bar_wait = [&](int b) {
-        mbar_wait(&bars[b], (ph >> b) & 1u);
+    auto bar_wait = [&](int b) {  // raw ring barriers
+        mbar_wait(&braw[b], (ph >> b) & 1u);
         ph ^= 1u << b;
     };
 
@@ -445,8 +515,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             if (tid == 0) {
                 fence_proxy_async();
                 for (int ck = 0; ck < (C::NCHK > 1 ? 2 : 1); ++ck) {
-                    mbar_expect_tx(&bars[NSTG + ck], C::CHB);
-                    bulk_g2s(raw + (size_t)ck * C::RCH * W, fbase + (size_t)ck * C::RCH * W, C::CHB, &bars[NSTG + ck]);
+                    mbar_expect_tx(&braw[ck], C::CHB);
+                    bulk_g2s(raw + (size_t)ck * C::RCH * W, fbase + (size_t)ck * C::RCH * W, C::CHB, &braw[ck]);
                 }
                 if (f + ncl < p.batch) {  // pull the next frame of this cluster into L2
                     const PIX *nb = fbase + (size_t)ncl * H * W;
@@ -458,7 +528,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             const float c0f = (float)p.c0;
             for (int ck = 0; ck < C::NCHK; ++ck) {
                 const int rb = ck & 1;
-                bar_wait(NSTG + rb);
+                bar_wait(rb);
                 const PIX *rw = raw + (size_t)rb * C::RCH * W;
                 for (int jp = warp; jp < C::RCH / 2; jp += NWARP) {
                     const PIX *ra = rw + (size_t)jp * W;
@@ -488,8 +558,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
                 __syncthreads();
                 if (tid == 0 && ck + 2 < C::NCHK) {
-                    mbar_expect_tx(&bars[NSTG + rb], C::CHB);
-                    bulk_g2s(raw + (size_t)rb * C::RCH * W, fbase + (size_t)(ck + 2) * C::RCH * W, C::CHB, &bars[NSTG + rb]);
+                    mbar_expect_tx(&braw[rb], C::CHB);
+                    bulk_g2s(raw + (size_t)rb * C::RCH * W, fbase + (size_t)(ck + 2) * C::RCH * W, C::CHB, &braw[rb]);
                 }
             }
         }
@@ -681,144 +751,223 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             continue;
         }
 
-        // =============================================================== a6/a7: upsampled DFT as two FP32 GEMMs
+        // =============================================================== a6/a7: upsampled DFT as two symmetric FP32 GEMMs
+        // Row pairs about the integer peak become their sum and difference (in place):
+        //   S[(y0+j)] <- Q(y0+j) + Q(y0-j),  S[(y0-j)] <- Q(y0+j) - Q(y0-j),  0 < j < H/2.
+        for (int idx = tid; idx < (H / 2 - 1) * NC; idx += NT) {
+            const int j = 1 + idx / NC, ql = idx % NC;
+            float2 *pa = Sl + (size_t)((y0 + j) & (H - 1)) * NC + ql, *pb = Sl + (size_t)((y0 - j) & (H - 1)) * NC + ql;
+            const float2 a = *pa, b = *pb;
+            *pa = make_float2(a.x + b.x, a.y + b.y);
+            *pb = make_float2(a.x - b.x, a.y - b.y);
+        }
+        __syncthreads();
+
         Best sub{-INFINITY, 0x7fffffff};
         {
-            const int MS = p.MS, MSB = MS * CS;
-            constexpr int TPN1 = C::TPN1, MC1 = C::MC1;
-            const int tn1 = tid % TPN1, tm1 = tid / TPN1;
-            const int TPN2 = p.TPN2, TPM2 = NT / TPN2, NCH2 = p.NCH2;
-            const int tn2 = tid % TPN2, tm2 = tid / TPN2;
-            for (int mb = 0; mb < M; mb += MSB) {
-                const int mend = min(M, mb + MSB);
-                // ---------------- stage 1: T[m][kx] = sum_j Dt[j][m] * Q[(y0+j) mod H][kx]
-                for (int mc = mb; mc < mend; mc += MC1) {
+            const int DS = p.DS, nd = p.nd, DSBp = p.DSBp, DSB = DS * CS;
+            constexpr int TN1 = C::TN1, TM1 = C::TM1, MC1 = C::MC1, R1 = C::R1, Cn1 = C::Cn1, BK1 = C::BK1;
+            constexpr int TM2 = C::TM2, TN2 = C::TN2, R2 = C::R2, Cn2 = C::Cn2, KS2 = C::KS2, G2 = C::G2, GF2 = C::GF2;
+            const int tn1 = (warp % C::WG1C) * C::WC1 + lane % C::WC1;
+            const int tm1 = (warp / C::WG1C) * C::WR1 + lane / C::WC1;
+            const int ks2 = warp / (C::WG2R * C::WG2C), w2 = warp % (C::WG2R * C::WG2C);
+            const int tn2 = (w2 % C::WG2C) * C::WC2 + lane % C::WC2;
+            const int tm2 = (w2 / C::WG2C) * C::WR2 + lane / C::WC2;
+            float *const red = Tb + (size_t)2 * DS * LDT;  // k-split partial sums (KS2 > 1)
+            for (int sb = 0; sb < p.nsb; ++sb) {
+                const int db = sb * DSB;
+                // ---------------- stage 1: rows [U(d) | V(d)] of this super-block, my 2*NC spectrum floats
+                //   U(d) = sum_j Ee[d][j] S[(y0+j)],  V(d) = sum_j Eo[d][j] S[(y0-j)];  T(c+d) = U+V, T(c-d) = U-V
+                for (int ch = 0; ch < p.nch1; ++ch) {
+                    const int gc0 = ch * MC1 + tm1 * TM1;
+                    const bool isV = gc0 >= DSBp;
                     float acc[TM1][TN1];
 #pragma unroll
                     for (int i = 0; i < TM1; ++i)
 #pragma unroll
                         for (int j = 0; j < TN1; ++j) acc[i][j] = 0.f;
-                    constexpr int NKT = H / BK;
-                    const float *Asrc = p.Dt + mc;
-                    if (tid == 0)
-                        for (int t = 0; t < NSTG - 1 && t < NKT; ++t) stage_issue(t % NSTG, Asrc, t, p.Mp1, MC1);
-                    for (int kt = 0; kt < NKT; ++kt) {
-                        const int slot = kt % NSTG;
-                        if (tid == 0 && kt + NSTG - 1 < NKT) stage_issue((kt + NSTG - 1) % NSTG, Asrc, kt + NSTG - 1, p.Mp1, MC1);
-                        bar_wait(slot);
-                        const float *At = stg + (size_t)slot * p.stg_floats + tm1 * TM1;
+                    for (int kt = 0; kt < p.KT1; ++kt) {
+                        const float *At = ring_acquire();
 #pragma unroll
-                        for (int kk = 0; kk < BK; ++kk) {
-                            const int ys = (y0 + kt * BK + kk) & (H - 1);
+                        for (int kk = 0; kk < BK1; ++kk) {
+                            const int jj = kt * BK1 + kk;
+                            const int ys = (isV ? y0 - jj : y0 + jj) & (H - 1);
                             float a[TM1], b[TN1];
-                            load_vec<TM1>(a, At + kk * MC1);
-                            load_vec<TN1>(b, reinterpret_cast<const float *>(Sl + (size_t)ys * NC) + tn1 * TN1);
+#pragma unroll
+                            for (int ci = 0; ci < cc_tm1_nchunks(TM1); ++ci) {
+                                const int w = cc_tm1_width(TM1, ci), st = cc_tm1_start(TM1, ci);
+                                const float *src = At + kk * MC1 + R1 * st + tm1 * w;
+                                if (w == 4) {
+                                    const float4 t = *reinterpret_cast<const float4 *>(src);
+                                    a[st] = t.x, a[st + 1] = t.y, a[st + 2] = t.z, a[st + 3] = t.w;
+                                } else if (w == 2) {
+                                    const float2 t = *reinterpret_cast<const float2 *>(src);
+                                    a[st] = t.x, a[st + 1] = t.y;
+                                } else {
+                                    a[st] = src[0];
+                                }
+                            }
+                            const float *brow = reinterpret_cast<const float *>(Sl + (size_t)ys * NC) + tn1 * 4;
+#pragma unroll
+                            for (int v = 0; v < TN1 / 4; ++v) {
+                                const float4 t = *reinterpret_cast<const float4 *>(brow + v * Cn1 * 4);
+                                b[4 * v] = t.x, b[4 * v + 1] = t.y, b[4 * v + 2] = t.z, b[4 * v + 3] = t.w;
+                            }
 #pragma unroll
                             for (int i = 0; i < TM1; ++i)
 #pragma unroll
                                 for (int j = 0; j < TN1; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
                         }
-                        __syncthreads();  // slot may be refilled
+                        ring_release();
                     }
-                    // epilogue: rotate by exp(2 pi i kx x0 / W), send rows to the CTA that owns them in stage 2
+                    // epilogue: rotate by exp(2 pi i kx x0 / W), send rows to the CTA that owns offset d
 #pragma unroll
-                    for (int j = 0; j < TN1 / 2; ++j) {
-                        const int q = rank * NC + tn1 * (TN1 / 2) + j;
-                        if (q == 0) {
-                            const float sg = (x0 & 1) ? -1.f : 1.f;
+                    for (int v = 0; v < TN1 / 4; ++v)
 #pragma unroll
-                            for (int i = 0; i < TM1; ++i) acc[i][2 * j + 1] *= sg;
-                        } else {
-                            const float2 w = tw[((q * x0) & (W - 1)) * (NTW / W)];  // (cos, -sin)
+                        for (int pp = 0; pp < 2; ++pp) {
+                            const int q = rank * NC + v * Cn1 * 2 + tn1 * 2 + pp;
+                            const int j0 = 4 * v + 2 * pp;
+                            if (q == 0) {
+                                const float sg = (x0 & 1) ? -1.f : 1.f;
 #pragma unroll
-                            for (int i = 0; i < TM1; ++i) {
-                                const float2 t = cmulc(make_float2(acc[i][2 * j], acc[i][2 * j + 1]), w);
-                                acc[i][2 * j] = t.x;
-                                acc[i][2 * j + 1] = t.y;
+                                for (int i = 0; i < TM1; ++i) acc[i][j0 + 1] *= sg;
+                            } else {
+                                const float2 w = tw[((q * x0) & (W - 1)) * (NTW / W)];  // (cos, -sin)
+#pragma unroll
+                                for (int i = 0; i < TM1; ++i) {
+                                    const float2 t = cmulc(make_float2(acc[i][j0], acc[i][j0 + 1]), w);
+                                    acc[i][j0] = t.x;
+                                    acc[i][j0 + 1] = t.y;
+                                }
                             }
                         }
-                    }
 #pragma unroll
                     for (int i = 0; i < TM1; ++i) {
-                        const int m = mc + tm1 * TM1 + i;
-                        if (m < mend) {
-                            const int dr = (m - mb) / MS, row = (m - mb) % MS;
+                        const int dsb = gc0 + i - (isV ? DSBp : 0);
+                        if (dsb < DSB && db + dsb < nd) {
+                            const int dr = dsb / DS, row = dsb % DS + (isV ? DS : 0);
                             float *Td = Tb;
                             if constexpr (CS > 1) Td = cluster.map_shared_rank(Tb, dr);
-                            float *dst = Td + (size_t)row * LDT + 2 * (rank * NC + tn1 * (TN1 / 2));
-                            if constexpr (TN1 % 4 == 0) {
+                            float *dst = Td + (size_t)row * LDT + rank * 2 * NC + tn1 * 4;
 #pragma unroll
-                                for (int j = 0; j < TN1 / 4; ++j)
-                                    reinterpret_cast<float4 *>(dst)[j] =
-                                        make_float4(acc[i][4 * j], acc[i][4 * j + 1], acc[i][4 * j + 2], acc[i][4 * j + 3]);
-                            } else {
-#pragma unroll
-                                for (int j = 0; j < TN1 / 2; ++j)
-                                    reinterpret_cast<float2 *>(dst)[j] = make_float2(acc[i][2 * j], acc[i][2 * j + 1]);
-                            }
+                            for (int v = 0; v < TN1 / 4; ++v)
+                                *reinterpret_cast<float4 *>(dst + v * Cn1 * 4) =
+                                    make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]);
                         }
                     }
                 }
-                csync();  // T rows are at their owners
+                csync();  // U, V rows are at their owners
+                // rows dl and DS+dl become T(c+d) = U+V and T(c-d) = U-V
+                for (int idx = tid; idx < DS * (W / 4); idx += NT) {
+                    const int dl = idx / (W / 4), c4 = idx % (W / 4);
+                    float4 *pu = reinterpret_cast<float4 *>(Tb + (size_t)dl * LDT) + c4;
+                    float4 *pv = reinterpret_cast<float4 *>(Tb + (size_t)(DS + dl) * LDT) + c4;
+                    const float4 a = *pu, b = *pv;
+                    *pu = make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w);
+                    *pv = make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w);
+                }
+                __syncthreads();
                 stamp(4, f);
 
-                // ---------------- stage 2: C[m][n] = sum_k T[m][k] * AxT[k][n], streamed into the argmax
-                {
-                    const int mrow0 = mb + rank * MS;  // global m of my T row 0
-                    const int nrows = max(0, min(MS, mend - mrow0));
-                    for (int rc = 0; rc < nrows; rc += TPM2 * TM2) {
-                        for (int nc = 0; nc < M; nc += TPN2 * TN2) {
-                            float acc[TM2][TN2];
+                // ---------------- stage 2: E(m,e) = sum_q T_re w cos, O(m,e) = sum_q T_im w sin;
+                //   C(m, c+e) = E - O,  C(m, c-e) = E + O, streamed into the argmax
+                const int d0 = db + rank * DS;  // offset d of my T row 0
+                for (int rc2 = 0; rc2 < p.nrc2; ++rc2) {
+                    const int rbase = rc2 * R2 * TM2 + tm2 * TM2;
+                    const float *Arow[TM2];
 #pragma unroll
-                            for (int i = 0; i < TM2; ++i)
+                    for (int i = 0; i < TM2; ++i) Arow[i] = Tb + (size_t)min(rbase + i, 2 * DS - 1) * LDT;
+                    for (int nc2 = 0; nc2 < p.nnc2; ++nc2) {
+                        float aE[TM2][TN2], aO[TM2][TN2];
 #pragma unroll
-                                for (int j = 0; j < TN2; ++j) acc[i][j] = 0.f;
-                            constexpr int NKT = W / BK;
-                            const float *Bsrc = p.AxT + nc;
-                            const bool active = tm2 < TPM2;
-                            const float *Arow[TM2];
+                        for (int i = 0; i < TM2; ++i)
 #pragma unroll
-                            for (int i = 0; i < TM2; ++i) Arow[i] = Tb + (size_t)min(rc + tm2 * TM2 + i, MS - 1) * LDT;
-                            if (tid == 0)
-                                for (int t = 0; t < NSTG - 1 && t < NKT; ++t) stage_issue(t % NSTG, Bsrc, t, p.Np2, NCH2);
-                            for (int kt = 0; kt < NKT; ++kt) {
-                                const int slot = kt % NSTG;
-                                if (tid == 0 && kt + NSTG - 1 < NKT)
-                                    stage_issue((kt + NSTG - 1) % NSTG, Bsrc, kt + NSTG - 1, p.Np2, NCH2);
-                                bar_wait(slot);
-                                if (active) {
-                                    const float *Bt = stg + (size_t)slot * p.stg_floats + tn2 * TN2;
+                            for (int j = 0; j < TN2; ++j) aE[i][j] = 0.f, aO[i][j] = 0.f;
+                        constexpr int KT2 = W / (4 * G2);
+                        for (int kt = 0; kt < KT2; ++kt) {
+                            const float *Bt = ring_acquire();
 #pragma unroll
-                                    for (int k4 = 0; k4 < BK / 4; ++k4) {
-                                        float4 a4[TM2];
+                            for (int gi = 0; gi < G2 / KS2; ++gi) {
+                                const int g = gi * KS2 + ks2;
+                                const int k0 = (kt * G2 + g) * 4;
+                                const float *grp = Bt + g * GF2 + tn2 * 4;
+                                float4 a4[TM2];
 #pragma unroll
-                                        for (int i = 0; i < TM2; ++i)
-                                            a4[i] = *reinterpret_cast<const float4 *>(Arow[i] + kt * BK + k4 * 4);
+                                for (int i = 0; i < TM2; ++i) a4[i] = *reinterpret_cast<const float4 *>(Arow[i] + k0);
+                                float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                                if constexpr (C::X2 == 1) x4 = *reinterpret_cast<const float4 *>(grp + 16 * Cn2);
 #pragma unroll
-                                        for (int kk = 0; kk < 4; ++kk) {
-                                            float b[TN2];
-                                            load_vec<TN2>(b, Bt + (k4 * 4 + kk) * NCH2);
+                                for (int kk = 0; kk < 4; ++kk) {
+                                    const float4 b4 = *reinterpret_cast<const float4 *>(grp + kk * Cn2 * 4);
+                                    float b[TN2];
+                                    b[0] = b4.x, b[1] = b4.y, b[2] = b4.z, b[3] = b4.w;
+                                    if constexpr (C::X2 == 1) b[4] = kk == 0 ? x4.x : kk == 1 ? x4.y : kk == 2 ? x4.z : x4.w;
 #pragma unroll
-                                            for (int i = 0; i < TM2; ++i) {
-                                                const float av = kk == 0 ? a4[i].x : kk == 1 ? a4[i].y : kk == 2 ? a4[i].z : a4[i].w;
+                                    for (int i = 0; i < TM2; ++i) {
+                                        const float av = kk == 0 ? a4[i].x : kk == 1 ? a4[i].y : kk == 2 ? a4[i].z : a4[i].w;
 #pragma unroll
-                                                for (int j = 0; j < TN2; ++j) acc[i][j] = fmaf(av, b[j], acc[i][j]);
-                                            }
+                                        for (int j = 0; j < TN2; ++j) {
+                                            if ((kk & 1) == 0) aE[i][j] = fmaf(av, b[j], aE[i][j]);
+                                            else aO[i][j] = fmaf(av, b[j], aO[i][j]);
                                         }
                                     }
                                 }
-                                __syncthreads();
                             }
-                            if (active) {
+                            ring_release();
+                        }
+                        if constexpr (KS2 > 1) {  // sum the k-slices into slice 0
+                            const int t2 = tm2 * Cn2 + tn2;
+                            if (ks2 > 0) {
+                                float *r = red + (size_t)(ks2 - 1) * (2 * TM2 * TN2) * (R2 * Cn2) + t2;
 #pragma unroll
-                                for (int i = 0; i < TM2; ++i) {
-                                    const int r = rc + tm2 * TM2 + i;
-                                    const int m = mrow0 + r;
+                                for (int i = 0; i < TM2; ++i)
 #pragma unroll
                                     for (int j = 0; j < TN2; ++j) {
-                                        const int n = nc + tn2 * TN2 + j;
-                                        if (r < nrows && n < M && better(acc[i][j], m * M + n, sub.v, sub.i))
-                                            sub.v = acc[i][j], sub.i = m * M + n;
+                                        r[(size_t)(2 * (i * TN2 + j)) * (R2 * Cn2)] = aE[i][j];
+                                        r[(size_t)(2 * (i * TN2 + j) + 1) * (R2 * Cn2)] = aO[i][j];
+                                    }
+                            }
+                            __syncthreads();
+                            if (ks2 == 0) {
+                                for (int s2 = 0; s2 < KS2 - 1; ++s2) {
+                                    const float *r = red + (size_t)s2 * (2 * TM2 * TN2) * (R2 * Cn2) + t2;
+#pragma unroll
+                                    for (int i = 0; i < TM2; ++i)
+#pragma unroll
+                                        for (int j = 0; j < TN2; ++j) {
+                                            aE[i][j] += r[(size_t)(2 * (i * TN2 + j)) * (R2 * Cn2)];
+                                            aO[i][j] += r[(size_t)(2 * (i * TN2 + j) + 1) * (R2 * Cn2)];
+                                        }
+                                }
+                            }
+                            __syncthreads();
+                        }
+                        if (ks2 == 0) {
+                            const int ebase = nc2 * C::NCOL2;
+                            float ny[TN2];
+                            int ee[TN2];
+#pragma unroll
+                            for (int j = 0; j < TN2; ++j) {
+                                ee[j] = ebase + (j < 4 ? tn2 * 4 + j : 4 * Cn2 + tn2);
+                                ny[j] = __ldg(&p.nyqc[ee[j]]);
+                            }
+#pragma unroll
+                            for (int i = 0; i < TM2; ++i) {
+                                const int r = rbase + i;
+                                const bool lower = r >= DS;          // row holds T(c-d)
+                                const int d = d0 + (lower ? r - DS : r);
+                                const int m = lower ? cM - d : cM + d;
+                                const bool rok = r < 2 * DS && d < nd && m >= 0 && m < M && !(lower && d == 0);
+                                const float tny = Arow[i][1];         // Nyquist column of this T row
+#pragma unroll
+                                for (int j = 0; j < TN2; ++j) {
+                                    const int e = ee[j];
+                                    const float E = fmaf(tny, ny[j], aE[i][j]), O = aO[i][j];
+                                    if (rok && e < nd) {
+                                        const float cp = E - O, cm = E + O;
+                                        const int np = cM + e, nm = cM - e;
+                                        if (np < M && better(cp, m * M + np, sub.v, sub.i)) sub.v = cp, sub.i = m * M + np;
+                                        if (e > 0 && better(cm, m * M + nm, sub.v, sub.i)) sub.v = cm, sub.i = m * M + nm;
                                     }
                                 }
                             }
@@ -826,7 +975,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                 }
                 stamp(5, f);
-                if (mb + MSB < M) csync();  // T is overwritten by the next super-block
+                if (sb + 1 < p.nsb) csync();  // T is overwritten by the next super-block
             }
         }
         int ms, ns;
@@ -857,10 +1006,21 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             double2 *R64 = part + 3 * NSL * NC;                                // [3][NC]
             double *terms = reinterpret_cast<double *>(R64 + 3 * NC);          // [9][NC]
             for (int iter = 0; iter < 8; ++iter) {
-                for (int e = tid; e < 3 * H; e += NT) {
-                    const int a = e / H, j = e % H;
+                // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
+                // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j')
+                for (int e = tid; e < 3 * (H / 2 + 1); e += NT) {
+                    const int a = e / (H / 2 + 1), j = e % (H / 2 + 1);
                     const int mm = ms - 1 + a;
-                    dtab[e] = (mm >= 0 && mm < M) ? dirichlet64((long long)(mm - cM) - (long long)j * u, u, H) : 0.0;
+                    const bool ok = mm >= 0 && mm < M;
+                    const long long tnum = (long long)(mm - cM);
+                    if (j == 0 || j == H / 2) {
+                        dtab[a * H + j] = ok ? dirichlet64(tnum - (long long)j * u, u, H) : 0.0;
+                    } else {
+                        double we = 0.0, wo = 0.0;
+                        if (ok) dirichlet_pair64(tnum, j, u, H, &we, &wo);
+                        dtab[a * H + j] = we;
+                        dtab[a * H + H - j] = wo;
+                    }
                 }
                 __syncthreads();
                 for (int e = tid; e < NSL * NC; e += NT) {
@@ -977,8 +1137,9 @@ struct Launcher {
         CcVariant v{};
         v.H = C::H, v.W = C::W, v.CS = C::CS, v.NT = C::NT, v.dtype = sizeof(typename C::PIX) == 1 ? 0 : 1;
         v.TM1 = C::TM1, v.TN1 = C::TN1, v.TM2 = C::TM2, v.TN2 = C::TN2;
+        v.R1 = C::R1, v.Cn1 = C::Cn1, v.R2 = C::R2, v.Cn2 = C::Cn2, v.KS2 = C::KS2, v.BK1 = C::BK1, v.G2 = C::G2;
         v.s_global = C::SG ? 1 : 0;
-        v.BK = BK, v.NSTG = NSTG;
+        v.NSTG = NSTG;
         v.fixed_smem = &fixed_smem;
         v.raw_scratch_bytes = &raw_scratch_bytes;
         v.prepare = &prepare;
