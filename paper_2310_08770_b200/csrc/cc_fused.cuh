@@ -391,14 +391,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     const uint32_t my_frames = p.batch > cid ? (uint32_t)((p.batch - cid + ncl - 1) / ncl) : 0u;
     const uint32_t total_tiles = my_frames * (uint32_t)p.ntiles_frame;
     uint32_t g_cons = 0, g_load = 0, s_idx = 0;
+    uint32_t next_ti = (tid == 0 && total_tiles > 0) ? __ldg(&p.sched[0]) : 0u;  // schedule entry of the next tile, fetched one tile ahead
     auto ring_produce = [&]() {  // thread 0 only
         const uint32_t slot = g_load % NSTG;
         mbar_wait(&bempty[slot], ((g_load / NSTG) & 1u) ^ 1u);
-        const uint32_t ti = __ldg(&p.sched[s_idx]);
+        const uint32_t ti = next_ti;
         mbar_expect_tx(&bfull[slot], (uint32_t)C::TILEF * 4u);
         bulk_g2s(stg + (size_t)slot * C::TILEF, p.blob + (size_t)ti * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[slot]);
         ++g_load;
         if (++s_idx == (uint32_t)p.ntiles_frame) s_idx = 0;
+        next_ti = __ldg(&p.sched[s_idx]);  // latency overlaps the tile's compute
     };
     auto ring_acquire = [&]() -> const float * {
         if (tid == 0 && g_load < total_tiles) ring_produce();
