@@ -129,6 +129,21 @@ cc_status cc_track_profile(const cc_plan *plan, const void *frames, int batch,
 cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
                         float *dx, float *dy, float *peak);
 
+/*
+ * cc_track_latency_probe -- measurement aid for the real-time (batch-1)
+ * mode of the paper (one displacement per camera frame):
+ * n sequential calls of cc_track(batch = 1) on consecutive frames, each
+ * followed by cudaStreamSynchronize, with the host monotonic clock read
+ * around every call + synchronise pair.
+ *   frames   DEVICE pointer, n frames (as for cc_track)
+ *   dx,dy    DEVICE pointers, n float32 each (call i writes element i)
+ *   peak     DEVICE pointer, n float32, or NULL
+ *   lat_us   HOST pointer, receives n latencies in microseconds
+ * Synchronises the stream.
+ */
+cc_status cc_track_latency_probe(const cc_plan *plan, const void *frames, int n,
+                                 float *dx, float *dy, float *peak, double *lat_us, void *stream);
+
 /* Frees every device/host allocation of the plan.  NULL is a no-op. */
 cc_status cc_plan_destroy(cc_plan *plan);
 

@@ -20,7 +20,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_fp32_peak_probe", "cc_status_string", "cc_last_error"]
+           "cc_plan_info", "cc_fp32_peak_probe", "cc_track_latency_probe", "cc_status_string", "cc_last_error"]
 
 
 class CcError(RuntimeError):
@@ -59,6 +59,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_track_profile.restype = ci
         lib.cc_track_host.argtypes = [vp, vp, ci, vp, vp, vp]
         lib.cc_track_host.restype = ci
+        lib.cc_track_latency_probe.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp]
+        lib.cc_track_latency_probe.restype = ci
         lib.cc_plan_destroy.argtypes = [vp]
         lib.cc_plan_destroy.restype = ci
         lib.cc_plan_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
@@ -170,6 +172,23 @@ class Plan:
         _check(load_library().cc_track_profile(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(),
                                                pk.data_ptr(), cyc.data_ptr(), torch.cuda.current_stream(dev).cuda_stream))
         return dx, dy, pk, cyc
+
+    def latency_probe(self, frames_dev, n: int | None = None):
+        """cc_track_latency_probe: n sequential batch-1 calls timed by the library's native loop.
+        Returns (dx, dy, peak) device tensors and a numpy array of per-call latencies in microseconds."""
+        torch = _torch()
+        fb = self.H * self.W * self.np_dtype.itemsize
+        if n is None:
+            n = frames_dev.numel() * frames_dev.element_size() // fb
+        dev = frames_dev.device
+        dx = torch.empty(n, dtype=torch.float32, device=dev)
+        dy = torch.empty(n, dtype=torch.float32, device=dev)
+        pk = torch.empty(n, dtype=torch.float32, device=dev)
+        lat = np.empty(n, np.float64)
+        _check(load_library().cc_track_latency_probe(self._h, frames_dev.data_ptr(), n, dx.data_ptr(), dy.data_ptr(),
+                                                     pk.data_ptr(), lat.ctypes.data_as(ctypes.c_void_p),
+                                                     torch.cuda.current_stream(dev).cuda_stream))
+        return dx, dy, pk, lat
 
     def track_host(self, frames_np, dx=None, dy=None, peak=None):
         """cc_track_host: host numpy frames in, host numpy results out (H2D/D2H inside)."""

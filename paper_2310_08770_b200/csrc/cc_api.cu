@@ -6,6 +6,8 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
+#include <time.h>
 
 #include <algorithm>
 #include <complex>
@@ -69,6 +71,8 @@ struct cc_plan {
     float2 *tw = nullptr, *Gt = nullptr;
     uint16_t *row_slot = nullptr, *col_partner = nullptr;
     float4 *ab = nullptr;
+    double2 *tw64 = nullptr, *Xpol = nullptr;  // fp64 tables of the argmax polish steps
+    double *Dpol = nullptr, *nyq64 = nullptr;
     size_t table_bytes = 0;
     VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
     bool has_lat = false;
@@ -179,6 +183,37 @@ static double dirichlet_host(long long tnum, int u, int H)
     return s1 * cos(x) / ((double)H * sin(x));
 }
 
+// ---- long-double versions for the fp64 polish tables
+static const long double PI_L = 3.14159265358979323846264338327950288L;
+static long double sinpi_frac_l(long long num, long long den)  // sin(pi num / den), phase reduced exactly
+{
+    long long r = num % (2 * den);
+    if (r < 0) r += 2 * den;
+    if (r == 0 || r == den) return 0.0L;
+    return sinl(PI_L * (long double)r / (long double)den);
+}
+static long double dirichlet_l(long long tnum, int u, int H)
+{
+    const long long den = (long long)u * H;
+    const long long r = ((tnum % den) + den) % den;
+    if (r == 0) return 1.0L;
+    const long double s1 = sinpi_frac_l(tnum, u);
+    const long double x = PI_L * (long double)r / (long double)den;  // in (0, pi)
+    return s1 * cosl(x) / ((long double)H * sinl(x));
+}
+// Even / odd parts of the Dirichlet weight about row offset j (0 < j < H/2), t = tnum / u, |t| < 1:
+//   we = (D_H(t-j) + D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2x) / (2 H sin(x-y) sin(x+y)),
+//   wo = (D_H(t-j) - D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2y) / (2 H sin(x-y) sin(x+y)),   x = pi t / H, y = pi j / H
+static void dirichlet_pair_l(long long tnum, int j, int u, int H, double *we, double *wo)
+{
+    const long long den = (long long)u * H;
+    const long double s = sinpi_frac_l(tnum, u);
+    const long double sa = sinpi_frac_l(tnum - (long long)j * u, den), sb = sinpi_frac_l(tnum + (long long)j * u, den);
+    const long double pref = ((j & 1) ? -s : s) / (2.0L * (long double)H * sa * sb);
+    *we = (double)(pref * sinpi_frac_l(2 * tnum, den));
+    *wo = (double)(pref * sinpi_frac_l(2LL * j, H));
+}
+
 // operand tiles of one variant: stage-1 even/odd Dirichlet tiles, stage-2 cos/sin tiles, the tile schedule
 static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *acc)
 {
@@ -279,6 +314,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     if (!plan) return CC_OK;
     cudaFree(plan->tw), cudaFree(plan->Gt), cudaFree(plan->row_slot), cudaFree(plan->col_partner);
     cudaFree(plan->ab);
+    cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
     for (VarPlan *vp : {&plan->thr, &plan->lat}) cudaFree(vp->Sg), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
@@ -306,6 +342,7 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
     pl->M = (3 * upsample + 1) / 2;  // ceil(1.5 u)
     pl->c = pl->M / 2;
     const int M = pl->M, c = pl->c, u = upsample;
+    (void)c;
 
     // ---- variants: smallest cluster = throughput variant, largest = small-batch (latency) variant
     {
@@ -323,6 +360,9 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
         std::sort(fits.begin(), fits.end(), [](const VarPlan &a, const VarPlan &b) { return a.v.CS < b.v.CS; });
         pl->thr = fits.front();
         if (fits.back().v.CS != fits.front().v.CS) pl->lat = fits.back(), pl->has_lat = true;
+        if (const char *ev = getenv("CC_LAT_CS")) {  // EXPERIMENT
+            for (auto &f : fits) if (f.v.CS == atoi(ev)) pl->lat = f, pl->has_lat = true;
+        }
     }
 
     // ---- reference image to the host
@@ -381,7 +421,32 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
     if (e == cudaSuccess) e = upload(&pl->col_partner, col_partner, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->Gt, Gt, &pl->table_bytes);
     if (e == cudaSuccess) e = upload(&pl->ab, ab, &pl->table_bytes);
+    // ---- fp64 tables of the polish steps (R9): every phase from an exactly reduced integer numerator
+    {
+        std::vector<double2> tw64(W);
+        for (int j = 0; j < W; ++j) tw64[j] = make_double2((double)cosl(2.0L * PI_L * j / W), (double)sinl(2.0L * PI_L * j / W));
+        if (e == cudaSuccess) e = upload(&pl->tw64, tw64, &pl->table_bytes);
+    }
     if (u > 1) {
+        std::vector<double> Dpol((size_t)M * H), nyq64(M);
+        std::vector<double2> Xpol((size_t)M * Wh);
+        const long long denx = (long long)u * W;
+        for (int m = 0; m < M; ++m) {
+            const long long tnum = m - c;  // t = tnum / u, |t| < 1
+            double *row = Dpol.data() + (size_t)m * H;
+            row[0] = (double)dirichlet_l(tnum, u, H);
+            row[H / 2] = (double)dirichlet_l(tnum - (long long)(H / 2) * u, u, H);
+            for (int j = 1; j < H / 2; ++j) dirichlet_pair_l(tnum, j, u, H, &row[j], &row[H - j]);
+            nyq64[m] = (double)cosl(PI_L * (long double)(((tnum % (2LL * u)) + 2LL * u) % (2LL * u)) / (long double)u);
+            for (int q = 0; q < Wh; ++q) {
+                const long long num = (((long long)q * tnum) % denx + denx) % denx;
+                const long double th = 2.0L * PI_L * (long double)num / (long double)denx;
+                Xpol[(size_t)m * Wh + q] = make_double2((double)cosl(th), (double)sinl(th));
+            }
+        }
+        if (e == cudaSuccess) e = upload(&pl->Dpol, Dpol, &pl->table_bytes);
+        if (e == cudaSuccess) e = upload(&pl->Xpol, Xpol, &pl->table_bytes);
+        if (e == cudaSuccess) e = upload(&pl->nyq64, nyq64, &pl->table_bytes);
         if (e == cudaSuccess) e = build_tiles(pl->thr, H, W, u, M, &pl->table_bytes);
         if (e == cudaSuccess && pl->has_lat) e = build_tiles(pl->lat, H, W, u, M, &pl->table_bytes);
     }
@@ -416,6 +481,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
 {
     p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
     p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg;
+    p.tw64 = pl->tw64, p.Dpol = pl->Dpol, p.Xpol = pl->Xpol, p.nyq64 = pl->nyq64;
     p.u = pl->u, p.M = pl->M, p.c = pl->c, p.nd = pl->c + 1;
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
@@ -504,6 +570,29 @@ extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
     }
     CK(cudaStreamSynchronize(plan->hs[0]));
     CK(cudaStreamSynchronize(plan->hs[1]));
+    return CC_OK;
+}
+
+extern "C" cc_status cc_track_latency_probe(const cc_plan *plan, const void *frames, int n, float *dx, float *dy,
+                                            float *peak, double *lat_us, void *stream)
+{
+    if (!plan || n < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_latency_probe: bad plan or n");
+    if (n == 0) return CC_OK;
+    if (!frames || !dx || !dy || !lat_us) return fail(CC_ERR_INVALID_ARG, "cc_track_latency_probe: null pointer");
+    const size_t fbytes = (size_t)plan->H * plan->W * (plan->dtype == CC_U8 ? 1 : 2);
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaStreamSynchronize(st));
+    for (int i = 0; i < n; ++i) {
+        struct timespec t0, t1;
+        clock_gettime(CLOCK_MONOTONIC, &t0);
+        cc_status s = cc_track(plan, (const unsigned char *)frames + (size_t)i * fbytes, 1, dx + i, dy + i,
+                               peak ? peak + i : nullptr, stream);
+        if (s != CC_OK) return s;
+        cudaError_t e = cudaStreamSynchronize(st);
+        clock_gettime(CLOCK_MONOTONIC, &t1);
+        if (e != cudaSuccess) return fail_cuda(e, "cudaStreamSynchronize");
+        lat_us[i] = (double)(t1.tv_sec - t0.tv_sec) * 1e6 + (double)(t1.tv_nsec - t0.tv_nsec) * 1e-3;
+    }
     return CC_OK;
 }
 

@@ -70,6 +70,12 @@ struct CcParams {
     const uint32_t *sched;        // [ntiles_frame] blob tile index of the i-th tile a frame consumes
     const float *nyqc;            // [ne_pad] cos(pi e / u): Nyquist-column weight of stage 2
     float2 *Sg;                   // global spectrum scratch (variants with S in L2), else null
+    // fp64 tables of the two argmax polish steps (exactly reduced integer phase numerators, built at plan time)
+    const double2 *tw64;          // [W] (cos, sin)(2 pi j / W)
+    const double *Dpol;           // [M][H] Dirichlet weights of grid row m for the physical rows (y0+j) mod H of the
+                                  //        sum/difference layout: j = 0, H/2: D_H(t-j); 0 < j < H/2: even part; H-j: odd part
+    const double2 *Xpol;          // [M][W/2] (cos, sin)(2 pi q (n - c) / (u W))
+    const double *nyq64;          // [M] cos(pi (n - c) / u)
 
     int u, M, c;        // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
     int nd;             // c + 1: number of |offsets| d (and e) evaluated per axis

@@ -233,42 +233,6 @@ __device__ __forceinline__ void load_vec(float (&d)[n], const float *s)
     }
 }
 
-// fp64 periodic-sinc (Dirichlet) interpolation weight of the even-length DFT
-// with the Nyquist bin split half/half:  D_H(t) = sin(pi t) cot(pi t / H) / H,
-// t = tnum / u.
-__device__ __forceinline__ double dirichlet64(long long tnum, int u, int Hn)
-{
-    const long long den = (long long)u * Hn;
-    long long r = tnum % den;
-    if (r < 0) r += den;
-    if (r == 0) return 1.0;
-    long long r2 = tnum % (2LL * u);
-    if (r2 < 0) r2 += 2LL * u;
-    const double s1 = sinpi((double)r2 / (double)u);
-    const double x = (double)r / (double)den;  // in (0, 1)
-    return s1 * cospi(x) / ((double)Hn * sinpi(x));
-}
-
-// Even / odd parts of the Dirichlet weight about row offset j (0 < j < H/2), t = tnum / u, |t| < 1:
-//   we = (D_H(t-j) + D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2x) / (2 H sin(x-y) sin(x+y)),
-//   wo = (D_H(t-j) - D_H(t+j)) / 2 = (-1)^j sin(pi t) sin(2y) / (2 H sin(x-y) sin(x+y)),
-// x = pi t / H, y = pi j / H; every sine gets an exactly reduced integer phase numerator.
-__device__ __forceinline__ double sinpi_frac(long long num, long long den)  // sin(pi num / den)
-{
-    long long r = num % (2 * den);
-    if (r < 0) r += 2 * den;
-    return sinpi((double)r / (double)den);
-}
-__device__ __forceinline__ void dirichlet_pair64(long long tnum, int j, int u, int Hn, double *we, double *wo)
-{
-    const long long den = (long long)u * Hn;
-    const double s = sinpi_frac(tnum, u);
-    const double sa = sinpi_frac(tnum - (long long)j * u, den), sb = sinpi_frac(tnum + (long long)j * u, den);
-    const double pref = ((j & 1) ? -s : s) / (2.0 * (double)Hn * sa * sb);
-    *we = pref * sinpi_frac(2 * tnum, den);
-    *wo = pref * sinpi_frac(2LL * j, Hn);
-}
-
 // ------------------------------------------------------------------ the kernel
 template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
           int R2_, int KS2_>
@@ -458,30 +422,23 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         ph ^= 1u << b;
     };
 
-    // 3x3 evaluation in fp64 of  sum_q w_q Re( R[a][q] * exp(2 pi i q xnum[b] / den) )  over this
-    // CTA's columns, summed over the cluster in rank order.  R64[a][ql] (double2) in shared memory;
-    // packed column (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b] = cos(pi * x_b).
-    // Scratch `terms` = double[9][NC].  Result: out[a*3+b] valid in all threads of all CTAs.
-    auto xeval9 = [&](const double2 *R64, const long long *xnum, long long den, const double *nyq_c, double *terms,
-                      double *out) {
+    // 3x3 evaluation in fp64 of  sum_q w_q Re( R[a][q] * (cs + i sn)(b, q) )  over this CTA's columns,
+    // summed over the cluster in rank order.  R64[a][ql] (double2) in shared memory; the packed column
+    // (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b].  phase(b, q) -> (cos, sin) of the column phase,
+    // from the plan's fp64 tables.  Scratch `terms` = double[9][NC].  Result: out[a*3+b] valid in all
+    // threads of all CTAs.
+    auto xeval9 = [&](const double2 *R64, auto phase, const double *nyq_c, double *terms, double *out) {
         for (int e = tid; e < 3 * NC; e += NT) {
             const int b = e / NC, ql = e % NC;
             const int q = rank * NC + ql;
-            double cs, sn, w;
-            if (q == 0) {
-                cs = 1.0, sn = 0.0, w = 1.0;
-            } else {
-                long long num = ((long long)q * xnum[b]) % den;
-                if (num < 0) num += den;
-                sincospi(2.0 * (double)num / (double)den, &sn, &cs);
-                w = 2.0;
-            }
+            double2 cs = make_double2(1.0, 0.0);
+            if (q != 0) cs = phase(b, q);
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const double2 r = R64[a * NC + ql];
                 double t;
                 if (q == 0) t = r.x + r.y * nyq_c[b];
-                else t = w * (r.x * cs - r.y * sn);
+                else t = 2.0 * (r.x * cs.x - r.y * cs.y);
                 terms[(a * 3 + b) * NC + ql] = t;
             }
         }
@@ -712,16 +669,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 const float2 v = Sl[(size_t)((y0 - 1 + a) & (H - 1)) * NC + ql];
                 R64[e] = make_double2((double)v.x, (double)v.y);
             }
-            long long xnum[3];
             double nyq[3], c9[9];
 #pragma unroll
-            for (int b = 0; b < 3; ++b) {
-                const int xx = (x0 - 1 + b) & (W - 1);
-                xnum[b] = xx;
-                nyq[b] = (xx & 1) ? -1.0 : 1.0;
-            }
+            for (int b = 0; b < 3; ++b) nyq[b] = ((x0 - 1 + b) & 1) ? -1.0 : 1.0;
             __syncthreads();
-            xeval9(R64, xnum, (long long)W, nyq, terms, c9);
+            xeval9(R64, [&](int b, int q) { return __ldg(&p.tw64[(q * ((x0 - 1 + b) & (W - 1))) & (W - 1)]); }, nyq, terms, c9);
             double bv = -INFINITY;
             int bi = 0x7fffffff;
 #pragma unroll
@@ -1009,20 +961,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             double *terms = reinterpret_cast<double *>(R64 + 3 * NC);          // [9][NC]
             for (int iter = 0; iter < 8; ++iter) {
                 // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
-                // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j')
-                for (int e = tid; e < 3 * (H / 2 + 1); e += NT) {
-                    const int a = e / (H / 2 + 1), j = e % (H / 2 + 1);
+                // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j'):
+                // rows ms-1..ms+1 of the plan's fp64 table Dpol[M][H] (zero weights outside the grid)
+                for (int e = tid; e < 3 * H; e += NT) {
+                    const int a = e / H, j = e % H;
                     const int mm = ms - 1 + a;
-                    const bool ok = mm >= 0 && mm < M;
-                    const long long tnum = (long long)(mm - cM);
-                    if (j == 0 || j == H / 2) {
-                        dtab[a * H + j] = ok ? dirichlet64(tnum - (long long)j * u, u, H) : 0.0;
-                    } else {
-                        double we = 0.0, wo = 0.0;
-                        if (ok) dirichlet_pair64(tnum, j, u, H, &we, &wo);
-                        dtab[a * H + j] = we;
-                        dtab[a * H + H - j] = wo;
-                    }
+                    dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
                 }
                 __syncthreads();
                 for (int e = tid; e < NSL * NC; e += NT) {
@@ -1050,18 +994,24 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                     R64[e] = s;
                 }
-                long long xnum[3];
                 double nyq[3], c9[9];
+                const double sgx = (x0 & 1) ? -1.0 : 1.0;
 #pragma unroll
                 for (int b = 0; b < 3; ++b) {
-                    const long long xn = (long long)x0 * u + (ns - 1 + b - cM);
-                    xnum[b] = xn;
-                    long long r2 = xn % (2LL * u);
-                    if (r2 < 0) r2 += 2LL * u;
-                    nyq[b] = cospi((double)r2 / (double)u);
+                    const int nn = min(max(ns - 1 + b, 0), M - 1);  // out-of-grid neighbours are skipped below
+                    nyq[b] = sgx * __ldg(&p.nyq64[nn]);
                 }
                 __syncthreads();
-                xeval9(R64, xnum, (long long)u * W, nyq, terms, c9);
+                xeval9(
+                    R64,
+                    [&](int b, int q) {
+                        // exp(2 pi i q (x0 u + n - c) / (u W)) = exp(2 pi i q x0 / W) * exp(2 pi i q (n - c) / (u W))
+                        const int nn = min(max(ns - 1 + b, 0), M - 1);
+                        const double2 w0 = __ldg(&p.tw64[(q * x0) & (W - 1)]);
+                        const double2 w1 = __ldg(&p.Xpol[(size_t)nn * (W / 2) + q]);
+                        return make_double2(w0.x * w1.x - w0.y * w1.y, w0.x * w1.y + w0.y * w1.x);
+                    },
+                    nyq, terms, c9);
                 double bv = -INFINITY;
                 int ba = 1, bb = 1, bi = 0x7fffffff;
 #pragma unroll

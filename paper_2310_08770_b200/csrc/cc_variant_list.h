@@ -12,6 +12,8 @@ CCV(f64_u8,        64,   64, 1, uint8_t,  256,  5, 8, 10, 5, false,  4,  2, 16, 
 CCV(f128_u8,      128,  128, 1, uint8_t,  256,  2, 8,  4, 4, false, 16,  8,  8,  8)
 CCV(f128_u16,     128,  128, 1, uint16_t, 256,  2, 8,  4, 4, false, 16,  8,  8,  8)
 CCV(f128_u8_c8,   128,  128, 8, uint8_t,  256,  1, 4,  1, 4, false,  8,  8,  8,  8)
+CCV(f128_u8_c4,   128,  128, 4, uint8_t,  256,  1, 8,  1, 4, false,  8,  8,  8,  8)
+CCV(f128_u8_c2,   128,  128, 2, uint8_t,  256,  2, 8,  2, 4, false,  8,  8,  8,  8)
 CCV(f128_u16_c8,  128,  128, 8, uint16_t, 256,  1, 4,  1, 4, false,  8,  8,  8,  8)
 CCV(f256_u16,     256,  256, 2, uint16_t, 256, 10, 8,  5, 5, false,  4,  2, 16,  1)
 CCV(f256_u8,      256,  256, 2, uint8_t,  256, 10, 8,  5, 5, false,  4,  2, 16,  1)
