@@ -331,7 +331,7 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
     if (!out || !reference || H <= 0 || W <= 0 || upsample < 1 || (dtype != CC_U8 && dtype != CC_U16))
         return fail(CC_ERR_INVALID_ARG, "cc_plan_create: bad argument");
     if (upsample > 4096) return fail(CC_ERR_UNSUPPORTED, "upsample factor above 4096");
-    if (!is_pow2(H) || !is_pow2(W) || cc_radix(H, 0) == 0 || cc_radix(W, 0) == 0)
+    if (!is_pow2(H) || !is_pow2(W) || cc_radix_col(H, 0) == 0 || cc_radix_row(W, 0) == 0)
         return fail(CC_ERR_UNSUPPORTED, "frame sides must be powers of two in 64..1024");
     cc_status st = check_device();
     if (st != CC_OK) return st;
@@ -395,15 +395,15 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
         tw[j] = make_float2((float)cos(a), (float)(-sin(a)));
     }
     std::vector<uint16_t> row_slot(W), col_slot(H), col_partner(H);
-    for (int p = 0; p < W; ++p) row_slot[cc_freq_of_slot(W, p)] = (uint16_t)p;
-    for (int p = 0; p < H; ++p) col_slot[cc_freq_of_slot(H, p)] = (uint16_t)p;
-    for (int p = 0; p < H; ++p) col_partner[p] = col_slot[(H - cc_freq_of_slot(H, p)) % H];
+    for (int p = 0; p < W; ++p) row_slot[cc_freq_of_slot(W, p, true)] = (uint16_t)p;
+    for (int p = 0; p < H; ++p) col_slot[cc_freq_of_slot(H, p, false)] = (uint16_t)p;
+    for (int p = 0; p < H; ++p) col_partner[p] = col_slot[(H - cc_freq_of_slot(H, p, false)) % H];
 
     const int Wh = W / 2;
     std::vector<float2> Gt((size_t)H * Wh);
     std::vector<float4> ab(H);
     for (int p = 0; p < H; ++p) {
-        const int ky = cc_freq_of_slot(H, p);
+        const int ky = cc_freq_of_slot(H, p, false);
         for (int q = 1; q < Wh; ++q) {
             const std::complex<double> g = std::conj(G[(size_t)ky * W + q]) / HW;
             Gt[(size_t)p * Wh + q] = make_float2((float)g.real(), (float)g.imag());

@@ -7,7 +7,8 @@
 // Mixed-radix decomposition of the in-place FFTs (forward = decimation in
 // frequency, natural order in -> "slot" order out; inverse = the transpose,
 // slot order in -> natural order out).  N = r[0]*r[1]*r[2].
-__host__ __device__ constexpr int cc_radix(int N, int p)
+// Column FFTs (one thread per butterfly, NC columns in parallel) use large radices: fewer sweeps of S.
+__host__ __device__ constexpr int cc_radix_col(int N, int p)
 {
     return N == 64   ? (p == 0 ? 8 : p == 1 ? 8 : 1)
          : N == 128  ? (p == 0 ? 16 : p == 1 ? 8 : 1)
@@ -16,14 +17,26 @@ __host__ __device__ constexpr int cc_radix(int N, int p)
          : N == 1024 ? (p == 0 ? 16 : p == 1 ? 8 : 8)
                      : 0;
 }
+// Row FFTs (one warp per FFT) use radices small enough that a pass has >= 32 butterflies where possible:
+// all lanes busy instead of N/16 of them.
+__host__ __device__ constexpr int cc_radix_row(int N, int p)
+{
+    return N == 64   ? (p == 0 ? 4 : p == 1 ? 4 : 4)
+         : N == 128  ? (p == 0 ? 4 : p == 1 ? 4 : 8)
+         : N == 256  ? (p == 0 ? 4 : p == 1 ? 8 : 8)
+         : N == 512  ? (p == 0 ? 8 : p == 1 ? 8 : 8)
+         : N == 1024 ? (p == 0 ? 16 : p == 1 ? 8 : 8)
+                     : 0;
+}
+__host__ __device__ constexpr int cc_radix(int N, int p, bool row) { return row ? cc_radix_row(N, p) : cc_radix_col(N, p); }
 
 // Frequency held by slot p after the forward FFT of length N:
 // p = k1*(N/r0) + k2*(N/(r0 r1)) + k3  <->  k = k1 + r0*k2 + r0*r1*k3.
-static inline int cc_freq_of_slot(int N, int p)
+static inline int cc_freq_of_slot(int N, int p, bool row)
 {
     int k = 0, mult = 1, L = N, rem = p;
     for (int i = 0; i < 3; ++i) {
-        int r = cc_radix(N, i);
+        int r = cc_radix(N, i, row);
         if (r <= 1) break;
         L /= r;
         int d = rem / L;

@@ -180,7 +180,7 @@ __device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *tw, int 
 template <int N, bool INV, int NTW>
 __device__ __forceinline__ void warp_fft(float2 *sc, const float2 *tw, int lane)
 {
-    constexpr int R0 = cc_radix(N, 0), R1 = cc_radix(N, 1), R2 = cc_radix(N, 2);
+    constexpr int R0 = cc_radix_row(N, 0), R1 = cc_radix_row(N, 1), R2 = cc_radix_row(N, 2);
     if (!INV) {
         warp_fft_pass<N, N, R0, false, NTW>(sc, tw, lane);
         warp_fft_pass<N, N / R0, R1, false, NTW>(sc, tw, lane);
@@ -527,7 +527,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
         // =============================================================== a2/a3/a4: column FFT (x) Gc, column inverse
         {
-            constexpr int R0 = cc_radix(H, 0), R1 = cc_radix(H, 1), R2 = cc_radix(H, 2);
+            constexpr int R0 = cc_radix_col(H, 0), R1 = cc_radix_col(H, 1), R2 = cc_radix_col(H, 2);
             constexpr int RL = R2 > 1 ? R2 : R1;   // radix of the last forward pass (fused with the product)
             constexpr int NPASS = R2 > 1 ? 3 : 2;
             // forward pass 0
