@@ -19,13 +19,13 @@
 #include "cc_common.h"
 
 // ------------------------------------------------------------------ variants
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2) CcVariant cc_variant_##name();
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD) CcVariant cc_variant_##name();
 #include "cc_variant_list.h"
 #undef CCV
 
 typedef CcVariant (*cc_variant_fn)();
 static const cc_variant_fn g_variant_fns[] = {
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2) &cc_variant_##name,
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD) &cc_variant_##name,
 #include "cc_variant_list.h"
 #undef CCV
 };
@@ -360,9 +360,6 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
         std::sort(fits.begin(), fits.end(), [](const VarPlan &a, const VarPlan &b) { return a.v.CS < b.v.CS; });
         pl->thr = fits.front();
         if (fits.back().v.CS != fits.front().v.CS) pl->lat = fits.back(), pl->has_lat = true;
-        if (const char *ev = getenv("CC_LAT_CS")) {  // EXPERIMENT
-            for (auto &f : fits) if (f.v.CS == atoi(ev)) pl->lat = f, pl->has_lat = true;
-        }
     }
 
     // ---- reference image to the host

@@ -27,10 +27,7 @@
 namespace ccf {
 namespace cg = cooperative_groups;
 
-constexpr int NSTG = 6;   // staging ring depth
-constexpr int PFD = 4;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
 constexpr int XN = 10;    // doubles per cluster-exchange record
-constexpr int NBARS = 2 * NSTG + 2;  // full[NSTG], empty[NSTG], raw ring [2]
 
 // ------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -235,8 +232,12 @@ __device__ __forceinline__ void load_vec(float (&d)[n], const float *s)
 
 // ------------------------------------------------------------------ the kernel
 template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
-          int R2_, int KS2_>
+          int R2_, int KS2_, int NSTG_, int PFD_>
 struct Cfg {
+    static constexpr int NSTG = NSTG_;  // staging ring depth
+    static constexpr int PFD = PFD_;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
+    static constexpr int NBARS = 2 * NSTG + 2;  // full[NSTG], empty[NSTG], raw ring [2]
+    static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
     static constexpr int BK1 = BK1_, G2 = G2_, R2 = R2_, KS2 = KS2_;
@@ -277,7 +278,8 @@ struct Cfg {
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
     static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64;
-    static constexpr size_t FIXED_BYTES = S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES;
+    static constexpr size_t FIXED_BYTES =
+        S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
     static_assert(NR % RCH == 0 && RCH % 2 == 0, "bad raw chunking");
     static_assert((2 * NC) % TN1 == 0 && NT % Cn1 == 0 && TN1 % 4 == 0 && Cn1 % WC1 == 0 && 32 % WC1 == 0, "bad stage-1 tiling");
@@ -297,6 +299,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     constexpr int NWARP = C::NWARP, NTW = C::NTW, PADW = C::PADW;
     constexpr int LDT = C::LDT;
     constexpr bool SG = C::SG;
+    constexpr int NSTG = C::NSTG, PFD = C::PFD, NBARS = C::NBARS;
     using PIX = typename C::PIX;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -320,6 +323,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
+
+    const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
+    if constexpr (C::LAT) {
+        double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
+        for (int i = tid; i < W; i += NT) t64[i] = p.tw64[i];
+        tw64 = t64;
+    }
 
     PIX *const raw = reinterpret_cast<PIX *>(U);
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
@@ -355,7 +365,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     const uint32_t my_frames = p.batch > cid ? (uint32_t)((p.batch - cid + ncl - 1) / ncl) : 0u;
     const uint32_t total_tiles = my_frames * (uint32_t)p.ntiles_frame;
     uint32_t g_cons = 0, g_load = 0, s_idx = 0;
-    uint32_t next_ti = (tid == 0 && total_tiles > 0) ? __ldg(&p.sched[0]) : 0u;  // schedule entry of the next tile, fetched one tile ahead
+    uint32_t next_ti = 0u;  // schedule entry of the next tile, fetched one tile ahead (thread 0)
     auto ring_produce = [&]() {  // thread 0 only
         const uint32_t slot = g_load % NSTG;
         mbar_wait(&bempty[slot], ((g_load / NSTG) & 1u) ^ 1u);
@@ -377,8 +387,21 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if (lane == 0) mbar_arrive(&bempty[g_cons % NSTG]);
         ++g_cons;
     };
-    if (tid == 0)
-        for (int i = 0; i < PFD && g_load < total_tiles; ++i) ring_produce();
+    if (tid == 0 && total_tiles > 0) {
+        // initial burst: fetch the first PFD schedule entries with independent loads, then issue the copies
+        uint32_t first[PFD];
+#pragma unroll
+        for (int i = 0; i < PFD; ++i) first[i] = __ldg(&p.sched[i % p.ntiles_frame]);
+#pragma unroll
+        for (int i = 0; i < PFD; ++i)
+            if (g_load < total_tiles) {
+                mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
+                bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)first[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
+                ++g_load;
+            }
+        s_idx = g_load % (uint32_t)p.ntiles_frame;
+        next_ti = __ldg(&p.sched[s_idx]);
+    }
 
     const int u = p.u, M = p.M, cM = p.c;
 
@@ -423,37 +446,44 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     };
 
     // 3x3 evaluation in fp64 of  sum_q w_q Re( R[a][q] * (cs + i sn)(b, q) )  over this CTA's columns,
-    // summed over the cluster in rank order.  R64[a][ql] (double2) in shared memory; the packed column
-    // (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b].  phase(b, q) -> (cos, sin) of the column phase,
-    // from the plan's fp64 tables.  Scratch `terms` = double[9][NC].  Result: out[a*3+b] valid in all
-    // threads of all CTAs.
-    auto xeval9 = [&](const double2 *R64, auto phase, const double *nyq_c, double *terms, double *out) {
-        for (int e = tid; e < 3 * NC; e += NT) {
-            const int b = e / NC, ql = e % NC;
+    // summed over the cluster in rank order.  Eight lanes (sub = 0..7) serve each (a, ql): getR(a, ql, sub)
+    // returns R[a][ql] to all of them (it may shuffle inside the 8-lane group); lanes sub = b < 3 then form the
+    // term of column phase b.  The packed column (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b].
+    // phase(b, q) -> (cos, sin) of the column phase from the plan's fp64 tables.  Scratch `terms` =
+    // double[9][NC].  Result: out[a*3+b] valid in all threads of all CTAs.  Summation order is fixed.
+    auto xeval9 = [&](auto getR, auto phase, const double *nyq_c, double *terms, double *out) {
+        static_assert((24 * NC) % 32 == 0, "whole warps per (a, ql) group sweep");
+        for (int t = tid; t < 24 * NC; t += NT) {  // warp-uniform trip count
+            const int o = t >> 3, sub = t & 7;
+            const int a = o / NC, ql = o % NC;
             const int q = rank * NC + ql;
             double2 cs = make_double2(1.0, 0.0);
-            if (q != 0) cs = phase(b, q);
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const double2 r = R64[a * NC + ql];
-                double t;
-                if (q == 0) t = r.x + r.y * nyq_c[b];
-                else t = 2.0 * (r.x * cs.x - r.y * cs.y);
-                terms[(a * 3 + b) * NC + ql] = t;
+            if (sub < 3 && q != 0) cs = phase(sub, q);  // issued before the group sum: the latency overlaps
+            const double2 r = getR(a, ql, sub);
+            if (sub < 3) {
+                double v;
+                if (q == 0) v = r.x + r.y * nyq_c[sub];
+                else v = 2.0 * (r.x * cs.x - r.y * cs.y);
+                terms[(a * 3 + sub) * NC + ql] = v;
             }
         }
         __syncthreads();
-        if (tid < 9) {
-            double s = 0.0;
-            for (int ql = 0; ql < NC; ++ql) s += terms[tid * NC + ql];
-            xsrc[tid] = s;
+        if (tid < 96) {  // three whole warps: 8 lanes per output k = a*3+b (k >= 9: idle groups)
+            const int k = tid >> 3, sub = tid & 7;
+            double sum = 0.0;
+            if (k < 9)
+                for (int ql = sub; ql < NC; ql += 8) sum += terms[k * NC + ql];
+            sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+            sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+            sum += __shfl_xor_sync(0xffffffffu, sum, 4);
+            if (k < 9 && sub == 0) xsrc[k] = sum;
         }
         const double *res = exchange(9);
 #pragma unroll
         for (int k = 0; k < 9; ++k) {
-            double s = 0.0;
-            for (int r = 0; r < CS; ++r) s += res[r * XN + k];
-            out[k] = s;
+            double sum = 0.0;
+            for (int r = 0; r < CS; ++r) sum += res[r * XN + k];
+            out[k] = sum;
         }
     };
 
@@ -662,18 +692,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             stamp(2, f);
 
             // fp64 re-evaluation of the 3x3 neighbourhood of the fp32 winner
-            double2 *R64 = reinterpret_cast<double2 *>(U);
-            double *terms = reinterpret_cast<double *>(R64 + 3 * NC);
-            for (int e = tid; e < 3 * NC; e += NT) {
-                const int a = e / NC, ql = e % NC;
-                const float2 v = Sl[(size_t)((y0 - 1 + a) & (H - 1)) * NC + ql];
-                R64[e] = make_double2((double)v.x, (double)v.y);
-            }
+            double *terms = reinterpret_cast<double *>(U);
             double nyq[3], c9[9];
 #pragma unroll
             for (int b = 0; b < 3; ++b) nyq[b] = ((x0 - 1 + b) & 1) ? -1.0 : 1.0;
-            __syncthreads();
-            xeval9(R64, [&](int b, int q) { return __ldg(&p.tw64[(q * ((x0 - 1 + b) & (W - 1))) & (W - 1)]); }, nyq, terms, c9);
+            xeval9(
+                [&](int a, int ql, int) {
+                    const float2 v = Sl[(size_t)((y0 - 1 + a) & (H - 1)) * NC + ql];
+                    return make_double2((double)v.x, (double)v.y);
+                },
+                [&](int b, int q) { return tw64[(q * ((x0 - 1 + b) & (W - 1))) & (W - 1)]; }, nyq, terms, c9);
             double bv = -INFINITY;
             int bi = 0x7fffffff;
 #pragma unroll
@@ -957,8 +985,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             constexpr int NSL = (NT / NC) > 0 ? (NT / NC) : 1;  // j-slices per column
             double *dtab = reinterpret_cast<double *>(U);                      // [3][H]
             double2 *part = reinterpret_cast<double2 *>(dtab + 3 * H);         // [3][NSL][NC]
-            double2 *R64 = part + 3 * NSL * NC;                                // [3][NC]
-            double *terms = reinterpret_cast<double *>(R64 + 3 * NC);          // [9][NC]
+            double *terms = reinterpret_cast<double *>(part + 3 * NSL * NC);   // [9][NC]
             for (int iter = 0; iter < 8; ++iter) {
                 // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
                 // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j'):
@@ -984,16 +1011,6 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     part[(1 * NSL + sl) * NC + ql] = s1;
                     part[(2 * NSL + sl) * NC + ql] = s2;
                 }
-                __syncthreads();
-                for (int e = tid; e < 3 * NC; e += NT) {
-                    const int a = e / NC, ql = e % NC;
-                    double2 s = make_double2(0.0, 0.0);
-                    for (int sl = 0; sl < NSL; ++sl) {
-                        const double2 t = part[(a * NSL + sl) * NC + ql];
-                        s.x += t.x, s.y += t.y;
-                    }
-                    R64[e] = s;
-                }
                 double nyq[3], c9[9];
                 const double sgx = (x0 & 1) ? -1.0 : 1.0;
 #pragma unroll
@@ -1003,11 +1020,23 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
                 __syncthreads();
                 xeval9(
-                    R64,
+                    [&](int a, int ql, int sub) {  // sum of the j-slices, 8 lanes per (a, ql)
+                        double sx = 0.0, sy = 0.0;
+                        for (int sl = sub; sl < NSL; sl += 8) {
+                            const double2 t = part[(a * NSL + sl) * NC + ql];
+                            sx += t.x, sy += t.y;
+                        }
+#pragma unroll
+                        for (int o = 1; o < 8; o <<= 1) {
+                            sx += __shfl_xor_sync(0xffffffffu, sx, o);
+                            sy += __shfl_xor_sync(0xffffffffu, sy, o);
+                        }
+                        return make_double2(sx, sy);
+                    },
                     [&](int b, int q) {
                         // exp(2 pi i q (x0 u + n - c) / (u W)) = exp(2 pi i q x0 / W) * exp(2 pi i q (n - c) / (u W))
                         const int nn = min(max(ns - 1 + b, 0), M - 1);
-                        const double2 w0 = __ldg(&p.tw64[(q * x0) & (W - 1)]);
+                        const double2 w0 = tw64[(q * x0) & (W - 1)];
                         const double2 w1 = __ldg(&p.Xpol[(size_t)nn * (W / 2) + q]);
                         return make_double2(w0.x * w1.x - w0.y * w1.y, w0.x * w1.y + w0.y * w1.x);
                     },
@@ -1091,7 +1120,7 @@ struct Launcher {
         v.TM1 = C::TM1, v.TN1 = C::TN1, v.TM2 = C::TM2, v.TN2 = C::TN2;
         v.R1 = C::R1, v.Cn1 = C::Cn1, v.R2 = C::R2, v.Cn2 = C::Cn2, v.KS2 = C::KS2, v.BK1 = C::BK1, v.G2 = C::G2;
         v.s_global = C::SG ? 1 : 0;
-        v.NSTG = NSTG;
+        v.NSTG = C::NSTG;
         v.fixed_smem = &fixed_smem;
         v.raw_scratch_bytes = &raw_scratch_bytes;
         v.prepare = &prepare;
