@@ -19,13 +19,13 @@
 #include "cc_common.h"
 
 // ------------------------------------------------------------------ variants
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD) CcVariant cc_variant_##name();
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1) CcVariant cc_variant_##name();
 #include "cc_variant_list.h"
 #undef CCV
 
 typedef CcVariant (*cc_variant_fn)();
 static const cc_variant_fn g_variant_fns[] = {
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD) &cc_variant_##name,
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1) &cc_variant_##name,
 #include "cc_variant_list.h"
 #undef CCV
 };
@@ -144,7 +144,7 @@ static bool plan_variant(VarPlan &vp, int M, int W, int H)
     const int NSL = std::max(1, v.NT / NC);
     const int polish = 3 * H * 8 + 3 * NSL * NC * 16 + 3 * NC * 16 + 9 * NC * 8;
     const int lower = std::max(v.raw_scratch_bytes(), polish);
-    const int red_bytes = (v.KS2 - 1) * v.R2 * v.Cn2 * 2 * v.TM2 * v.TN2 * 4;
+    const int red_bytes = std::max((v.KS2 - 1) * v.R2 * v.Cn2 * 2 * v.TM2 * v.TN2, (v.KS1 - 1) * v.R1 * v.Cn1 * v.TM1 * v.TN1) * 4;
     const long avail = (long)SMEM_LIMIT - (long)v.fixed_smem() - 32;
     if (avail < lower) return false;
     const int LDT = W + 4;

@@ -110,6 +110,7 @@ struct CcVariant {
     int H, W, CS, NT, dtype;  // dtype: 0 = u8, 1 = u16
     int TM1, TN1, TM2, TN2;
     int R1, Cn1, R2, Cn2, KS2;  // thread grids of the two GEMM stages (rows x cols [x k-split])
+    int KS1;                    // k-split of stage 1
     int BK1, G2;                // stage-1 k-rows per tile; stage-2 groups of 4 k-rows per tile
     int s_global;  // 1: spectrum array lives in global memory (L2), 0: shared memory / DSMEM
     int NSTG;

@@ -232,7 +232,7 @@ __device__ __forceinline__ void load_vec(float (&d)[n], const float *s)
 
 // ------------------------------------------------------------------ the kernel
 template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
-          int R2_, int KS2_, int NSTG_, int PFD_>
+          int R2_, int KS2_, int NSTG_, int PFD_, int KS1_>
 struct Cfg {
     static constexpr int NSTG = NSTG_;  // staging ring depth
     static constexpr int PFD = PFD_;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
@@ -240,7 +240,7 @@ struct Cfg {
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
-    static constexpr int BK1 = BK1_, G2 = G2_, R2 = R2_, KS2 = KS2_;
+    static constexpr int BK1 = BK1_, G2 = G2_, R2 = R2_, KS2 = KS2_, KS1 = KS1_;
     static constexpr bool SG = SG_;
     using PIX = PIX_;
     static constexpr int NC = W / 2 / CS;   // spectrum columns per CTA (column 0 of rank 0 packs DC + Nyquist)
@@ -255,9 +255,10 @@ struct Cfg {
     static constexpr int CHB = RCH * W * (int)sizeof(PIX);
     static constexpr int RAWB = (NCHK > 1 ? 2 : 1) * CHB;
     static constexpr int SCRB = NWARP * PADW * 8;
-    // stage 1: thread grid R1 (rows of [U|V]) x Cn1 (groups of TN1 spectrum floats); a warp covers WR1 x WC1 threads
+    // stage 1: thread grid R1 (rows of [U|V]) x Cn1 (groups of TN1 spectrum floats) x KS1 (k-split); a warp covers
+    // WR1 x WC1 threads of one k-slice
     static constexpr int Cn1 = 2 * NC / TN1;
-    static constexpr int R1 = NT / Cn1;
+    static constexpr int R1 = NT / (Cn1 * KS1);
     static constexpr int WC1 = Cn1 < 8 ? Cn1 : 8;
     static constexpr int WR1 = 32 / WC1;
     static constexpr int WG1C = Cn1 / WC1;
@@ -274,7 +275,9 @@ struct Cfg {
     static constexpr int T2F = G2 * GF2;                 // floats of a stage-2 tile
     static constexpr int NCOL2 = Cn2 * TN2;              // e-columns per stage-2 chunk
     static constexpr int TILEF = T1F > T2F ? T1F : T2F;  // floats per staging slot
-    static constexpr int RED_FLOATS = (KS2 - 1) * R2 * Cn2 * 2 * TM2 * TN2;
+    static constexpr int RED2_FLOATS = (KS2 - 1) * R2 * Cn2 * 2 * TM2 * TN2;
+    static constexpr int RED1_FLOATS = (KS1 - 1) * R1 * Cn1 * TM1 * TN1;
+    static constexpr int RED_FLOATS = RED1_FLOATS > RED2_FLOATS ? RED1_FLOATS : RED2_FLOATS;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
     static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64;
@@ -282,8 +285,8 @@ struct Cfg {
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
     static_assert(NR % RCH == 0 && RCH % 2 == 0, "bad raw chunking");
-    static_assert((2 * NC) % TN1 == 0 && NT % Cn1 == 0 && TN1 % 4 == 0 && Cn1 % WC1 == 0 && 32 % WC1 == 0, "bad stage-1 tiling");
-    static_assert(R1 % 4 == 0 && R1 % WR1 == 0 && (R1 / WR1) * WG1C == NWARP, "bad stage-1 warp grid");
+    static_assert((2 * NC) % TN1 == 0 && NT % (Cn1 * KS1) == 0 && TN1 % 4 == 0 && Cn1 % WC1 == 0 && 32 % WC1 == 0, "bad stage-1 tiling");
+    static_assert(R1 % 4 == 0 && R1 % WR1 == 0 && (R1 / WR1) * WG1C * KS1 == NWARP && BK1 % KS1 == 0, "bad stage-1 warp grid");
     static_assert(TM1 == 1 || TM1 == 2 || TM1 == 3 || TM1 == 4 || TM1 == 5 || TM1 == 8 || TM1 == 10, "TM1 chunking");
     static_assert(R2 * Cn2 * KS2 == NT && Cn2 % WC2 == 0 && 32 % WC2 == 0 && R2 % WR2 == 0, "bad stage-2 tiling");
     static_assert(WG2R * WG2C * KS2 == NWARP && (TN2 == 4 || TN2 == 5) && G2 % KS2 == 0 && W % (4 * G2) == 0, "bad stage-2 tiling");
@@ -324,14 +327,6 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
 
-    const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
-    if constexpr (C::LAT) {
-        double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
-        for (int i = tid; i < W; i += NT) t64[i] = p.tw64[i];
-        tw64 = t64;
-    }
-
-    PIX *const raw = reinterpret_cast<PIX *>(U);
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
 
@@ -347,17 +342,22 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         else __syncthreads();
     };
 
-    // ---- one-time setup
-    for (int i = tid; i < NTW; i += NT) tw[i] = p.tw[i];
-    for (int i = tid; i < W; i += NT) rslot[i] = p.row_slot[i];
-    if (tid == 0) {
-        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
-        mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
-        fence_mbar_init();
-    }
-    uint32_t ph = 0;   // phase parity bits of the raw ring
-    int xpar = 0;      // exchange buffer parity
-    csync();
+    PIX *const raw = reinterpret_cast<PIX *>(U);
+    // raw-pixel ring: the first (up to two) chunks of frame f and an L2 prefetch of the cluster's next frame
+    auto issue_raw_head = [&](int f) {  // thread 0 only
+        const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
+        fence_proxy_async();
+        for (int ck = 0; ck < (C::NCHK > 1 ? 2 : 1); ++ck) {
+            mbar_expect_tx(&braw[ck], C::CHB);
+            bulk_g2s(raw + (size_t)ck * C::RCH * W, fbase + (size_t)ck * C::RCH * W, C::CHB, &braw[ck]);
+        }
+        if (f + ncl < p.batch) {  // pull the next frame of this cluster into L2
+            const PIX *nb = fbase + (size_t)ncl * H * W;
+            constexpr uint32_t tot = (uint32_t)NR * W * sizeof(PIX);
+            for (uint32_t o = 0; o < tot; o += 32768u)
+                bulk_prefetch_l2(reinterpret_cast<const unsigned char *>(nb) + o, tot - o < 32768u ? tot - o : 32768u);
+        }
+    };
 
     // ---- operand ring: every frame consumes the same p.ntiles_frame tiles of p.blob in the order of
     // p.sched.  Thread 0 keeps PFD tiles in flight (also across frames and phases); a slot is refilled
@@ -387,21 +387,46 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if (lane == 0) mbar_arrive(&bempty[g_cons % NSTG]);
         ++g_cons;
     };
-    if (tid == 0 && total_tiles > 0) {
-        // initial burst: fetch the first PFD schedule entries with independent loads, then issue the copies
-        uint32_t first[PFD];
+
+    // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts the first PFD operand tiles and
+    // the first frame's raw rows in flight; the table copies of all threads overlap those copies; one cluster
+    // barrier ends the setup.
+    if (tid == 0) {
+        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
+        mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
+        fence_mbar_init();
+        if (total_tiles > 0) {
+            uint32_t first[PFD];  // independent loads of the first schedule entries
+            uint32_t si = 0;
 #pragma unroll
-        for (int i = 0; i < PFD; ++i) first[i] = __ldg(&p.sched[i % p.ntiles_frame]);
-#pragma unroll
-        for (int i = 0; i < PFD; ++i)
-            if (g_load < total_tiles) {
-                mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
-                bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)first[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
-                ++g_load;
+            for (int i = 0; i < PFD; ++i) {
+                first[i] = __ldg(&p.sched[si]);
+                if (++si == (uint32_t)p.ntiles_frame) si = 0;
             }
-        s_idx = g_load % (uint32_t)p.ntiles_frame;
-        next_ti = __ldg(&p.sched[s_idx]);
+            next_ti = __ldg(&p.sched[si]);
+            fence_proxy_async();
+#pragma unroll
+            for (int i = 0; i < PFD; ++i)
+                if (g_load < total_tiles) {
+                    mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
+                    bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)first[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
+                    ++g_load;
+                }
+            s_idx = si;  // == g_load % ntiles_frame whenever the burst was not cut short (otherwise unused)
+        }
+        if (cid < p.batch) issue_raw_head(cid);
     }
+    for (int i = tid; i < NTW; i += NT) tw[i] = p.tw[i];
+    for (int i = tid; i < W; i += NT) rslot[i] = p.row_slot[i];
+    const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
+    if constexpr (C::LAT) {
+        double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
+        for (int i = tid; i < W; i += NT) t64[i] = p.tw64[i];
+        tw64 = t64;
+    }
+    uint32_t ph = 0;   // phase parity bits of the raw ring
+    int xpar = 0;      // exchange buffer parity
+    csync();
 
     const int u = p.u, M = p.M, cM = p.c;
 
@@ -501,19 +526,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         // =============================================================== a1 + a2: ingest and row FFTs
         {
             const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
-            if (tid == 0) {
-                fence_proxy_async();
-                for (int ck = 0; ck < (C::NCHK > 1 ? 2 : 1); ++ck) {
-                    mbar_expect_tx(&braw[ck], C::CHB);
-                    bulk_g2s(raw + (size_t)ck * C::RCH * W, fbase + (size_t)ck * C::RCH * W, C::CHB, &braw[ck]);
-                }
-                if (f + ncl < p.batch) {  // pull the next frame of this cluster into L2
-                    const PIX *nb = fbase + (size_t)ncl * H * W;
-                    constexpr uint32_t tot = (uint32_t)NR * W * sizeof(PIX);
-                    for (uint32_t o = 0; o < tot; o += 32768u)
-                        bulk_prefetch_l2(reinterpret_cast<const unsigned char *>(nb) + o, tot - o < 32768u ? tot - o : 32768u);
-                }
-            }
+            if (tid == 0 && f != cid) issue_raw_head(f);  // the first frame's rows were requested during the setup
             const float c0f = (float)p.c0;
             for (int ck = 0; ck < C::NCHK; ++ck) {
                 const int rb = ck & 1;
@@ -750,12 +763,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             const int DS = p.DS, nd = p.nd, DSBp = p.DSBp, DSB = DS * CS;
             constexpr int TN1 = C::TN1, TM1 = C::TM1, MC1 = C::MC1, R1 = C::R1, Cn1 = C::Cn1, BK1 = C::BK1;
             constexpr int TM2 = C::TM2, TN2 = C::TN2, R2 = C::R2, Cn2 = C::Cn2, KS2 = C::KS2, G2 = C::G2, GF2 = C::GF2;
-            const int tn1 = (warp % C::WG1C) * C::WC1 + lane % C::WC1;
-            const int tm1 = (warp / C::WG1C) * C::WR1 + lane / C::WC1;
+            constexpr int KS1 = C::KS1, NW1 = NWARP / KS1;  // warps per stage-1 k-slice
+            const int ks1 = warp / NW1, w1 = warp % NW1;
+            const int tn1 = (w1 % C::WG1C) * C::WC1 + lane % C::WC1;
+            const int tm1 = (w1 / C::WG1C) * C::WR1 + lane / C::WC1;
             const int ks2 = warp / (C::WG2R * C::WG2C), w2 = warp % (C::WG2R * C::WG2C);
             const int tn2 = (w2 % C::WG2C) * C::WC2 + lane % C::WC2;
             const int tm2 = (w2 / C::WG2C) * C::WR2 + lane / C::WC2;
-            float *const red = Tb + (size_t)2 * DS * LDT;  // k-split partial sums (KS2 > 1)
+            float *const red = Tb + (size_t)2 * DS * LDT;  // k-split partial sums (KS1 > 1, KS2 > 1)
             for (int sb = 0; sb < p.nsb; ++sb) {
                 const int db = sb * DSB;
                 // ---------------- stage 1: rows [U(d) | V(d)] of this super-block, my 2*NC spectrum floats
@@ -771,7 +786,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     for (int kt = 0; kt < p.KT1; ++kt) {
                         const float *At = ring_acquire();
 #pragma unroll
-                        for (int kk = 0; kk < BK1; ++kk) {
+                        for (int kq = 0; kq < BK1 / KS1; ++kq) {
+                            const int kk = kq * KS1 + ks1;
                             const int jj = kt * BK1 + kk;
                             const int ys = (isV ? y0 - jj : y0 + jj) & (H - 1);
                             float a[TM1], b[TN1];
@@ -802,7 +818,29 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         }
                         ring_release();
                     }
+                    if constexpr (KS1 > 1) {  // sum the k-slices into slice 0
+                        const int t1 = tm1 * Cn1 + tn1;
+                        if (ks1 > 0) {
+                            float *r = red + (size_t)(ks1 - 1) * (TM1 * TN1) * (R1 * Cn1) + t1;
+#pragma unroll
+                            for (int i = 0; i < TM1; ++i)
+#pragma unroll
+                                for (int j = 0; j < TN1; ++j) r[(size_t)(i * TN1 + j) * (R1 * Cn1)] = acc[i][j];
+                        }
+                        __syncthreads();
+                        if (ks1 == 0) {
+                            for (int s1 = 0; s1 < KS1 - 1; ++s1) {
+                                const float *r = red + (size_t)s1 * (TM1 * TN1) * (R1 * Cn1) + t1;
+#pragma unroll
+                                for (int i = 0; i < TM1; ++i)
+#pragma unroll
+                                    for (int j = 0; j < TN1; ++j) acc[i][j] += r[(size_t)(i * TN1 + j) * (R1 * Cn1)];
+                            }
+                        }
+                        __syncthreads();
+                    }
                     // epilogue: rotate by exp(2 pi i kx x0 / W), send rows to the CTA that owns offset d
+                    if (ks1 == 0) {
 #pragma unroll
                     for (int v = 0; v < TN1 / 4; ++v)
 #pragma unroll
@@ -837,6 +875,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                     make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]);
                         }
                     }
+                    }  // ks1 == 0
                 }
                 csync();  // U, V rows are at their owners
                 // rows dl and DS+dl become T(c+d) = U+V and T(c-d) = U-V
@@ -1119,6 +1158,7 @@ struct Launcher {
         v.H = C::H, v.W = C::W, v.CS = C::CS, v.NT = C::NT, v.dtype = sizeof(typename C::PIX) == 1 ? 0 : 1;
         v.TM1 = C::TM1, v.TN1 = C::TN1, v.TM2 = C::TM2, v.TN2 = C::TN2;
         v.R1 = C::R1, v.Cn1 = C::Cn1, v.R2 = C::R2, v.Cn2 = C::Cn2, v.KS2 = C::KS2, v.BK1 = C::BK1, v.G2 = C::G2;
+        v.KS1 = C::KS1;
         v.s_global = C::SG ? 1 : 0;
         v.NSTG = C::NSTG;
         v.fixed_smem = &fixed_smem;

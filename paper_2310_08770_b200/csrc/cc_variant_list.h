@@ -1,5 +1,5 @@
 // cc_variant_list.h -- the compiled kernel variants (X-macro).
-// CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD)
+// CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1)
 //   CS  : CTAs per frame (thread-block cluster size)
 //   TM1 x TN1 : per-thread tile of the stage-1 GEMM ([U|V] rows x spectrum floats)
 //   TM2 x TN2 : per-thread tile of the stage-2 GEMM (T rows x offsets e; two accumulators E, O each)
@@ -8,16 +8,17 @@
 //   R2  : thread rows of stage 2;  KS2 : k-split of stage 2 (thread grid R2 x NT/(R2*KS2) x KS2)
 //   NSTG, PFD : operand-ring depth and prefetch distance (tiles); the small-batch variants keep a whole frame's
 //               tiles in flight from kernel start
+//   KS1 : k-split of stage 1 (thread grid NT/(Cn1*KS1) x Cn1 x KS1); > 1 only where M is too small to fill the CTA
 // build.py compiles cc_variant.cu once per line.
-CCV(f64_u16,       64,   64, 1, uint16_t, 256,  5, 8, 10, 5, false,  4,  2, 16,  1,  6,  4)
-CCV(f64_u8,        64,   64, 1, uint8_t,  256,  5, 8, 10, 5, false,  4,  2, 16,  1,  6,  4)
-CCV(f128_u8,      128,  128, 1, uint8_t,  256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4)
-CCV(f128_u16,     128,  128, 1, uint16_t, 256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4)
-CCV(f128_u8_c8,   128,  128, 8, uint8_t,  256,  1, 4,  1, 4, false,  8,  8,  8,  8, 16, 14)
-CCV(f128_u16_c8,  128,  128, 8, uint16_t, 256,  1, 4,  1, 4, false,  8,  8,  8,  8, 16, 14)
-CCV(f256_u16,     256,  256, 2, uint16_t, 256, 10, 8,  5, 5, false,  4,  2, 16,  1,  6,  4)
-CCV(f256_u8,      256,  256, 2, uint8_t,  256, 10, 8,  5, 5, false,  4,  2, 16,  1,  6,  4)
-CCV(f512_u16,     512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false,  8,  4,  8,  4,  6,  4)
-CCV(f512_u8,      512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false,  8,  4,  8,  4,  6,  4)
-CCV(f1024_u16,   1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,   8,  4,  4,  4,  6,  4)
-CCV(f1024_u8,    1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,   8,  4,  4,  4,  6,  4)
+CCV(f64_u16,       64,   64, 1, uint16_t, 256,  5, 8, 10, 5, false,  4,  2, 16,  1,  6,  4,  1)
+CCV(f64_u8,        64,   64, 1, uint8_t,  256,  5, 8, 10, 5, false,  4,  2, 16,  1,  6,  4,  1)
+CCV(f128_u8,      128,  128, 1, uint8_t,  256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4,  1)
+CCV(f128_u16,     128,  128, 1, uint16_t, 256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4,  1)
+CCV(f128_u8_c8,    128,  128, 8, uint8_t,  256,  2, 4,  1, 4, false, 68, 32,  8,  8,  8,  6,  4)
+CCV(f128_u16_c8,   128,  128, 8, uint16_t, 256,  2, 4,  1, 4, false, 68, 32,  8,  8,  8,  6,  4)
+CCV(f256_u16,     256,  256, 2, uint16_t, 256, 10, 8,  5, 5, false,  4,  2, 16,  1,  6,  4,  1)
+CCV(f256_u8,      256,  256, 2, uint8_t,  256, 10, 8,  5, 5, false,  4,  2, 16,  1,  6,  4,  1)
+CCV(f512_u16,     512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false,  8,  4,  8,  4,  6,  4,  1)
+CCV(f512_u8,      512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false,  8,  4,  8,  4,  6,  4,  1)
+CCV(f1024_u16,   1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,   8,  4,  4,  4,  6,  4,  1)
+CCV(f1024_u8,    1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,   8,  4,  4,  4,  6,  4,  1)
