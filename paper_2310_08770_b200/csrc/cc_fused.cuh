@@ -67,6 +67,19 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes
 {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
+// address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+// 8-byte store into a peer CTA's shared memory that completes 8 tx-bytes on the peer's mbarrier
+__device__ __forceinline__ void st_async_b64(uint32_t raddr, uint64_t v, uint32_t rbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr), "l"(v), "r"(rbar)
+                 : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -236,7 +249,7 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
 struct Cfg {
     static constexpr int NSTG = NSTG_;  // staging ring depth
     static constexpr int PFD = PFD_;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
-    static constexpr int NBARS = 2 * NSTG + 2;  // full[NSTG], empty[NSTG], raw ring [2]
+    static constexpr int NBARS = 2 * NSTG + 4;  // full[NSTG], empty[NSTG], raw ring [2], cluster exchange [2]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -320,7 +333,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     unsigned char *misc = reinterpret_cast<unsigned char *>(rslot + W);
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
-    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG;
+    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG, *const xbar = braw + 2;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
     float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
@@ -394,6 +407,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     if (tid == 0) {
         for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
         mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
+        mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1);
         fence_mbar_init();
         if (total_tiles > 0) {
             uint32_t first[PFD];  // independent loads of the first schedule entries
@@ -426,43 +440,83 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     }
     uint32_t ph = 0;   // phase parity bits of the raw ring
     int xpar = 0;      // exchange buffer parity
+    uint32_t xph = 0;  // phase parity bits of the two exchange barriers
     csync();
 
     const int u = p.u, M = p.M, cM = p.c;
 
-    // cluster-wide exchange of xsrc[0..n): after the call xchg[par][r][k] holds rank r's record
+    // cluster-wide exchange of xsrc[0..n): after the call xchg[par][r][k] holds rank r's record.  Every CTA
+    // stores its record into every peer with st.async, which completes tx-bytes on the PEER's mbarrier: a
+    // one-way DSMEM latency instead of remote stores + a full cluster barrier.  Two buffers/barriers alternate;
+    // a CTA cannot run two exchanges ahead of a peer because each exchange needs that peer's record.
     auto exchange = [&](int n) -> const double * {
-        __syncthreads();
-        if (tid < CS * n) {
-            const int r = tid / n, k = tid % n;
-            double *dst = xchg + ((size_t)xpar * CS + rank) * XN + k;
-            if constexpr (CS > 1) dst = cluster.map_shared_rank(dst, r);
-            *dst = xsrc[k];
-        }
-        csync();
+        __syncthreads();  // xsrc complete; all reads of the buffer used two exchanges ago are done
         const double *res = xchg + (size_t)xpar * CS * XN;
+        if constexpr (CS > 1) {
+            if (tid == 0) mbar_expect_tx(&xbar[xpar], (uint32_t)(CS * n * 8));
+            if (tid < CS * n) {
+                const int r = tid / n, k = tid - r * n;
+                const uint32_t dst = mapa_u32(smem_u32(xchg + ((size_t)xpar * CS + rank) * XN + k), (uint32_t)r);
+                st_async_b64(dst, (uint64_t)__double_as_longlong(xsrc[k]), mapa_u32(smem_u32(&xbar[xpar]), (uint32_t)r));
+            }
+            mbar_wait(&xbar[xpar], (xph >> xpar) & 1u);
+            xph ^= 1u << xpar;
+        } else {
+            if (tid < n) xchg[(size_t)xpar * XN + tid] = xsrc[tid];
+            __syncthreads();
+        }
         xpar ^= 1;
         return res;
     };
-    // block-wide argmax; result valid in thread 0
-    auto block_best = [&](Best b) -> Best {
+    // one exchange round: arm the barrier of buffer xpar (thread 0), wait for every rank's record, flip
+    auto xchg_arm = [&](int bytes_per_rank) {
+        if constexpr (CS > 1) mbar_expect_tx(&xbar[xpar], (uint32_t)(CS * bytes_per_rank));
+    };
+    auto xchg_send = [&](int k, uint64_t bits, int r) {  // my record word k -> rank r
+        if constexpr (CS > 1) {
+            const uint32_t dst = mapa_u32(smem_u32(xchg + ((size_t)xpar * CS + rank) * XN + k), (uint32_t)r);
+            st_async_b64(dst, bits, mapa_u32(smem_u32(&xbar[xpar]), (uint32_t)r));
+        } else {
+            reinterpret_cast<uint64_t *>(xchg)[(size_t)xpar * XN + k] = bits;
+        }
+    };
+    auto xchg_wait = [&]() -> const double * {
+        const double *res = xchg + (size_t)xpar * CS * XN;
+        if constexpr (CS > 1) {
+            mbar_wait(&xbar[xpar], (xph >> xpar) & 1u);
+            xph ^= 1u << xpar;
+        } else {
+            __syncthreads();
+        }
+        xpar ^= 1;
+        return res;
+    };
+    // cluster-wide argmax: warp shuffles -> warp 0 over the warp records -> one 8-byte record (value, index) per
+    // rank to every peer.  The same (larger value, then smaller index) rule at every level; result in all threads.
+    auto cluster_best = [&](Best b) -> Best {
         b = warp_best(b);
         if (lane == 0) {
             wv[warp] = b.v;
             wi[warp] = b.i;
         }
-        __syncthreads();
-        Best r = b;
-        if (tid == 0) {
-            r.v = wv[0];
-            r.i = wi[0];
-            for (int w = 1; w < NWARP; ++w)
-                if (better(wv[w], wi[w], r.v, r.i)) {
-                    r.v = wv[w];
-                    r.i = wi[w];
-                }
+        __syncthreads();  // also: all reads of the exchange buffer used two rounds ago are done
+        if (warp == 0) {
+            Best c{-INFINITY, 0x7fffffff};
+            if (lane < NWARP) c.v = wv[lane], c.i = wi[lane];
+            c = warp_best(c);
+            if (lane == 0) xchg_arm(8);
+            if (lane < CS) xchg_send(0, (uint64_t)__float_as_uint(c.v) | ((uint64_t)(uint32_t)c.i << 32), lane);
         }
-        return r;
+        const uint64_t *res = reinterpret_cast<const uint64_t *>(xchg_wait());
+        Best g{-INFINITY, 0x7fffffff};
+#pragma unroll
+        for (int r = 0; r < CS; ++r) {
+            const uint64_t w = res[r * XN];
+            const float v = __uint_as_float((uint32_t)w);
+            const int i = (int)(uint32_t)(w >> 32);
+            if (better(v, i, g.v, g.i)) g.v = v, g.i = i;
+        }
+        return g;
     };
 
     auto bar_wait = [&](int b) {  // raw ring barriers
@@ -487,12 +541,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             const double2 r = getR(a, ql, sub);
             if (sub < 3) {
                 double v;
-                if (q == 0) v = r.x + r.y * nyq_c[sub];
+                if (q == 0) v = r.x + r.y * (sub == 0 ? nyq_c[0] : sub == 1 ? nyq_c[1] : nyq_c[2]);
                 else v = 2.0 * (r.x * cs.x - r.y * cs.y);
                 terms[(a * 3 + sub) * NC + ql] = v;
             }
         }
-        __syncthreads();
+        __syncthreads();  // terms complete; all reads of the exchange buffer used two rounds ago are done
+        if (tid == 0) xchg_arm(72);
         if (tid < 96) {  // three whole warps: 8 lanes per output k = a*3+b (k >= 9: idle groups)
             const int k = tid >> 3, sub = tid & 7;
             double sum = 0.0;
@@ -501,15 +556,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             sum += __shfl_xor_sync(0xffffffffu, sum, 1);
             sum += __shfl_xor_sync(0xffffffffu, sum, 2);
             sum += __shfl_xor_sync(0xffffffffu, sum, 4);
-            if (k < 9 && sub == 0) xsrc[k] = sum;
+            if (k < 9 && sub < CS) {  // lane sub sends this CTA's k-th sum to rank sub (CS <= 8)
+                for (int r = sub; r < CS; r += 8) xchg_send(k, (uint64_t)__double_as_longlong(sum), r);
+            }
         }
-        const double *res = exchange(9);
+        const double *res = xchg_wait();
+        double mine = 0.0;  // lane k < 9 of every warp: sum over the ranks, in rank order
+        if (lane < 9)
+            for (int r = 0; r < CS; ++r) mine += res[r * XN + lane];
 #pragma unroll
-        for (int k = 0; k < 9; ++k) {
-            double sum = 0.0;
-            for (int r = 0; r < CS; ++r) sum += res[r * XN + k];
-            out[k] = sum;
-        }
+        for (int k = 0; k < 9; ++k) out[k] = __shfl_sync(0xffffffffu, mine, k);
     };
 
     long long tph = 0;
@@ -688,18 +744,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
                 __syncwarp();
             }
-            bst = block_best(bst);
-            if (tid == 0) {
-                xsrc[0] = (double)bst.v;
-                xsrc[1] = (double)bst.i;
-            }
-            const double *res = exchange(2);
-            Best g{(float)res[0], (int)res[1]};
-            for (int r = 1; r < CS; ++r) {
-                const float v = (float)res[r * XN];
-                const int i = (int)res[r * XN + 1];
-                if (better(v, i, g.v, g.i)) g.v = v, g.i = i;
-            }
+            const Best g = cluster_best(bst);
             y0 = g.i / W;
             x0 = g.i % W;
             stamp(2, f);
@@ -1001,18 +1046,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
         int ms, ns;
         {
-            sub = block_best(sub);
-            if (tid == 0) {
-                xsrc[0] = (double)sub.v;
-                xsrc[1] = (double)sub.i;
-            }
-            const double *res = exchange(2);
-            Best g{(float)res[0], (int)res[1]};
-            for (int r = 1; r < CS; ++r) {
-                const float v = (float)res[r * XN];
-                const int i = (int)res[r * XN + 1];
-                if (better(v, i, g.v, g.i)) g.v = v, g.i = i;
-            }
+            const Best g = cluster_best(sub);
             ms = g.i / M;
             ns = g.i % M;
         }
