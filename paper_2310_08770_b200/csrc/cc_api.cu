@@ -57,6 +57,7 @@ struct VarPlan {
     int ntiles_frame = 0, tile_floats = 0, u_bytes = 0;
     float *blob = nullptr;      // device: staged operand tiles
     uint32_t *sched = nullptr;  // device: per-frame tile order
+    uint32_t sched_head[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     float *nyqc = nullptr;      // device: cos(pi e / u)
     float2 *Sg = nullptr;       // global spectrum scratch (s_global variants)
     size_t sg_bytes = 0;
@@ -291,6 +292,7 @@ static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *
         const long long r2 = (long long)e % (2LL * u);
         nyq[e] = (float)cos(M_PI * (double)r2 / (double)u);
     }
+    for (int i = 0; i < 8; ++i) vp.sched_head[i] = sched.empty() ? 0u : sched[(size_t)i % sched.size()];
     cudaError_t e = upload(&vp.blob, blob, acc);
     if (e == cudaSuccess) e = upload(&vp.sched, sched, acc);
     if (e == cudaSuccess) e = upload(&vp.nyqc, nyq, acc);
@@ -478,6 +480,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
 {
     p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
     p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg;
+    for (int i = 0; i < 8; ++i) p.sched_head[i] = vp.sched_head[i];
     p.tw64 = pl->tw64, p.Dpol = pl->Dpol, p.Xpol = pl->Xpol, p.nyq64 = pl->nyq64;
     p.u = pl->u, p.M = pl->M, p.c = pl->c, p.nd = pl->c + 1;
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;

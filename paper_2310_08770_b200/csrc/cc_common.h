@@ -81,6 +81,7 @@ struct CcParams {
     const float *blob;            // staged GEMM operand tiles (stage-1 even/odd Dirichlet tiles, stage-2 cos/sin tiles),
                                   // tile t at blob + t * tile_floats
     const uint32_t *sched;        // [ntiles_frame] blob tile index of the i-th tile a frame consumes
+    uint32_t sched_head[8];       // sched[i % ntiles_frame], i < 8: the initial burst of the operand ring
     const float *nyqc;            // [ne_pad] cos(pi e / u): Nyquist-column weight of stage 2
     float2 *Sg;                   // global spectrum scratch (variants with S in L2), else null
     // fp64 tables of the two argmax polish steps (exactly reduced integer phase numerators, built at plan time)

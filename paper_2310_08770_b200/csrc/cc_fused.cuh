@@ -305,7 +305,7 @@ struct Cfg {
     static_assert(WG2R * WG2C * KS2 == NWARP && (TN2 == 4 || TN2 == 5) && G2 % KS2 == 0 && W % (4 * G2) == 0, "bad stage-2 tiling");
     static_assert(TILEF % 4 == 0 && MC1 % 4 == 0, "tile alignment");
     static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
-    static_assert(NSTG - PFD >= 2, "ring");
+    static_assert(NSTG - PFD >= 2 && PFD <= 8, "ring (sched_head carries 8 entries)");
 };
 
 template <class C>
@@ -410,11 +410,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1);
         fence_mbar_init();
         if (total_tiles > 0) {
-            uint32_t first[PFD];  // independent loads of the first schedule entries
+            uint32_t first[PFD];  // the first schedule entries ride in the kernel parameters: no load latency
             uint32_t si = 0;
 #pragma unroll
             for (int i = 0; i < PFD; ++i) {
-                first[i] = __ldg(&p.sched[si]);
+                first[i] = p.sched_head[i];
                 if (++si == (uint32_t)p.ntiles_frame) si = 0;
             }
             next_ti = __ldg(&p.sched[si]);
@@ -430,13 +430,34 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
         if (cid < p.batch) issue_raw_head(cid);
     }
-    for (int i = tid; i < NTW; i += NT) tw[i] = p.tw[i];
-    for (int i = tid; i < W; i += NT) rslot[i] = p.row_slot[i];
     const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
-    if constexpr (C::LAT) {
-        double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
-        for (int i = tid; i < W; i += NT) t64[i] = p.tw64[i];
-        tw64 = t64;
+    {   // table copies: all loads first (independent, non-coherent path), then the stores
+        constexpr int NI_TW = (NTW + NT - 1) / NT, NI_W = (W + NT - 1) / NT;
+        float2 r_tw[NI_TW];
+        uint16_t r_rs[NI_W];
+        double2 r_64[C::LAT ? NI_W : 1];
+#pragma unroll
+        for (int e = 0; e < NI_TW; ++e)
+            if (tid + e * NT < NTW) r_tw[e] = __ldg(&p.tw[tid + e * NT]);
+#pragma unroll
+        for (int e = 0; e < NI_W; ++e)
+            if (tid + e * NT < W) {
+                r_rs[e] = __ldg(&p.row_slot[tid + e * NT]);
+                if constexpr (C::LAT) r_64[e] = __ldg(&p.tw64[tid + e * NT]);
+            }
+#pragma unroll
+        for (int e = 0; e < NI_TW; ++e)
+            if (tid + e * NT < NTW) tw[tid + e * NT] = r_tw[e];
+#pragma unroll
+        for (int e = 0; e < NI_W; ++e)
+            if (tid + e * NT < W) rslot[tid + e * NT] = r_rs[e];
+        if constexpr (C::LAT) {
+            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
+#pragma unroll
+            for (int e = 0; e < NI_W; ++e)
+                if (tid + e * NT < W) t64[tid + e * NT] = r_64[e];
+            tw64 = t64;
+        }
     }
     uint32_t ph = 0;   // phase parity bits of the raw ring
     int xpar = 0;      // exchange buffer parity
@@ -445,29 +466,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     const int u = p.u, M = p.M, cM = p.c;
 
-    // cluster-wide exchange of xsrc[0..n): after the call xchg[par][r][k] holds rank r's record.  Every CTA
-    // stores its record into every peer with st.async, which completes tx-bytes on the PEER's mbarrier: a
-    // one-way DSMEM latency instead of remote stores + a full cluster barrier.  Two buffers/barriers alternate;
-    // a CTA cannot run two exchanges ahead of a peer because each exchange needs that peer's record.
-    auto exchange = [&](int n) -> const double * {
-        __syncthreads();  // xsrc complete; all reads of the buffer used two exchanges ago are done
-        const double *res = xchg + (size_t)xpar * CS * XN;
-        if constexpr (CS > 1) {
-            if (tid == 0) mbar_expect_tx(&xbar[xpar], (uint32_t)(CS * n * 8));
-            if (tid < CS * n) {
-                const int r = tid / n, k = tid - r * n;
-                const uint32_t dst = mapa_u32(smem_u32(xchg + ((size_t)xpar * CS + rank) * XN + k), (uint32_t)r);
-                st_async_b64(dst, (uint64_t)__double_as_longlong(xsrc[k]), mapa_u32(smem_u32(&xbar[xpar]), (uint32_t)r));
-            }
-            mbar_wait(&xbar[xpar], (xph >> xpar) & 1u);
-            xph ^= 1u << xpar;
-        } else {
-            if (tid < n) xchg[(size_t)xpar * XN + tid] = xsrc[tid];
-            __syncthreads();
-        }
-        xpar ^= 1;
-        return res;
-    };
+    // Cluster-wide exchanges: every CTA stores its record into every peer with st.async, which completes
+    // tx-bytes on the PEER's mbarrier: a one-way DSMEM latency instead of remote stores + a full cluster barrier.
+    // Two buffers/barriers alternate; a CTA cannot run two exchanges ahead of a peer because each exchange needs
+    // that peer's record.
     // one exchange round: arm the barrier of buffer xpar (thread 0), wait for every rank's record, flip
     auto xchg_arm = [&](int bytes_per_rank) {
         if constexpr (CS > 1) mbar_expect_tx(&xbar[xpar], (uint32_t)(CS * bytes_per_rank));
