@@ -144,6 +144,49 @@ cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
 cc_status cc_track_latency_probe(const cc_plan *plan, const void *frames, int n,
                                  float *dx, float *dy, float *peak, double *lat_us, void *stream);
 
+/*
+ * Real-time session -- the paper's real-time mode (PAPER.md:L102-104, L216:
+ * every camera frame is analysed as it arrives and the displacement is fed
+ * back): one persistent cluster kernel stays resident and serves single
+ * frames handed to it through a mailbox in mapped host memory, so a frame
+ * costs neither a kernel launch nor a stream synchronisation.  Same kernel
+ * code, same results as cc_track(batch = 1).
+ *
+ * cc_rt_open      starts the session kernel on a stream owned by the session.
+ *   idle_timeout_ms  the kernel exits by itself after this long without a
+ *                    frame (<= 0: 1000 ms); the next cc_rt_submit restarts it.
+ *                    While the kernel is resident, device-wide synchronisation
+ *                    (cudaDeviceSynchronize, cudaFree, ...) blocks until it
+ *                    exits: use stream or event synchronisation instead.
+ * cc_rt_submit    hands over one frame: DEVICE pointer, or HOST pointer to
+ *                 pinned mapped memory (the kernel then reads the pixels over
+ *                 PCIe itself); H*W pixels, 16-byte aligned; must stay valid
+ *                 until cc_rt_wait returns.  One frame in flight at a time.
+ * cc_rt_wait      spins (host) until the result of the submitted frame has
+ *                 arrived; dx, dy, peak are HOST pointers (peak may be NULL).
+ * cc_rt_track     submit + wait.
+ * cc_rt_close     ends the kernel, frees the session.  NULL is a no-op.  Close
+ *                 every session before cc_plan_destroy.
+ * Errors: CC_ERR_INVALID_ARG (NULL/misaligned/no frame submitted),
+ * CC_ERR_CUDA (launch failure, or no answer from the kernel).
+ */
+typedef struct cc_rt cc_rt;
+cc_status cc_rt_open(cc_plan *plan, int idle_timeout_ms, cc_rt **out);
+cc_status cc_rt_submit(cc_rt *rt, const void *frame);
+cc_status cc_rt_wait(cc_rt *rt, float *dx, float *dy, float *peak);
+cc_status cc_rt_track(cc_rt *rt, const void *frame, float *dx, float *dy, float *peak);
+cc_status cc_rt_close(cc_rt *rt);
+
+/*
+ * cc_rt_latency_probe -- measurement aid: n sequential cc_rt_track calls on
+ * consecutive frames with the host monotonic clock around each call.
+ *   frames   n frames, DEVICE or pinned mapped HOST pointer
+ *   dx,dy,peak  HOST pointers, n float32 each (peak may be NULL)
+ *   lat_us   HOST pointer, n latencies in microseconds
+ */
+cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, float *dy, float *peak,
+                              double *lat_us);
+
 /* Frees every device/host allocation of the plan.  NULL is a no-op. */
 cc_status cc_plan_destroy(cc_plan *plan);
 

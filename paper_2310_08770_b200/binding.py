@@ -20,7 +20,8 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_fp32_peak_probe", "cc_track_latency_probe", "cc_status_string", "cc_last_error"]
+           "cc_plan_info", "cc_fp32_peak_probe", "cc_track_latency_probe",
+           "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
 class CcError(RuntimeError):
@@ -61,6 +62,19 @@ def load_library() -> ctypes.CDLL:
         lib.cc_track_host.restype = ci
         lib.cc_track_latency_probe.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp]
         lib.cc_track_latency_probe.restype = ci
+        lib.cc_rt_open.argtypes = [vp, ci, ctypes.POINTER(vp)]
+        lib.cc_rt_open.restype = ci
+        lib.cc_rt_submit.argtypes = [vp, vp]
+        lib.cc_rt_submit.restype = ci
+        fp = ctypes.POINTER(ctypes.c_float)
+        lib.cc_rt_wait.argtypes = [vp, fp, fp, fp]
+        lib.cc_rt_wait.restype = ci
+        lib.cc_rt_track.argtypes = [vp, vp, fp, fp, fp]
+        lib.cc_rt_track.restype = ci
+        lib.cc_rt_close.argtypes = [vp]
+        lib.cc_rt_close.restype = ci
+        lib.cc_rt_latency_probe.argtypes = [vp, vp, ci, vp, vp, vp, vp]
+        lib.cc_rt_latency_probe.restype = ci
         lib.cc_plan_destroy.argtypes = [vp]
         lib.cc_plan_destroy.restype = ci
         lib.cc_plan_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
@@ -203,6 +217,42 @@ class Plan:
                                  dx.ctypes.data_as(ctypes.c_void_p), dy.ctypes.data_as(ctypes.c_void_p),
                                  peak.ctypes.data_as(ctypes.c_void_p)))
         return dx, dy, peak
+
+
+class RtSession:
+    """cc_rt_open / cc_rt_track / cc_rt_close (include/cc.h): a resident session kernel serves single frames.
+    While a session is open, do not call device-wide synchronisation (torch.cuda.synchronize())."""
+
+    def __init__(self, plan: Plan, idle_timeout_ms: int = 1000):
+        self.plan = plan
+        self._h = ctypes.c_void_p()
+        _check(load_library().cc_rt_open(plan._h, int(idle_timeout_ms), ctypes.byref(self._h)))
+        self._out = (ctypes.c_float * 3)()
+
+    def track(self, frame_ptr: int):
+        """One frame at device (or pinned host) address `frame_ptr`; returns (dx, dy, peak) as Python floats."""
+        o = self._out
+        f = ctypes.c_float
+        _check(load_library().cc_rt_track(self._h, ctypes.c_void_p(frame_ptr), ctypes.cast(ctypes.byref(o, 0), ctypes.POINTER(f)),
+                                          ctypes.cast(ctypes.byref(o, 4), ctypes.POINTER(f)),
+                                          ctypes.cast(ctypes.byref(o, 8), ctypes.POINTER(f))))
+        return o[0], o[1], o[2]
+
+    def latency_probe(self, frames_ptr: int, n: int):
+        """cc_rt_latency_probe: returns (dx, dy, peak, lat_us) numpy arrays."""
+        dx, dy, pk = np.empty(n, np.float32), np.empty(n, np.float32), np.empty(n, np.float32)
+        lat = np.empty(n, np.float64)
+        vp = ctypes.c_void_p
+        _check(load_library().cc_rt_latency_probe(self._h, vp(frames_ptr), n, dx.ctypes.data_as(vp), dy.ctypes.data_as(vp),
+                                                  pk.ctypes.data_as(vp), lat.ctypes.data_as(vp)))
+        return dx, dy, pk, lat
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().cc_rt_close(self._h)
+            self._h = None
+
+    __del__ = close
 
 
 def fp32_peak_probe() -> float:

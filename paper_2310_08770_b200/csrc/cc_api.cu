@@ -596,6 +596,177 @@ extern "C" cc_status cc_track_latency_probe(const cc_plan *plan, const void *fra
     return CC_OK;
 }
 
+// ------------------------------------------------------------------ real-time session
+struct cc_rt {
+    cc_plan *plan = nullptr;
+    const VarPlan *vp = nullptr;
+    cudaStream_t stream = nullptr;
+    void *hbox = nullptr;                      // mapped host memory: [0,16) command, [64,80) result, [128,132) alive
+    volatile unsigned long long *cmd = nullptr;
+    volatile uint32_t *res = nullptr;
+    volatile int *alive = nullptr;
+    void *dbox = nullptr;                      // device view of hbox
+    unsigned long long seq = 0;                // sequence number of the last submitted frame
+    const void *pending = nullptr;             // frame of that submission (for a restart)
+    bool in_flight = false;
+    unsigned long long timeout_ns = 0;
+};
+
+static double mono_us()
+{
+    struct timespec t;
+    clock_gettime(CLOCK_MONOTONIC, &t);
+    return (double)t.tv_sec * 1e6 + (double)t.tv_nsec * 1e-3;
+}
+
+static cc_status rt_launch(cc_rt *rt)
+{
+    // a fresh kernel starts counting at sequence 0: rebase the mailbox
+    CK(cudaStreamSynchronize(rt->stream));
+    rt->seq = 0;
+    rt->cmd[0] = 0, rt->cmd[1] = 0;
+    rt->res[3] = 0;
+    *rt->alive = 1;
+    __sync_synchronize();
+    CcParams p{};
+    fill_params(rt->plan, *rt->vp, p);
+    p.batch = 0;
+    p.rt_cmd = (const volatile unsigned long long *)rt->dbox;
+    p.rt_res = (float *)((char *)rt->dbox + 64);
+    p.rt_alive = (int *)((char *)rt->dbox + 128);
+    p.rt_timeout_ns = rt->timeout_ns;
+    cudaError_t e = rt->vp->v.launch(p, 1, rt->vp->smem_bytes, rt->stream);
+    if (e != cudaSuccess) {
+        *rt->alive = 0;
+        return fail_cuda(e, "session kernel launch");
+    }
+    return CC_OK;
+}
+
+extern "C" cc_status cc_rt_close(cc_rt *rt)
+{
+    if (!rt) return CC_OK;
+    if (rt->cmd) {
+        rt->cmd[0] = ~0ull;  // quit
+        __sync_synchronize();
+    }
+    if (rt->stream) {
+        cudaStreamSynchronize(rt->stream);
+        cudaStreamDestroy(rt->stream);
+    }
+    if (rt->hbox) cudaFreeHost(rt->hbox);
+    delete rt;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_rt_open(cc_plan *plan, int idle_timeout_ms, cc_rt **out)
+{
+    if (!plan || !out) return fail(CC_ERR_INVALID_ARG, "cc_rt_open: null pointer");
+    cc_rt *rt = new (std::nothrow) cc_rt();
+    if (!rt) return fail(CC_ERR_NOMEM, "host allocation failed");
+    rt->plan = plan;
+    rt->vp = plan->has_lat ? &plan->lat : &plan->thr;
+    rt->timeout_ns = (unsigned long long)(idle_timeout_ms > 0 ? idle_timeout_ms : 1000) * 1000000ull;
+    cudaError_t e = cudaHostAlloc(&rt->hbox, 256, cudaHostAllocMapped | cudaHostAllocPortable);
+    if (e == cudaSuccess) {
+        memset(rt->hbox, 0, 256);
+        e = cudaHostGetDevicePointer(&rt->dbox, rt->hbox, 0);
+    }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&rt->stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {
+        cc_status s = fail_cuda(e, "cc_rt_open");
+        if (rt->hbox) cudaFreeHost(rt->hbox);
+        delete rt;
+        return s;
+    }
+    rt->cmd = (volatile unsigned long long *)rt->hbox;
+    rt->res = (volatile uint32_t *)((char *)rt->hbox + 64);
+    rt->alive = (volatile int *)((char *)rt->hbox + 128);
+    cc_status s = rt_launch(rt);
+    if (s != CC_OK) {
+        rt->cmd = nullptr;
+        cc_rt_close(rt);
+        return s;
+    }
+    *out = rt;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_rt_submit(cc_rt *rt, const void *frame)
+{
+    if (!rt || !frame) return fail(CC_ERR_INVALID_ARG, "cc_rt_submit: null pointer");
+    if (((uintptr_t)frame & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_rt_submit: frame must be 16-byte aligned");
+    if (rt->in_flight) return fail(CC_ERR_INVALID_ARG, "cc_rt_submit: a frame is already in flight");
+    if (!*rt->alive) {  // the kernel left after its idle timeout: start it again
+        cc_status s = rt_launch(rt);
+        if (s != CC_OK) return s;
+    }
+    rt->pending = frame;
+    ++rt->seq;
+    rt->cmd[1] = (unsigned long long)(uintptr_t)frame | (rt->seq & 15ull);  // tag: low 4 bits of the sequence number
+    __atomic_store_n((unsigned long long *)&rt->cmd[0], rt->seq, __ATOMIC_RELEASE);
+    rt->in_flight = true;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_rt_wait(cc_rt *rt, float *dx, float *dy, float *peak)
+{
+    if (!rt || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_rt_wait: null pointer");
+    if (!rt->in_flight) return fail(CC_ERR_INVALID_ARG, "cc_rt_wait: no frame submitted");
+    int restarts = 0;
+    double t0 = mono_us();
+    for (;;) {
+        if (__atomic_load_n((uint32_t *)&rt->res[3], __ATOMIC_ACQUIRE) == (uint32_t)rt->seq) break;
+        if (mono_us() - t0 > 2.0e5) {  // 200 ms without an answer
+            // the kernel may have hit its idle timeout just as the frame was submitted: restart once
+            if (!*rt->alive && restarts == 0) {
+                const void *frame = rt->pending;
+                rt->in_flight = false;
+                cc_status s = rt_launch(rt);
+                if (s == CC_OK) s = cc_rt_submit(rt, frame);
+                if (s != CC_OK) return s;
+                ++restarts;
+                t0 = mono_us();
+                continue;
+            }
+            rt->in_flight = false;
+            cudaError_t e = cudaStreamQuery(rt->stream);
+            return fail(CC_ERR_CUDA, std::string("cc_rt_wait: no answer from the session kernel (") +
+                                         cudaGetErrorString(e == cudaErrorNotReady ? cudaSuccess : e) + ")");
+        }
+    }
+    union { uint32_t u; float f; } c;
+    c.u = rt->res[0], *dx = c.f;
+    c.u = rt->res[1], *dy = c.f;
+    c.u = rt->res[2];
+    if (peak) *peak = c.f;
+    rt->in_flight = false;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_rt_track(cc_rt *rt, const void *frame, float *dx, float *dy, float *peak)
+{
+    cc_status s = cc_rt_submit(rt, frame);
+    if (s != CC_OK) return s;
+    return cc_rt_wait(rt, dx, dy, peak);
+}
+
+extern "C" cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, float *dy, float *peak,
+                                         double *lat_us)
+{
+    if (!rt || n < 0) return fail(CC_ERR_INVALID_ARG, "cc_rt_latency_probe: bad session or n");
+    if (n == 0) return CC_OK;
+    if (!frames || !dx || !dy || !lat_us) return fail(CC_ERR_INVALID_ARG, "cc_rt_latency_probe: null pointer");
+    const size_t fbytes = (size_t)rt->plan->H * rt->plan->W * (rt->plan->dtype == CC_U8 ? 1 : 2);
+    for (int i = 0; i < n; ++i) {
+        const double t0 = mono_us();
+        cc_status s = cc_rt_track(rt, (const unsigned char *)frames + (size_t)i * fbytes, dx + i, dy + i, peak ? peak + i : nullptr);
+        lat_us[i] = mono_us() - t0;
+        if (s != CC_OK) return s;
+    }
+    return CC_OK;
+}
+
 extern "C" cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info)
 {
     if (!plan || !info) return fail(CC_ERR_INVALID_ARG, "cc_plan_info: null pointer");

@@ -91,6 +91,12 @@ struct CcParams {
     const double2 *Xpol;          // [M][W/2] (cos, sin)(2 pi q (n - c) / (u W))
     const double *nyq64;          // [M] cos(pi (n - c) / u)
 
+    // real-time session (cc_rt_*): mapped host memory; null outside a session
+    const volatile unsigned long long *rt_cmd;  // [0] sequence number of the newest command (~0: quit), [1] frame pointer | seq & 15
+    float *rt_res;                              // dx, dy, peak, sequence number (as bits): one 16-byte record
+    int *rt_alive;                              // cleared by the kernel when it exits
+    unsigned long long rt_timeout_ns;           // the kernel exits after this long without a command
+
     int u, M, c;        // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
     int nd;             // c + 1: number of |offsets| d (and e) evaluated per axis
     int DS;             // offsets d owned per CTA per super-block (T holds 2*DS rows)

@@ -80,6 +80,18 @@ __device__ __forceinline__ void st_async_b64(uint32_t raddr, uint64_t v, uint32_
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr), "l"(v), "r"(rbar)
                  : "memory");
 }
+__device__ __forceinline__ void ld_sys_v2u64(const volatile unsigned long long *p, uint64_t &a, uint64_t &b)
+{
+    unsigned long long x, y;
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(x), "=l"(y) : "l"(p) : "memory");
+    a = x, b = y;
+}
+__device__ __forceinline__ uint64_t globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -249,7 +261,7 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
 struct Cfg {
     static constexpr int NSTG = NSTG_;  // staging ring depth
     static constexpr int PFD = PFD_;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
-    static constexpr int NBARS = 2 * NSTG + 4;  // full[NSTG], empty[NSTG], raw ring [2], cluster exchange [2]
+    static constexpr int NBARS = 2 * NSTG + 5;  // full[NSTG], empty[NSTG], raw ring [2], cluster exchange [2], rt command [1]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -293,7 +305,7 @@ struct Cfg {
     static constexpr int RED_FLOATS = RED1_FLOATS > RED2_FLOATS ? RED1_FLOATS : RED2_FLOATS;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
-    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64;
+    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64 + 16;
     static constexpr size_t FIXED_BYTES =
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
@@ -333,12 +345,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     unsigned char *misc = reinterpret_cast<unsigned char *>(rslot + W);
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
-    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG, *const xbar = braw + 2;
+    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
     float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
+    uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
 
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
@@ -357,8 +370,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     PIX *const raw = reinterpret_cast<PIX *>(U);
     // raw-pixel ring: the first (up to two) chunks of frame f and an L2 prefetch of the cluster's next frame
-    auto issue_raw_head = [&](int f) {  // thread 0 only
-        const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
+    auto issue_raw_head = [&](const void *frames, int f) {  // thread 0 only
+        const PIX *fbase = reinterpret_cast<const PIX *>(frames) + (size_t)f * H * W + (size_t)rank * NR * W;
         fence_proxy_async();
         for (int ck = 0; ck < (C::NCHK > 1 ? 2 : 1); ++ck) {
             mbar_expect_tx(&braw[ck], C::CHB);
@@ -376,29 +389,31 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     // p.sched.  Thread 0 keeps PFD tiles in flight (also across frames and phases); a slot is refilled
     // once all NWARP warps have released it (empty mbarrier) -- no CTA barrier inside the GEMM loops.
     const uint32_t my_frames = p.batch > cid ? (uint32_t)((p.batch - cid + ncl - 1) / ncl) : 0u;
-    const uint32_t total_tiles = my_frames * (uint32_t)p.ntiles_frame;
-    uint32_t g_cons = 0, g_load = 0, s_idx = 0;
+    // real-time session: frames arrive one by one for as long as the session lives; the ring runs ahead freely
+    const uint32_t total_tiles = p.rt_cmd ? (p.ntiles_frame ? 0xffffffffu : 0u) : my_frames * (uint32_t)p.ntiles_frame;
+    uint32_t g_load = 0, s_idx = 0;            // tiles requested so far (saturating in a session), schedule position
+    uint32_t l_slot = 0, l_par = 0;            // producer: next ring slot and the parity of its empty barrier
+    uint32_t c_slot = 0, c_par = 0;            // consumer: current ring slot and the parity of its full barrier
     uint32_t next_ti = 0u;  // schedule entry of the next tile, fetched one tile ahead (thread 0)
     auto ring_produce = [&]() {  // thread 0 only
-        const uint32_t slot = g_load % NSTG;
-        mbar_wait(&bempty[slot], ((g_load / NSTG) & 1u) ^ 1u);
+        mbar_wait(&bempty[l_slot], l_par ^ 1u);
         const uint32_t ti = next_ti;
-        mbar_expect_tx(&bfull[slot], (uint32_t)C::TILEF * 4u);
-        bulk_g2s(stg + (size_t)slot * C::TILEF, p.blob + (size_t)ti * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[slot]);
-        ++g_load;
+        mbar_expect_tx(&bfull[l_slot], (uint32_t)C::TILEF * 4u);
+        bulk_g2s(stg + (size_t)l_slot * C::TILEF, p.blob + (size_t)ti * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[l_slot]);
+        if (g_load != 0xffffffffu) ++g_load;
+        if (++l_slot == NSTG) l_slot = 0, l_par ^= 1u;
         if (++s_idx == (uint32_t)p.ntiles_frame) s_idx = 0;
         next_ti = __ldg(&p.sched[s_idx]);  // latency overlaps the tile's compute
     };
     auto ring_acquire = [&]() -> const float * {
-        if (tid == 0 && g_load < total_tiles) ring_produce();
-        const uint32_t slot = g_cons % NSTG;
-        mbar_wait(&bfull[slot], (g_cons / NSTG) & 1u);
-        return stg + (size_t)slot * C::TILEF;
+        if (tid == 0 && (g_load < total_tiles || total_tiles == 0xffffffffu)) ring_produce();
+        mbar_wait(&bfull[c_slot], c_par);
+        return stg + (size_t)c_slot * C::TILEF;
     };
     auto ring_release = [&]() {
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bempty[g_cons % NSTG]);
-        ++g_cons;
+        if (lane == 0) mbar_arrive(&bempty[c_slot]);
+        if (++c_slot == NSTG) c_slot = 0, c_par ^= 1u;
     };
 
     // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts the first PFD operand tiles and
@@ -407,7 +422,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     if (tid == 0) {
         for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
         mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
-        mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1);
+        mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1), mbar_init(cbar, 1);
         fence_mbar_init();
         if (total_tiles > 0) {
             uint32_t first[PFD];  // the first schedule entries ride in the kernel parameters: no load latency
@@ -425,10 +440,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
                     bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)first[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
                     ++g_load;
+                    ++l_slot;  // PFD < NSTG: no wrap during the burst
                 }
             s_idx = si;  // == g_load % ntiles_frame whenever the burst was not cut short (otherwise unused)
         }
-        if (cid < p.batch) issue_raw_head(cid);
+        if (!p.rt_cmd && cid < p.batch) issue_raw_head(p.frames, cid);
     }
     const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
     {   // table copies: all loads first (independent, non-coherent path), then the stores
@@ -452,7 +468,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         for (int e = 0; e < NI_W; ++e)
             if (tid + e * NT < W) rslot[tid + e * NT] = r_rs[e];
         if constexpr (C::LAT) {
-            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(f00 + 1) + 15) & ~(uintptr_t)15);
+            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(cmdslot + 2) + 15) & ~(uintptr_t)15);
 #pragma unroll
             for (int e = 0; e < NI_W; ++e)
                 if (tid + e * NT < W) t64[tid + e * NT] = r_64[e];
@@ -579,12 +595,77 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
     };
 
-    for (int f = cid; f < p.batch; f += ncl) {
+    // results of one frame (rank 0, thread 0): batch arrays, or the session's mapped host record
+    const bool RT = p.rt_cmd != nullptr;
+    uint64_t rt_seq = 0;    // sequence number of the command being served
+    uint32_t cph = 0;       // phase parity of the command barrier
+    auto emit = [&](int f, float dyv, float dxv, float pkv, int wyv, int wxv) {
+        if (RT) {  // one 16-byte store; the sequence number is the last word
+            asm volatile("st.volatile.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p.rt_res), "f"(dxv), "f"(dyv), "f"(pkv),
+                         "f"(__uint_as_float((uint32_t)rt_seq))
+                         : "memory");
+            __threadfence_system();
+        } else {
+            p.dy[f] = dyv;
+            p.dx[f] = dxv;
+            if (p.peak) p.peak[f] = pkv;
+            if (p.iy) p.iy[f] = wyv;
+            if (p.ix) p.ix[f] = wxv;
+        }
+    };
+
+    for (int f = cid; RT || f < p.batch; f += ncl) {
+        const void *frames = p.frames;
+        if (RT) {
+            // ---- real-time session (one displacement per camera frame, as it arrives): rank 0
+            // polls the host's command word; (seq, frame pointer) go to every CTA of the cluster by st.async
+            f = 0;
+            if constexpr (CS > 1) {
+                if (tid == 0) mbar_expect_tx(cbar, 16u);
+            }
+            if (rank == 0 && tid == 0) {
+                const uint64_t t0 = globaltimer_ns();
+                uint64_t seq, ptr = 0;
+                for (;;) {
+                    // one 16-byte read over PCIe: (seq, frame pointer | low 4 bits of seq); the tag in the pointer's
+                    // low bits (frames are 16-byte aligned) exposes a read torn between two commands
+                    ld_sys_v2u64(p.rt_cmd, seq, ptr);
+                    if (seq == ~0ull) break;
+                    if (seq == rt_seq + 1 && (ptr & 15ull) == (seq & 15ull)) break;
+                    if (globaltimer_ns() - t0 > p.rt_timeout_ns) {  // idle for too long: end the session kernel
+                        seq = ~0ull;
+                        break;
+                    }
+                }
+                ptr &= ~15ull;
+#pragma unroll
+                for (int r = 0; r < CS; ++r) {
+                    if constexpr (CS > 1) {
+                        const uint32_t rb = mapa_u32(smem_u32(cbar), (uint32_t)r);
+                        st_async_b64(mapa_u32(smem_u32(&cmdslot[0]), (uint32_t)r), seq, rb);
+                        st_async_b64(mapa_u32(smem_u32(&cmdslot[1]), (uint32_t)r), ptr, rb);
+                    } else {
+                        cmdslot[0] = seq, cmdslot[1] = ptr;
+                    }
+                }
+            }
+            if constexpr (CS > 1) {
+                mbar_wait(cbar, cph);
+                cph ^= 1u;
+            } else {
+                __syncthreads();
+            }
+            const uint64_t seq = cmdslot[0];
+            if (seq == ~0ull) break;
+            rt_seq = seq;
+            frames = reinterpret_cast<const void *>(cmdslot[1]);
+            if (tid == 0) issue_raw_head(frames, 0);
+        }
         if (p.phase_clk && rank == 0 && tid == 0) tph = clock64();
         // =============================================================== a1 + a2: ingest and row FFTs
         {
-            const PIX *fbase = reinterpret_cast<const PIX *>(p.frames) + (size_t)f * H * W + (size_t)rank * NR * W;
-            if (tid == 0 && f != cid) issue_raw_head(f);  // the first frame's rows were requested during the setup
+            const PIX *fbase = reinterpret_cast<const PIX *>(frames) + (size_t)f * H * W + (size_t)rank * NR * W;
+            if (tid == 0 && !RT && f != cid) issue_raw_head(frames, f);  // the first frame's rows were requested during the setup
             const float c0f = (float)p.c0;
             for (int ck = 0; ck < C::NCHK; ++ck) {
                 const int rb = ck & 1;
@@ -783,11 +864,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
         if (u == 1) {
             if (rank == 0 && tid == 0) {
-                p.dy[f] = (float)wy;
-                p.dx[f] = (float)wx;
-                if (p.peak) p.peak[f] = (float)(cc_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean);
-                if (p.iy) p.iy[f] = wy;
-                if (p.ix) p.ix[f] = wx;
+                emit(f, (float)wy, (float)wx, (float)(cc_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean), wy, wx);
             }
             csync();
             continue;
@@ -1137,15 +1214,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
         stamp(7, f);
         if (rank == 0 && tid == 0) {
-            p.dy[f] = (float)((double)wy + (double)(ms - cM) / (double)u);
-            p.dx[f] = (float)((double)wx + (double)(ns - cM) / (double)u);
-            if (p.peak) p.peak[f] = (float)(up_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean);
-            if (p.iy) p.iy[f] = wy;
-            if (p.ix) p.ix[f] = wx;
+            emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
+                 (float)(up_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean), wy, wx);
         }
         __syncthreads();  // U (polish scratch) is reused by the next frame's raw ring
     }
     csync();  // no CTA of the cluster exits while peers may still address its shared memory
+    if (RT && rank == 0 && tid == 0) {
+        *reinterpret_cast<volatile int *>(p.rt_alive) = 0;  // the session kernel is gone (quit or idle timeout)
+        __threadfence_system();
+    }
 }
 
 // ------------------------------------------------------------------ host-side launcher glue

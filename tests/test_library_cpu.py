@@ -57,6 +57,10 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.cc_track(None, None, 4, None, None, None, None) == 1
     assert lib.cc_plan_destroy(None) == 0
     assert lib.cc_plan_info(None, None) == 1
+    assert lib.cc_rt_open(None, 0, ctypes.byref(h)) == 1
+    assert lib.cc_rt_submit(None, None) == 1 and lib.cc_rt_wait(None, None, None, None) == 1
+    assert lib.cc_rt_close(None) == 0
+    assert lib.cc_track_latency_probe(None, None, 1, None, None, None, None, None) == 1
 
 
 def test_no_device_is_a_loud_error(lib):

@@ -222,3 +222,61 @@ def test_host_path_matches_device_path(gpu):
 def test_fp32_probe_reports_sane_rate(gpu):
     tf = gpu.fp32_peak_probe()
     assert 30.0 < tf < 80.0
+
+
+@pytest.mark.parametrize("ci,n", [(2, 200), (1, 64), (4, 12)])
+def test_realtime_session_matches_cc_track_and_oracle(gpu, oracle_mod, ci, n):
+    """cc_rt_*: the resident session kernel (mailbox in mapped host memory) returns exactly what
+    cc_track(batch = 1) returns, for frames in device memory and for frames in pinned host memory."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    fr = wl.frames(cfg, np.arange(n))
+    ref = wl.reference(cfg)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    d = plan.device_frames(fr)
+    bx, by, bp = [t.cpu().numpy() for t in plan.track(d)]
+    torch.cuda.current_stream().synchronize()
+    fb = fr[0].nbytes
+    rt = gpu.RtSession(plan, idle_timeout_ms=2000)
+    try:
+        got = np.array([rt.track(d.data_ptr() + i * fb) for i in range(n)], dtype=np.float32)
+        hfr = torch.from_numpy(fr.view(np.uint8).reshape(n, -1)).pin_memory()
+        got_h = np.array([rt.track(hfr.data_ptr() + i * fb) for i in range(n)], dtype=np.float32)
+        dx2, dy2, pk2, lat = rt.latency_probe(d.data_ptr(), n)
+    finally:
+        rt.close()
+    # the batched call may run another kernel variant (cluster size): peak sums associate differently
+    assert np.array_equal(got[:, 0], bx) and np.array_equal(got[:, 1], by) and np.max(np.abs(got[:, 2] / bp - 1)) < 1e-6
+    assert np.array_equal(got_h, got)
+    assert np.array_equal(dx2, got[:, 0]) and np.array_equal(dy2, got[:, 1]) and np.array_equal(pk2, got[:, 2]) and np.all(lat > 0)
+    m = min(n, 24)
+    o = oracle_mod.track(fr[:m], ref, cfg.upsample)
+    assert np.max(np.abs(got[:m, 0] - o.dx)) <= TOL_PX and np.max(np.abs(got[:m, 1] - o.dy)) <= TOL_PX
+    plan.close()
+
+
+def test_realtime_session_restarts_after_idle_timeout(gpu):
+    """The session kernel leaves after its idle timeout; the next frame restarts it transparently."""
+    import time
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(2)
+    fr = wl.frames(cfg, np.arange(4))
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, wl.reference(cfg))
+    d = plan.device_frames(fr)
+    bx, by, _ = [t.cpu().numpy() for t in plan.track(d)]
+    torch.cuda.current_stream().synchronize()
+    rt = gpu.RtSession(plan, idle_timeout_ms=150)
+    try:
+        a = rt.track(d.data_ptr())
+        time.sleep(0.6)                      # > idle timeout: the kernel has exited
+        b = rt.track(d.data_ptr() + fr[0].nbytes)
+        lib = gpu.load_library()
+        assert lib.cc_rt_submit(rt._h, ctypes.c_void_p(d.data_ptr() + 2)) == 1      # misaligned frame
+        assert lib.cc_rt_wait(rt._h, None, None, None) == 1
+    finally:
+        rt.close()
+    torch.cuda.synchronize()                 # returns at once: nothing resident any more
+    assert (a[0], a[1]) == (bx[0], by[0]) and (b[0], b[1]) == (bx[1], by[1])
+    plan.close()
