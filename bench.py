@@ -5,7 +5,8 @@ One "step" = one cc_track() pass of the whole hot path (ingest, FFTs, product,
 argmax, upsampled DFT, sub-pixel argmax) over one batch of seeded synthetic
 frames (BASELINE.json configs[2]: 256x256 uint16, batch 10,000, u = 100 --
 the configuration the roofline target is quoted on).  Also reports the
-single-frame latency of configs[1] (128x128 uint8, u = 20, batch-1 streaming).
+single-frame latency of the streaming configs (configs[1] 128x128 uint8 u = 20, configs[3] 512x512 uint16
+u = 50) through cc_track + stream sync and through the real-time session (cc_rt_*).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
@@ -100,9 +101,9 @@ class ClockSampler:
 
 
 def oracle_rate(cfg, n_frames: int):
-    """Frames/s of the float64 CPU oracle, as it stands, on the first n parity-subset frames."""
+    """Frames/s of the float64 CPU oracle, as it stands, on the first n frames of the batch."""
     import oracle
-    idx = wl.oracle_subset(cfg)[:n_frames]
+    idx = np.arange(min(n_frames, cfg.n_frames))
     fr = wl.frames(cfg, idx)
     ref = wl.reference(cfg)
     oracle.track(fr[:1], ref, cfg.upsample)  # build + warm
@@ -151,8 +152,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--batch", type=int, default=0, help="frames per step (default: the config's 10,000)")
     ap.add_argument("--ref-frames", type=int, default=256, help="frames per step of the --impl reference arm")
-    ap.add_argument("--cpu-frames", type=int, default=512, help="sample size of the cpu_baseline leg")
-    ap.add_argument("--latency-frames", type=int, default=10000)
+    ap.add_argument("--cpu-frames", type=int, default=2048, help="sample size of the cpu_baseline leg")
+    ap.add_argument("--latency-frames", type=int, default=2000)
     ap.add_argument("--no-latency", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -272,45 +273,56 @@ def main():
         "hbm_achieved_gbs": (frames[0].nbytes + 12) * B / (kern_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs,
     }
 
-    # ---- single-frame latency, configs[1]: 128x128 u8, u = 20, sequential batch-1 calls
+    # ---- single-frame latency, the streaming configs (configs[1]: 128x128 u8 u=20; configs[3]: 512x512 u16 u=50):
+    # sequential batch-1 frames, each timed on the host clock from hand-over to result-in-host-memory
     latency = None
     if not args.no_latency:
-        c2 = wl.config(2)
-        nlat = min(args.latency_frames, c2.n_frames)
-        f2 = wl.frames(c2, np.arange(nlat))
-        p2 = Plan(c2.H, c2.W, f2.dtype, c2.upsample, wl.reference(c2))
-        d2 = p2.device_frames(f2)
-        o2 = (torch.empty(1, dtype=torch.float32, device="cuda"), torch.empty(1, dtype=torch.float32, device="cuda"),
-              torch.empty(1, dtype=torch.float32, device="cuda"))
-        lib_track = p2.track
-        for i in range(50):
-            lib_track(d2[i % nlat], 1, out=o2)
-        torch.cuda.synchronize()
-        lat = np.empty(nlat)
-        for i in range(nlat):
-            t0 = time.perf_counter_ns()
-            lib_track(d2[i], 1, out=o2)
-            torch.cuda.synchronize()
-            lat[i] = (time.perf_counter_ns() - t0) * 1e-3
-        # GPU-only time of the same launches (events around 200 back-to-back calls)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for i in range(200):
-            lib_track(d2[i % nlat], 1, out=o2)
-        b.record()
-        torch.cuda.synchronize()
-        latency = {"workload": c2.name, "calls": nlat, "median_us": float(np.median(lat)), "p99_us": float(np.percentile(lat, 99)),
-                   "max_us": float(lat.max()), "gpu_only_us_per_call_back_to_back": a.elapsed_time(b) * 1e3 / 200,
-                   "cluster_size": p2.info()["lat_cluster_size"] or p2.info()["cluster_size"],
-                   "note": "host clock around cc_track(batch=1) + stream sync, frame resident in HBM, through the Python binding"}
-        p2.close()
+        from paper_2310_08770_b200 import RtSession
+        latency = {"note": "per-frame host-clock latency, sequential frames, native timing loops of the C-ABI "
+                           "(cc_track_latency_probe / cc_rt_latency_probe); frame resident in HBM unless stated"}
+        stat = lambda l: {"median_us": float(np.median(l)), "p99_us": float(np.percentile(l, 99)), "max_us": float(l.max())}
+        for ci in (2, 4):
+            c2 = wl.config(ci)
+            nlat = min(args.latency_frames, c2.n_frames)
+            f2 = wl.frames(c2, np.arange(nlat))
+            p2 = Plan(c2.H, c2.W, f2.dtype, c2.upsample, wl.reference(c2))
+            d2 = p2.device_frames(f2)
+            p2.latency_probe(d2, min(100, nlat))
+            leg = {"workload": c2.name, "calls": nlat,
+                   "cluster_size": p2.info()["lat_cluster_size"] or p2.info()["cluster_size"]}
+            # (a) cc_track(batch = 1) + cudaStreamSynchronize per frame
+            leg["cc_track_plus_stream_sync"] = stat(p2.latency_probe(d2, nlat)[3])
+            # GPU-only time of the same launches (events around back-to-back calls)
+            o2 = tuple(torch.empty(1, dtype=torch.float32, device="cuda") for _ in range(3))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for i in range(200):
+                p2.track(d2[i % nlat], 1, out=o2)
+            b.record()
+            torch.cuda.current_stream().synchronize()
+            leg["gpu_only_us_per_call_back_to_back"] = a.elapsed_time(b) * 1e3 / 200
+            # (b) real-time session: resident kernel, mailbox in mapped host memory
+            rt = RtSession(p2, 1000)
+            try:
+                rt.latency_probe(d2.data_ptr(), min(100, nlat))
+                rx, ry, _, lat_rt = rt.latency_probe(d2.data_ptr(), nlat)
+                leg["rt_session"] = stat(lat_rt)
+                h2 = torch.from_numpy(f2.view(np.uint8).reshape(nlat, -1)).pin_memory()
+                rt.latency_probe(h2.data_ptr(), min(100, nlat))
+                leg["rt_session_frame_in_pinned_host_memory"] = stat(rt.latency_probe(h2.data_ptr(), nlat)[3])
+            finally:
+                rt.close()
+            bx, by, _ = [t.cpu().numpy() for t in p2.track(d2)]
+            leg["rt_matches_cc_track"] = bool(np.array_equal(rx, bx) and np.array_equal(ry, by))
+            latency["cfg%d" % ci] = leg
+            p2.close()
 
     # ---- CPU oracle beside it
     cpu = None
     if not args.no_cpu:
         v, cores, n, dt = oracle_rate(cfg, args.cpu_frames)
         cpu = {"value": v, "unit": "frames/s", "cores": cores, "kind": "oracle",
-               "sample": "first %d frames of the cfg-3 parity subset, %.1f s wall" % (n, dt)}
+               "sample": "first %d frames of the 10,000-frame cfg-3 batch, %.1f s wall" % (n, dt)}
 
     line = {
         "metric": "frames_per_s", "value": value, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
