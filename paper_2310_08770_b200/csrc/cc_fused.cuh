@@ -161,56 +161,96 @@ __device__ __forceinline__ void dft_reg(float2 (&v)[R])
 }
 
 // One radix-R butterfly of an in-place FFT pass.  addr(i) -> float2* of the
-// i-th element.  Forward (DIF): DFT then twiddle w^(k*twstep); inverse (DIT):
-// conj twiddle w^(i*twstep) then inverse DFT.  tw[j] = (cos, -sin)(2 pi j / NTW).
-template <int R, bool INV, bool TW, int NTW, class Addr>
-__device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw)
+// i-th element; twf(i) -> twiddle w^(i*twstep) = (cos, -sin), i = 1..R-1.
+// Forward (DIF): DFT then twiddle; inverse (DIT): conj twiddle then inverse DFT.
+template <int R, bool INV, bool TW, class Addr, class Twf>
+__device__ __forceinline__ void fft_bfly(Addr addr, Twf twf)
 {
     float2 v[R];
 #pragma unroll
     for (int i = 0; i < R; ++i) v[i] = *addr(i);
     if (INV && TW) {
 #pragma unroll
-        for (int i = 1; i < R; ++i) v[i] = cmulc(v[i], tw[(i * twstep) & (NTW - 1)]);
+        for (int i = 1; i < R; ++i) v[i] = cmulc(v[i], twf(i));
     }
     dft_reg<R, INV>(v);
     constexpr int bits = ilog2c(R);
 #pragma unroll
     for (int k = 0; k < R; ++k) {
         float2 o = v[brev(k, bits)];
-        if (!INV && TW && k > 0) o = cmul(o, tw[(k * twstep) & (NTW - 1)]);
+        if (!INV && TW && k > 0) o = cmul(o, twf(k));
         *addr(k) = o;
     }
+}
+// twiddles from the table tw[j] = (cos, -sin)(2 pi j / NTW)
+template <int R, bool INV, bool TW, int NTW, class Addr>
+__device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw)
+{
+    fft_bfly<R, INV, TW>(addr, [&](int i) { return tw[(i * twstep) & (NTW - 1)]; });
 }
 
 __device__ __forceinline__ int padi(int i) { return i + (i >> 4); }  // 1 float2 of padding per 16
 
-// One pass (sub-FFT length L, radix R) of a length-N FFT held by one warp in a
-// padded scratch row.
-template <int N, int L, int R, bool INV, int NTW>
-__device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *tw, int lane)
+// Per-lane twiddles of the warp-level row FFT of length N: a lane handles the same butterflies of every row, so
+// its twiddles are loaded from the shared table once per phase and stay in registers (the inverse conjugates).
+template <int N, int NTW>
+struct RowTw {
+    static constexpr int R0 = cc_radix_row(N, 0), R1 = cc_radix_row(N, 1), R2 = cc_radix_row(N, 2);
+    static constexpr int NB0 = (N / R0 + 31) / 32;               // pass-0 butterflies per lane, b = g
+    static constexpr int L1 = N / R0, ST1 = L1 / R1;
+    static constexpr int NB1 = (N / R1 + 31) / 32;
+    static constexpr int S1 = ST1 <= 1 ? 0 : (ST1 <= 32 ? 1 : NB1);  // pass-1 twiddle sets (b = g % ST1 repeats when ST1 | 32)
+    float2 t0[NB0 * (R0 - 1)];
+    float2 t1[S1 > 0 ? S1 * (R1 - 1) : 1];
+    __device__ __forceinline__ void load(const float2 *tw, int lane)
+    {
+#pragma unroll
+        for (int n = 0; n < NB0; ++n) {
+            const int b = (lane + 32 * n) % (N / R0);
+#pragma unroll
+            for (int i = 1; i < R0; ++i) t0[n * (R0 - 1) + i - 1] = tw[(i * b * (NTW / N)) & (NTW - 1)];
+        }
+#pragma unroll
+        for (int n = 0; n < S1; ++n) {
+            const int b = (lane + 32 * n) % ST1;
+#pragma unroll
+            for (int i = 1; i < R1; ++i) t1[n * (R1 - 1) + i - 1] = tw[(i * b * (NTW / L1)) & (NTW - 1)];
+        }
+    }
+};
+
+// One pass (sub-FFT length L, radix R) of a length-N FFT held by one warp in a padded scratch row; rt = the
+// lane's twiddles (SETS sets of R-1), unused when the pass has none (L == R).
+template <int N, int L, int R, bool INV, int SETS>
+__device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int lane)
 {
-    constexpr int ST = L / R;
-    for (int g = lane; g < N / R; g += 32) {
-        const int blk = g / ST, b = g % ST;
-        const int base = blk * L + b;
-        fft_bfly<R, INV, (ST > 1), NTW>([&](int i) { return sc + padi(base + i * ST); }, b * (NTW / L), tw);
+    constexpr int ST = L / R, NB = (N / R + 31) / 32;
+#pragma unroll
+    for (int n = 0; n < NB; ++n) {
+        const int g = lane + 32 * n;
+        if (g < N / R) {
+            const int blk = g / ST, b = g % ST;
+            const int base = blk * L + b;
+            fft_bfly<R, INV, (ST > 1)>([&](int i) { return sc + padi(base + i * ST); },
+                                       [&](int i) { return rt[(SETS > 1 ? n : 0) * (R - 1) + i - 1]; });
+        }
     }
     __syncwarp();
 }
 
 template <int N, bool INV, int NTW>
-__device__ __forceinline__ void warp_fft(float2 *sc, const float2 *tw, int lane)
+__device__ __forceinline__ void warp_fft(float2 *sc, const RowTw<N, NTW> &rt, int lane)
 {
-    constexpr int R0 = cc_radix_row(N, 0), R1 = cc_radix_row(N, 1), R2 = cc_radix_row(N, 2);
+    using T = RowTw<N, NTW>;
+    constexpr int R0 = T::R0, R1 = T::R1, R2 = T::R2;
     if (!INV) {
-        warp_fft_pass<N, N, R0, false, NTW>(sc, tw, lane);
-        warp_fft_pass<N, N / R0, R1, false, NTW>(sc, tw, lane);
-        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, NTW>(sc, tw, lane);
+        warp_fft_pass<N, N, R0, false, T::NB0>(sc, rt.t0, lane);
+        warp_fft_pass<N, N / R0, R1, false, T::S1>(sc, rt.t1, lane);
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, 1>(sc, rt.t1, lane);
     } else {
-        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, NTW>(sc, tw, lane);
-        warp_fft_pass<N, N / R0, R1, true, NTW>(sc, tw, lane);
-        warp_fft_pass<N, N, R0, true, NTW>(sc, tw, lane);
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, 1>(sc, rt.t1, lane);
+        warp_fft_pass<N, N / R0, R1, true, T::S1>(sc, rt.t1, lane);
+        warp_fft_pass<N, N, R0, true, T::NB0>(sc, rt.t0, lane);
     }
 }
 
@@ -666,6 +706,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         {
             const PIX *fbase = reinterpret_cast<const PIX *>(frames) + (size_t)f * H * W + (size_t)rank * NR * W;
             if (tid == 0 && !RT && f != cid) issue_raw_head(frames, f);  // the first frame's rows were requested during the setup
+            RowTw<W, NTW> rtw;
+            rtw.load(tw, lane);
             const float c0f = (float)p.c0;
             for (int ck = 0; ck < C::NCHK; ++ck) {
                 const int rb = ck & 1;
@@ -677,7 +719,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     for (int x = lane; x < W; x += 32)
                         scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
                     __syncwarp();
-                    warp_fft<W, false, NTW>(scr, tw, lane);
+                    warp_fft<W, false, NTW>(scr, rtw, lane);
                     // untangle the two real rows and scatter to the column owners
                     const int ya = rank * NR + ck * C::RCH + jp, yb = ya + C::RCH / 2;
                     for (int k = lane; k < W / 2; k += 32) {
@@ -804,6 +846,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         int y0, x0;
         double cc_peak = 0.0;
         {
+            RowTw<W, NTW> rtw;
+            rtw.load(tw, lane);
             Best bst{-INFINITY, 0x7fffffff};
             for (int jp = warp; jp < NR / 2; jp += NWARP) {
                 const int ya = rank * NR + jp, yb = ya + NR / 2;
@@ -819,7 +863,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                 }
                 __syncwarp();
-                warp_fft<W, true, NTW>(scr, tw, lane);
+                warp_fft<W, true, NTW>(scr, rtw, lane);
                 for (int x = lane; x < W; x += 32) {
                     const float2 z = scr[padi(x)];
                     if (better(z.x, ya * W + x, bst.v, bst.i)) bst.v = z.x, bst.i = ya * W + x;
