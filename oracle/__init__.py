@@ -71,6 +71,9 @@ def _load():
         lib.cco_track.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                   ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float),
                                   ctypes.POINTER(_Result), ctypes.c_int]
+        lib.cco_track_sn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float),
+                                     ctypes.c_double, ctypes.POINTER(_Result), ctypes.c_int]
         lib.cco_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -186,9 +189,10 @@ def num_threads() -> int:
     return int(_load().cco_num_threads())
 
 
-def track(frames, reference, u: int, threads: int = 0) -> TrackResult:
+def track(frames, reference, u: int, threads: int = 0, method: str = "u", epsilon: float = 0.0) -> TrackResult:
     """The whole path O1-O7 for a batch of uint8/uint16 frames (B, H, W)
-    against a float32 reference (H, W)."""
+    against a float32 reference (H, W).  method "u": CC-U, Eq. (4); method "sn":
+    CC-SN, Eqs. (5)-(7) with offset epsilon (minimum of the weighted sum)."""
     frames = np.ascontiguousarray(frames)
     if frames.ndim == 2:
         frames = frames[None]
@@ -203,8 +207,14 @@ def track(frames, reference, u: int, threads: int = 0) -> TrackResult:
     if ref.shape != (H, W):
         raise ValueError("reference shape mismatch")
     out = (_Result * max(B, 1))()
-    rc = _load().cco_track(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
-                           ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), out, int(threads))
+    if method == "sn":
+        rc = _load().cco_track_sn(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                  ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(epsilon), out, int(threads))
+    elif method == "u":
+        rc = _load().cco_track(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                               ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), out, int(threads))
+    else:
+        raise ValueError("method must be 'u' or 'sn'")
     if rc:
         raise RuntimeError("oracle cco_track failed: %d" % rc)
     arr = np.frombuffer(out, dtype=np.dtype([

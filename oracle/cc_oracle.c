@@ -342,8 +342,19 @@ int cco_num_threads(void)
 #endif
 }
 
-int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
-              const float *reference, cco_result *out, int threads)
+/* The whole path for CC-U (sn == 0; Eq. (4)) and CC-SN (sn != 0;
+ * Eqs. (5)-(7)).  CC-SN: chi^2 of Eq. (6) is MINIMISED, and
+ * the only term that depends on the displacement is
+ *     S(s) = sum_r [I'(r+s)]^2 / E'(r),   I' = I + eps,  E' = E + eps
+ * (Eq. (7); E estimates the average image, so the offset added to the images
+ * is added to it too -- DESIGN.md R16).  The displacement is the position of
+ * the minimum of S (the sentence before Eq. (7) says "maximum"; Eq. (6) and
+ * Cauchy-Schwarz say minimum -- DESIGN.md R15).  argmin S = argmax (-S), so
+ * the weighted image pair (I'^2, -1/E') goes through exactly the steps of
+ * CC-U ("replacing I -> I'^2 and E -> 1/E") and `peak` is
+ * reported as the minimised sum S. */
+static int track_impl(const void *frames, int dtype, int batch, int H, int W, int u,
+                      const float *reference, int sn, double eps, cco_result *out, int threads)
 {
     if (!frames || !reference || !out || batch < 0 || H <= 0 || W <= 0 || u < 1 ||
         (dtype != 0 && dtype != 1))
@@ -354,6 +365,8 @@ int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
     if (!E) return -1;
     double *G_re = E + n, *G_im = E + 2 * n;
     for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    if (sn)
+        for (size_t i = 0; i < n; ++i) E[i] = -1.0 / (E[i] + eps);   /* -(1/E'), Eq. (7) */
     if (cco_dft2_real(E, H, W, G_re, G_im)) { free(E); return -1; }
 
     int fail = 0;
@@ -380,6 +393,8 @@ int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
             const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
             for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
         }
+        if (sn)                                                       /* I'^2, Eq. (7) */
+            for (size_t i = 0; i < n; ++i) I[i] = (I[i] + eps) * (I[i] + eps);
         int rc = cco_dft2_real(I, H, W, F_re, F_im);                 /* O2 */
         conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);          /* O3 */
         if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);         /* O4 */
@@ -401,6 +416,11 @@ int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
             r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
             r.peak = r.up_top1;
         }
+        if (sn) {   /* report S = -(-S): the minimised sum and its runner-up */
+            r.peak = -r.peak;
+            r.cc_top1 = -r.cc_top1; r.cc_top2 = -r.cc_top2;
+            r.up_top1 = -r.up_top1; r.up_top2 = -r.up_top2;
+        }
         out[b] = r;
         if (rc) {
             #pragma omp atomic write
@@ -410,4 +430,17 @@ int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
     }
     free(E);
     return fail ? -1 : 0;
+}
+
+int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
+              const float *reference, cco_result *out, int threads)
+{
+    return track_impl(frames, dtype, batch, H, W, u, reference, 0, 0.0, out, threads);
+}
+
+int cco_track_sn(const void *frames, int dtype, int batch, int H, int W, int u,
+                 const float *reference, double eps, cco_result *out, int threads)
+{
+    if (!(eps >= 0.0)) return -2;
+    return track_impl(frames, dtype, batch, H, W, u, reference, 1, eps, out, threads);
 }

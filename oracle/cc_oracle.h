@@ -97,6 +97,15 @@ typedef struct {
 int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
               const float *reference, cco_result *out, int threads);
 
+/* The same path for the shot-noise-weighted method CC-SN (PAPER.md:L72-84,
+ * Eqs. (5)-(7); L92 "replacing I -> I'^2 and E -> 1/E"): the displacement is
+ * the position of the MINIMUM of S(s) = sum_r (I(r+s)+eps)^2 / (E(r)+eps)
+ * (R15, R16), first on the integer lags, then on the upsampled
+ * grid; `peak`, cc_top1/2 and up_top1/2 are values of S (top1 = minimum,
+ * top2 = smallest value at any other index).  eps >= 0; E + eps must be > 0. */
+int cco_track_sn(const void *frames, int dtype, int batch, int H, int W, int u,
+                 const float *reference, double eps, cco_result *out, int threads);
+
 int cco_num_threads(void);
 
 #ifdef __cplusplus

@@ -351,3 +351,95 @@ def test_p11_shot_noise_sanity_band(oracle_mod):
     err = np.sqrt(np.mean((r.dy - s[:, 0]) ** 2 + (r.dx - s[:, 1]) ** 2) / 2)
     limit = 3.0 / np.sqrt(2 * np.pi * 9 * 1000)
     assert 0.5 * limit < err < 4.0 * limit
+
+
+# ---------------------------------------------------------------- CC-SN (Eqs. (5)-(7))
+# SN1  Cauchy-Schwarz closed form: frame = circshift(ref) -> d = shift, minimum value = sum(E + eps)
+# SN2  brute-force left-hand side of Eq. (7) on tiny frames: same integer minimiser, same minimum
+# SN3  chi^2 of Eq. (6) itself (all three terms) is minimised at the oracle's integer peak
+# SN4  large eps -> CC-SN results approach CC-U
+# SN5  common positive scaling of (I', E') leaves d unchanged; value scales linearly
+
+def _sn_direct(I, E, eps):
+    """S(s) = sum_r (I(r+s) + eps)^2 / (E(r) + eps), literal double loop over lags (Eq. (7), left side)."""
+    H, W = I.shape
+    Ip2 = (I + eps) ** 2
+    w = 1.0 / (E + eps)
+    S = np.empty((H, W))
+    for sy in range(H):
+        for sx in range(W):
+            S[sy, sx] = np.sum(np.roll(Ip2, (-sy, -sx), axis=(0, 1)) * w)
+    return S
+
+
+@pytest.mark.parametrize("H,W,u,eps", [(16, 16, 4, 7.5), (32, 64, 10, 0.0), (64, 64, 20, 200.0)])
+def test_sn1_circular_shift_closed_form(oracle_mod, H, W, u, eps):
+    rng = _rng(21)
+    ref = rng.integers(3, 900, size=(H, W)).astype(np.float32)
+    shifts = [(0, 0), (1, 0), (0, 1), (H // 2, W // 2), (H - 1, W - 1), (5, W - 7)]
+    fr = np.stack([np.roll(ref, s, axis=(0, 1)) for s in shifts]).astype(np.uint16)
+    o = oracle_mod.track(fr, ref, u, method="sn", epsilon=eps)
+    for k, (a, b) in enumerate(shifts):
+        wa = a - H if 2 * a >= H else a
+        wb = b - W if 2 * b >= W else b
+        assert (o.wy[k], o.wx[k]) == (wa, wb)
+        assert o.dy[k] == wa and o.dx[k] == wb           # (sum I')^2 <= S * sum E' with equality iff aligned
+    assert np.allclose(o.peak, np.sum(ref.astype(np.float64) + eps), rtol=1e-12)
+
+
+@pytest.mark.parametrize("shape,eps", [((8, 8), 3.0), ((12, 16), 50.0)])
+def test_sn2_brute_force_eq7(oracle_mod, shape, eps):
+    rng = _rng(22)
+    H, W = shape
+    ref = rng.integers(1, 300, size=shape).astype(np.float32)
+    fr = rng.integers(0, 300, size=(5,) + shape).astype(np.uint8)
+    o = oracle_mod.track(fr, ref, 1, method="sn", epsilon=eps)
+    for k in range(5):
+        S = _sn_direct(fr[k].astype(np.float64), ref.astype(np.float64), eps)
+        i = int(np.argmin(S))                              # first index among equal minima
+        y0, x0 = divmod(i, W)
+        assert (o.wy[k], o.wx[k]) == (y0 - H if 2 * y0 >= H else y0, x0 - W if 2 * x0 >= W else x0)
+        assert abs(o.peak[k] / S.min() - 1) < 1e-12
+        assert abs(o.cc_top2[k] / np.partition(S.ravel(), 1)[1] - 1) < 1e-12
+
+
+def test_sn3_minimises_chi2_of_eq6(oracle_mod):
+    """chi^2(s) = sum_r { E' - 2 I'(r+s) + I'(r+s)^2 / E' }: the oracle's integer peak is its minimiser."""
+    rng = _rng(23)
+    H, W, eps = 12, 12, 4.0
+    y, x = np.mgrid[0:H, 0:W]
+    ref = (100.0 * np.exp(-((y - 6) ** 2 + (x - 6) ** 2) / 6.0) + 5.0).astype(np.float32)
+    fr = rng.poisson(np.roll(ref.astype(np.float64), (2, -3), axis=(0, 1))).astype(np.uint16)[None]
+    o = oracle_mod.track(fr, ref, 1, method="sn", epsilon=eps)
+    Ep, Ip = ref.astype(np.float64) + eps, fr[0].astype(np.float64) + eps
+    chi2 = np.array([[np.sum(Ep - 2 * np.roll(Ip, (-sy, -sx), axis=(0, 1)) + np.roll(Ip, (-sy, -sx), axis=(0, 1)) ** 2 / Ep)
+                      for sx in range(W)] for sy in range(H)])
+    y0, x0 = divmod(int(np.argmin(chi2)), W)
+    assert (o.wy[0] % H, o.wx[0] % W) == (y0, x0) == (2, W - 3)
+
+
+def test_sn4_large_offset_approaches_ccu(oracle_mod):
+    """PAPER.md:L161: "for larger values [of eps] the CC-SN method's results approach those of the CC-U method"."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(24))
+    ref = wl.reference(cfg)
+    ou = oracle_mod.track(fr, ref, 20)
+    far = oracle_mod.track(fr, ref, 20, method="sn", epsilon=1e7)
+    near = oracle_mod.track(fr, ref, 20, method="sn", epsilon=1.0)
+    d_far = np.hypot(far.dx - ou.dx, far.dy - ou.dy)
+    d_near = np.hypot(near.dx - ou.dx, near.dy - ou.dy)
+    assert d_far.max() <= 0.05 + 1e-12 and np.mean(d_far == 0) >= 0.75    # at most one grid step away, mostly identical
+    assert d_near.mean() > d_far.mean()                                   # a small offset is a different estimator
+    truth = wl.shifts(cfg)[:24]
+    assert np.median(np.hypot(near.dx - truth[:, 1], near.dy - truth[:, 0])) < 0.2   # and still tracks the spot
+
+
+def test_sn5_scaling_invariance(oracle_mod):
+    rng = _rng(25)
+    ref = rng.integers(10, 120, size=(32, 32)).astype(np.float32)
+    fr = np.clip(rng.poisson(np.roll(ref.astype(np.float64), (3, 5), axis=(0, 1)), size=(4, 32, 32)), 0, 120).astype(np.uint16)
+    a = oracle_mod.track(fr, ref, 10, method="sn", epsilon=6.0)
+    b = oracle_mod.track((2 * fr).astype(np.uint16), 2 * ref, 10, method="sn", epsilon=12.0)   # I', E' both doubled
+    assert np.array_equal(a.dx, b.dx) and np.array_equal(a.dy, b.dy)
+    assert np.allclose(b.peak, 2 * a.peak, rtol=1e-12)
