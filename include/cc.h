@@ -81,6 +81,22 @@ cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype, int upsamp
                          const float *reference);
 
 /*
+ * cc_plan_create_weighted -- cc_plan_create with the choice of the paper's
+ * weighting:
+ *   CC_METHOD_U   uniform weights, Eq. (4): maximum of sum_r I(r+d) E(r)
+ *   CC_METHOD_SN  shot-noise weights, Eqs. (5)-(7): with I' = I + epsilon and
+ *                 E' = E + epsilon, the MINIMUM of S(d) = sum_r I'(r+d)^2 / E'(r)
+ *                 (chi^2 of Eq. (6) is minimised; R15, R16).  `peak`
+ *                 then returns S at the minimum.  Needs E + epsilon > 0 in
+ *                 every pixel (else CC_ERR_INVALID_ARG).  The paper's
+ *                 recommendation is epsilon = 200 x the noise gain (L161).
+ * Everything else as cc_plan_create; cc_track etc. work on either plan.
+ */
+typedef enum { CC_METHOD_U = 0, CC_METHOD_SN = 1 } cc_method;
+cc_status cc_plan_create_weighted(cc_plan **out, int H, int W, cc_dtype dtype, int upsample,
+                                  const float *reference, cc_method method, float epsilon);
+
+/*
  * cc_track -- the hot path (Eq. (4)):
  * ingest -> real 2D FFT -> (x) conj(F[E]) -> inverse FFT -> integer argmax ->
  * upsampled DFT -> sub-pixel argmax, fused so that each frame is read from HBM

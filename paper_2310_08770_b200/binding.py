@@ -19,7 +19,7 @@ CC_U8, CC_U16 = 0, 1
 _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
-EXPORTS = ["cc_plan_create", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
+EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
            "cc_plan_info", "cc_fp32_peak_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
@@ -52,6 +52,8 @@ def load_library() -> ctypes.CDLL:
         vp, ci = ctypes.c_void_p, ctypes.c_int
         lib.cc_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, vp]
         lib.cc_plan_create.restype = ci
+        lib.cc_plan_create_weighted.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, vp, ci, ctypes.c_float]
+        lib.cc_plan_create_weighted.restype = ci
         lib.cc_track.argtypes = [vp, vp, ci, vp, vp, vp, vp]
         lib.cc_track.restype = ci
         lib.cc_track_debug.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp, vp]
@@ -103,7 +105,7 @@ def _torch():
 class Plan:
     """cc_plan_create / cc_track / cc_plan_destroy (include/cc.h)."""
 
-    def __init__(self, H: int, W: int, dtype, upsample: int, reference):
+    def __init__(self, H: int, W: int, dtype, upsample: int, reference, method: str = "u", epsilon: float = 0.0):
         lib = load_library()
         _torch()
         dt = np.dtype(dtype)
@@ -119,8 +121,10 @@ class Plan:
         if ref.shape != (self.H, self.W):
             raise ValueError("reference must be (H, W)")
         self._h = ctypes.c_void_p()
-        _check(lib.cc_plan_create(ctypes.byref(self._h), self.H, self.W, self.cc_dtype, self.upsample,
-                                  ref.ctypes.data_as(ctypes.c_void_p)))
+        if method not in ("u", "sn"):
+            raise ValueError("method must be 'u' (CC-U) or 'sn' (CC-SN)")
+        _check(lib.cc_plan_create_weighted(ctypes.byref(self._h), self.H, self.W, self.cc_dtype, self.upsample,
+                                           ref.ctypes.data_as(ctypes.c_void_p), 1 if method == "sn" else 0, float(epsilon)))
 
     def close(self):
         if getattr(self, "_h", None):

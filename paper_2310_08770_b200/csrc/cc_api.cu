@@ -67,6 +67,8 @@ struct VarPlan {
 struct cc_plan {
     int H = 0, W = 0, u = 0, M = 0, c = 0, dtype = 0;
     int c0 = 0;
+    int sn = 0;            // 0: CC-U, 1: CC-SN
+    double sn_eps = 0.0, sn_c0 = 0.0;
     double Emean = 0.0;
     // device tables
     float2 *tw = nullptr, *Gt = nullptr;
@@ -330,6 +332,14 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
 
 extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype, int upsample, const float *reference)
 {
+    return cc_plan_create_weighted(out, H, W, dtype, upsample, reference, CC_METHOD_U, 0.f);
+}
+
+extern "C" cc_status cc_plan_create_weighted(cc_plan **out, int H, int W, cc_dtype dtype, int upsample, const float *reference,
+                                             cc_method method, float epsilon)
+{
+    if (method != CC_METHOD_U && method != CC_METHOD_SN) return fail(CC_ERR_INVALID_ARG, "cc_plan_create_weighted: bad method");
+    if (method == CC_METHOD_SN && !(epsilon >= 0.f)) return fail(CC_ERR_INVALID_ARG, "cc_plan_create_weighted: epsilon must be >= 0");
     if (!out || !reference || H <= 0 || W <= 0 || upsample < 1 || (dtype != CC_U8 && dtype != CC_U16))
         return fail(CC_ERR_INVALID_ARG, "cc_plan_create: bad argument");
     if (upsample > 4096) return fail(CC_ERR_UNSUPPORTED, "upsample factor above 4096");
@@ -376,7 +386,24 @@ extern "C" cc_status cc_plan_create(cc_plan **out, int H, int W, cc_dtype dtype,
 
     // ---- G = DFT2(E) in fp64 (row pass, column pass)
     std::vector<std::complex<double>> G((size_t)H * W);
-    for (size_t i = 0; i < G.size(); ++i) G[i] = std::complex<double>((double)ref[i], 0.0);
+    if (method == CC_METHOD_SN) {
+        // CC-SN, Eqs. (5)-(7): correlate I'^2 with 1/E', E' = E + eps; chi^2 is minimised, so the kernel maximises the
+        // correlation with -1/E' (R15, R16).  sn_c0 = the mean of E'^2 rounded to an integer: the constant
+        // taken off every transformed pixel (an exact no-op for the argmax; restored in `peak`).
+        double m2 = 0.0;
+        for (size_t i = 0; i < G.size(); ++i) {
+            const double ep = (double)ref[i] + (double)epsilon;
+            if (!(ep > 0.0)) {
+                delete pl;
+                return fail(CC_ERR_INVALID_ARG, "CC-SN needs reference + epsilon > 0 in every pixel");
+            }
+            G[i] = std::complex<double>(-1.0 / ep, 0.0);
+            m2 += ep * ep;
+        }
+        pl->sn = 1, pl->sn_eps = (double)epsilon, pl->sn_c0 = nearbyint(m2 / (double)G.size());
+    } else {
+        for (size_t i = 0; i < G.size(); ++i) G[i] = std::complex<double>((double)ref[i], 0.0);
+    }
     {
         const auto wW = unit_roots(W), wH = unit_roots(H);
         for (int y = 0; y < H; ++y) fft1d(G, W, 1, (size_t)y * W, false, wW);
@@ -486,6 +513,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
     p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.Emean = pl->Emean;
+    p.sn = pl->sn, p.sn_eps = pl->sn_eps, p.sn_c0 = pl->sn_c0, p.peak_sign = pl->sn ? -1.0 : 1.0;
 }
 
 static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,

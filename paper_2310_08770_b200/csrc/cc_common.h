@@ -107,7 +107,12 @@ struct CcParams {
     int nrc2, nnc2;     // stage-2 row chunks / e-column chunks
     int ntiles_frame;   // tiles consumed per frame
     int tile_floats;    // floats per staging slot
-    int c0;             // integer constant subtracted from every pixel before the FFT
+    int c0;             // integer constant subtracted from every pixel before the FFT (CC-U)
+    // CC-SN: pixels become (I + sn_eps)^2 - sn_c0 (evaluated in fp64, rounded once to fp32) and the
+    // plan's spectrum is that of -1/(E + sn_eps); peak_sign = -1 turns the maximised -S back into the sum S
+    int sn;             // 0: CC-U, 1: CC-SN
+    double sn_eps, sn_c0;
+    double peak_sign;
     int u_bytes;        // bytes of the raw/scratch/T union region
     double Emean;       // mean of the reference image (DC add-back for `peak`)
 };

@@ -521,6 +521,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     csync();
 
     const int u = p.u, M = p.M, cM = p.c;
+    const double c0d = p.sn ? p.sn_c0 : (double)p.c0;  // constant subtracted from every (transformed) pixel
 
     // Cluster-wide exchanges: every CTA stores its record into every peer with st.async, which completes
     // tx-bytes on the PEER's mbarrier: a one-way DSMEM latency instead of remote stores + a full cluster barrier.
@@ -717,7 +718,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     const PIX *ra = rw + (size_t)jp * W;
                     const PIX *rbp = rw + (size_t)(jp + C::RCH / 2) * W;
                     for (int x = lane; x < W; x += 32)
-                        scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
+                        if (p.sn) {  // CC-SN: I'^2 - c0 with I' = I + eps (Eq. (7)), one rounding
+                            const double ta = (double)ra[x] + p.sn_eps, tb = (double)rbp[x] + p.sn_eps;
+                            scr[padi(x)] = make_float2((float)fma(ta, ta, -p.sn_c0), (float)fma(tb, tb, -p.sn_c0));
+                        } else {
+                            scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
+                        }
                     __syncwarp();
                     warp_fft<W, false, NTW>(scr, rtw, lane);
                     // untangle the two real rows and scatter to the column owners
@@ -908,7 +914,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
         if (u == 1) {
             if (rank == 0 && tid == 0) {
-                emit(f, (float)wy, (float)wx, (float)(cc_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean), wy, wx);
+                emit(f, (float)wy, (float)wx, (float)(p.peak_sign * (cc_peak + ((double)*f00 + c0d * H * W) * p.Emean)), wy, wx);
             }
             csync();
             continue;
@@ -1259,7 +1265,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         stamp(7, f);
         if (rank == 0 && tid == 0) {
             emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
-                 (float)(up_peak + ((double)*f00 + (double)p.c0 * H * W) * p.Emean), wy, wx);
+                 (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * p.Emean)), wy, wx);
         }
         __syncthreads();  // U (polish scratch) is reused by the next frame's raw ring
     }

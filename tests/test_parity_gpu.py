@@ -38,9 +38,19 @@ def _run(pkg, frames, ref, u, debug=True):
     return res
 
 
-def _compare(o, dx, dy, pk, iy, ix, label):
+def _compare(o, dx, dy, pk, iy, ix, label, near_tie=0.0, u=None):
+    """near_tie > 0 (stress cases only, never the BASELINE configs): a sub-pixel mismatch is tolerated when the
+    ORACLE's own top-1/top-2 margin is below `near_tie` relative (a tie at float32 resolution of the inputs'
+    spectrum) and the GPU's point is one grid step away; every such frame is still counted and printed."""
     bad_i = np.nonzero((iy != o.wy) | (ix != o.wx))[0]
     bad_s = np.nonzero((np.abs(dx - o.dx) > TOL_PX) | (np.abs(dy - o.dy) > TOL_PX))[0]
+    if near_tie > 0.0 and len(bad_s):
+        marg = np.abs(o.up_top1 - o.up_top2) / np.maximum(np.abs(o.up_top1), 1e-300)
+        step = np.maximum(np.abs(dx - o.dx), np.abs(dy - o.dy))
+        ok = (marg[bad_s] < near_tie) & (step[bad_s] <= 1.0 / u + 1e-6)
+        if ok.any():
+            print("%s: %d near-tie frame(s) tolerated (oracle margin < %.0e): %s" % (label, int(ok.sum()), near_tie, bad_s[ok]))
+        bad_s = bad_s[~ok]
     msg = []
     for i in list(bad_i[:8]) + list(bad_s[:8]):
         margin = (o.up_top1[i] - o.up_top2[i]) / max(abs(o.up_top1[i]), 1e-300)
@@ -280,3 +290,51 @@ def test_realtime_session_restarts_after_idle_timeout(gpu):
     torch.cuda.synchronize()                 # returns at once: nothing resident any more
     assert (a[0], a[1]) == (bx[0], by[0]) and (b[0], b[1]) == (bx[1], by[1])
     plan.close()
+
+
+# ---------------------------------------------------------------- CC-SN: cc_plan_create_weighted
+@pytest.mark.parametrize("ci,n,eps", [(1, 400, 200.0), (2, 300, 40.0), (3, 120, 200.0), (4, 24, 200.0), (5, 8, 200.0), (1, 64, 0.5)])
+def test_ccsn_parity_subset(gpu, oracle_mod, ci, n, eps):
+    """Shot-noise-weighted method: same bar as CC-U (exact integer peaks, the oracle's grid point, peak to 1e-4)."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    idx = wl.oracle_subset(cfg)[:n]
+    fr = wl.frames(cfg, idx)
+    ref = wl.reference(cfg)
+    o = oracle_mod.track(fr, ref, cfg.upsample, method="sn", epsilon=eps)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref, method="sn", epsilon=eps)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr), debug=True)]
+    torch.cuda.synchronize()
+    plan.close()
+    # eps = 0.5 is a stress case far from the paper's recommendation (L161): weights 1/E' span two decades
+    _compare(o, dx, dy, pk, iy, ix, "%s CC-SN eps=%g" % (cfg.name, eps), near_tie=1e-7 if eps < 1 else 0.0, u=cfg.upsample)
+
+
+def test_ccsn_circular_shift_closed_form_and_full_range(gpu, oracle_mod):
+    """frame = circshift(ref): d = shift exactly and S = sum(E + eps) (Cauchy-Schwarz); full-range u16 pixels
+    ((65535 + eps)^2 ~ 4.3e9 exceeds fp32's integer range: the transformed pixel is rounded once)."""
+    rng = np.random.default_rng(31)
+    H = W = 128
+    eps = 200.0
+    ref = rng.integers(0, 65536, size=(H, W)).astype(np.uint16)
+    shifts = [(0, 0), (1, 0), (0, 1), (H // 2, W // 2), (H - 1, W - 1), (7, W - 9)]
+    fr = np.stack([np.roll(ref, s, axis=(0, 1)) for s in shifts])
+    plan = gpu.Plan(H, W, fr.dtype, 10, ref.astype(np.float32), method="sn", epsilon=eps)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr), debug=True)]
+    plan.close()
+    for k, (a, b) in enumerate(shifts):
+        assert (dy[k], dx[k]) == (float(a - H if 2 * a >= H else a), float(b - W if 2 * b >= W else b))
+    assert np.max(np.abs(pk / np.sum(ref.astype(np.float64) + eps) - 1)) < 1e-5
+    o = oracle_mod.track(fr, ref.astype(np.float32), 10, method="sn", epsilon=eps)
+    _compare(o, dx, dy, pk, iy, ix, "CC-SN circular shifts")
+
+
+def test_ccsn_argument_errors(gpu):
+    lib = gpu.load_library()
+    h = ctypes.c_void_p()
+    ref = np.zeros((64, 64), np.float32)                      # E + eps = 0 somewhere -> rejected
+    rp = ref.ctypes.data_as(ctypes.c_void_p)
+    assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 1, ctypes.c_float(0.0)) == 1
+    assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 1, ctypes.c_float(-1.0)) == 1
+    assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 7, ctypes.c_float(1.0)) == 1
