@@ -45,10 +45,12 @@ def flops_per_frame(H, W, u):
 
 
 def executed_flops_per_frame(H, W, u):
-    """Flops of the formulation the kernel executes (real Dirichlet stage 1: 4*M*H*W/2... see DESIGN.md)."""
+    """Flops of the formulation the kernel executes: real Dirichlet stage 1 on Q with
+    even/odd halves (2 x nd x (H/2+1) x W multiply-adds), stage 2 as E/O pairs (M x nd x W multiply-adds)."""
     M = (3 * u + 1) // 2
+    nd = M // 2 + 1
     fft = 5.0 * H * W * np.log2(H * W)
-    return fft + 6.0 * H * (W // 2) + 2.0 * M * H * W + 2.0 * M * M * W
+    return fft + 6.0 * H * (W // 2) + 2.0 * (2.0 * nd * (H // 2 + 1) * W) + 2.0 * (M * nd * W)
 
 
 class ClockSampler:
@@ -113,6 +115,35 @@ def oracle_rate(cfg, n_frames: int):
     return len(idx) / dt, oracle.num_threads(), len(idx), dt
 
 
+PHASES = ["ingest + row FFT", "column FFT x conj(G) + column inverse", "row C2R + integer argmax", "fp64 integer polish",
+          "upsampled stage 1", "upsampled stage 2", "sub-pixel argmax reduction", "fp64 sub-pixel polish"]
+
+
+def run_phases():
+    """--phases: per-phase SM-clock cycles per frame (cc_track_profile, median over frames) of every config,
+    batched configs in steady state and the streaming configs at batch 1."""
+    import torch
+    from paper_2310_08770_b200 import Plan
+    for ci, B in ((1, 1000), (2, 1), (3, 2960), (4, 1), (5, 30)):
+        cfg = wl.config(ci)
+        fr = wl.frames(cfg, np.arange(min(B, 64)))
+        if B > len(fr):
+            fr = np.concatenate([fr] * ((B + len(fr) - 1) // len(fr)))[:B]
+        plan = Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, wl.reference(cfg))
+        d = plan.device_frames(fr)
+        for _ in range(3):
+            out = plan.track_profile(d, B)
+        torch.cuda.synchronize()
+        med = np.median(out[3].cpu().numpy().astype(np.float64), axis=0)
+        info = plan.info()
+        cs = info["lat_cluster_size"] if (B <= info["lat_max_clusters"] and info["lat_cluster_size"]) else info["cluster_size"]
+        print("%s  batch %d  cluster size %d" % (cfg.name, B, cs))
+        for nm, v in zip(PHASES, med):
+            print("   %-40s %9.0f cycles %5.1f %%" % (nm, v, 100 * v / med.sum()))
+        print("   %-40s %9.0f cycles = %.1f us at 1965 MHz" % ("total per frame", med.sum(), med.sum() / 1965.0))
+        plan.close()
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -157,9 +188,13 @@ def main():
     ap.add_argument("--no-latency", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--phases", action="store_true", help="print the per-phase cycle breakdown of every config and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
+    if args.phases:
+        run_phases()
+        return
     cfg = wl.config(3)
     if args.impl == "reference":
         run_reference(args, cfg)
