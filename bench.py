@@ -144,6 +144,68 @@ def run_phases():
         plan.close()
 
 
+def run_table(args):
+    """--table: one JSON line per config for BASELINE.md section 3 -- batched configs: frames/s over the whole batch
+    (CUDA events, 3 warm-up + 5 timed calls) and roofline fractions; streaming configs: single-frame latency; every
+    config: the oracle's frames/s on a bounded sample."""
+    import torch
+    from paper_2310_08770_b200 import Plan, RtSession
+    import oracle
+    peak_tf = 148 * FP32_LANES_PER_SM * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
+    osample = {1: 1000, 2: 1000, 3: 256, 4: 64, 5: 32}
+    for ci in (1, 2, 3, 4, 5):
+        cfg = wl.config(ci)
+        row = {"cfg": ci, "workload": cfg.name}
+        ref = wl.reference(cfg)
+        if cfg.mode == "batched":
+            fr = wl.frames(cfg)
+            B = len(fr)
+            plan = Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+            d = plan.device_frames(fr)
+            out = tuple(torch.empty(B, dtype=torch.float32, device="cuda") for _ in range(3))
+            for _ in range(3):
+                plan.track(d, B, out=out)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+            for a, b in ev:
+                a.record()
+                plan.track(d, B, out=out)
+                b.record()
+            torch.cuda.synchronize()
+            ms = float(np.median([a.elapsed_time(b) for a, b in ev]))
+            fps = B / (ms * 1e-3)
+            row.update({"frames_per_s": fps, "ms_per_batch": ms, "batch": B,
+                        "roofline_frac_algorithmic": flops_per_frame(cfg.H, cfg.W, cfg.upsample) * fps / (peak_tf * 1e12),
+                        "roofline_frac_executed": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * fps / (peak_tf * 1e12),
+                        "input": "%.2f GB per call%s" % (fr.nbytes / 1e9, "" if fr.nbytes > 2e8 else " (fits L2; ALU-bound either way)")})
+            plan.close()
+            del d, fr
+        else:
+            n = min(2000, cfg.n_frames)
+            fr = wl.frames(cfg, np.arange(n))
+            plan = Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+            d = plan.device_frames(fr)
+            plan.latency_probe(d, 100)
+            l0 = plan.latency_probe(d, n)[3]
+            torch.cuda.current_stream().synchronize()
+            rt = RtSession(plan, 1000)
+            try:
+                rt.latency_probe(d.data_ptr(), 100)
+                l1 = rt.latency_probe(d.data_ptr(), n)[3]
+            finally:
+                rt.close()
+            row.update({"latency_us_cc_track_sync_median_p99": [float(np.median(l0)), float(np.percentile(l0, 99))],
+                        "latency_us_rt_session_median_p99": [float(np.median(l1)), float(np.percentile(l1, 99))], "calls": n})
+            plan.close()
+        idx = wl.oracle_subset(cfg)[: osample[ci]]
+        fo = wl.frames(cfg, idx)
+        oracle.track(fo[:1], ref, cfg.upsample)
+        t0 = time.perf_counter()
+        oracle.track(fo, ref, cfg.upsample)
+        dt = time.perf_counter() - t0
+        row.update({"oracle_frames_per_s": len(idx) / dt, "oracle_cores": oracle.num_threads(), "oracle_sample": len(idx)})
+        print(json.dumps(row), flush=True)
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -188,12 +250,16 @@ def main():
     ap.add_argument("--no-latency", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--table", action="store_true", help="per-config numbers for BASELINE.md section 3 and exit")
     ap.add_argument("--phases", action="store_true", help="print the per-phase cycle breakdown of every config and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
     if args.phases:
         run_phases()
+        return
+    if args.table:
+        run_table(args)
         return
     cfg = wl.config(3)
     if args.impl == "reference":
@@ -299,7 +365,7 @@ def main():
     t_hbm = (frames[0].nbytes + 12) / (hbm_gbs * 1e9)
     roofline = {
         "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": None, "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
+        "traffic": 1.317e9, "traffic_source": "ncu --set full capture profiles/r1c_summary.md: dram read 1.3123 GB + write 4.6 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
         "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
         "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,
