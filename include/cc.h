@@ -64,6 +64,8 @@ typedef struct {
     int lat_max_clusters;
     long long scratch_bytes;  /* plan-owned device scratch used by cc_track (0: stream-concurrent)  */
     long long table_bytes;    /* plan-owned constant tables (reference spectrum, upsampling tables) */
+    int super_blocks;         /* passes of the upsampled DFT over the offsets d (T buffer capacity), throughput variant */
+    int offsets_per_cta;      /* offsets d per CTA per pass                                                             */
 } cc_plan_info_t;
 
 /*

@@ -35,7 +35,8 @@ class PlanInfo(ctypes.Structure):
                 ("grid_M", ctypes.c_int), ("cluster_size", ctypes.c_int), ("threads", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("max_clusters", ctypes.c_int),
                 ("lat_cluster_size", ctypes.c_int), ("lat_max_clusters", ctypes.c_int),
-                ("scratch_bytes", ctypes.c_longlong), ("table_bytes", ctypes.c_longlong)]
+                ("scratch_bytes", ctypes.c_longlong), ("table_bytes", ctypes.c_longlong),
+                ("super_blocks", ctypes.c_int), ("offsets_per_cta", ctypes.c_int)]
 
 
 _lib = None
