@@ -300,8 +300,7 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
           int R2_, int KS2_, int NSTG_, int PFD_, int KS1_>
 struct Cfg {
     static constexpr int NSTG = NSTG_;  // staging ring depth
-    static constexpr int PFD = PFD_;    // prefetch distance (tiles) of the ring producer; NSTG - PFD >= 2 keeps it from blocking
-    static constexpr int NBARS = 2 * NSTG + 5;  // full[NSTG], empty[NSTG], raw ring [2], cluster exchange [2], rt command [1]
+    static constexpr int NBARS = NSTG + 5;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -345,7 +344,7 @@ struct Cfg {
     static constexpr int RED_FLOATS = RED1_FLOATS > RED2_FLOATS ? RED1_FLOATS : RED2_FLOATS;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
-    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64 + 16;
+    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64 + 16 + 4 * NSTG;
     static constexpr size_t FIXED_BYTES =
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
@@ -357,7 +356,7 @@ struct Cfg {
     static_assert(WG2R * WG2C * KS2 == NWARP && (TN2 == 4 || TN2 == 5) && G2 % KS2 == 0 && W % (4 * G2) == 0, "bad stage-2 tiling");
     static_assert(TILEF % 4 == 0 && MC1 % 4 == 0, "tile alignment");
     static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
-    static_assert(NSTG - PFD >= 2 && PFD <= 8, "ring (sched_head carries 8 entries)");
+    static_assert(NSTG <= 8, "ring (sched_head carries 8 entries)");
 };
 
 template <class C>
@@ -367,7 +366,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     constexpr int NWARP = C::NWARP, NTW = C::NTW, PADW = C::PADW;
     constexpr int LDT = C::LDT;
     constexpr bool SG = C::SG;
-    constexpr int NSTG = C::NSTG, PFD = C::PFD, NBARS = C::NBARS;
+    constexpr int NSTG = C::NSTG, NBARS = C::NBARS;
     using PIX = typename C::PIX;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -385,13 +384,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     unsigned char *misc = reinterpret_cast<unsigned char *>(rslot + W);
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
-    uint64_t *const bfull = bars, *const bempty = bars + NSTG, *const braw = bars + 2 * NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
+    uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
     float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
     uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
+    uint32_t *const relcnt = reinterpret_cast<uint32_t *>(cmdslot + 2);  // [NSTG] releases of each ring slot (mod NWARP)
 
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
@@ -426,63 +426,56 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     };
 
     // ---- operand ring: every frame consumes the same p.ntiles_frame tiles of p.blob in the order of
-    // p.sched.  Thread 0 keeps PFD tiles in flight (also across frames and phases); a slot is refilled
-    // once all NWARP warps have released it (empty mbarrier) -- no CTA barrier inside the GEMM loops.
+    // p.sched; the NSTG slots always hold the next NSTG tiles (landed or in flight), also across frames and
+    // phases.  A slot is refilled, with the tile NSTG positions ahead, by whichever warp is the LAST to release
+    // it (shared-memory release counter): the copy is issued at the first moment the slot is free, whatever the
+    // relative progress of the warps -- no dedicated producer, no CTA barrier inside the GEMM loops.
     const uint32_t my_frames = p.batch > cid ? (uint32_t)((p.batch - cid + ncl - 1) / ncl) : 0u;
     // real-time session: frames arrive one by one for as long as the session lives; the ring runs ahead freely
     const uint32_t total_tiles = p.rt_cmd ? (p.ntiles_frame ? 0xffffffffu : 0u) : my_frames * (uint32_t)p.ntiles_frame;
-    uint32_t g_load = 0, s_idx = 0;            // tiles requested so far (saturating in a session), schedule position
-    uint32_t l_slot = 0, l_par = 0;            // producer: next ring slot and the parity of its empty barrier
-    uint32_t c_slot = 0, c_par = 0;            // consumer: current ring slot and the parity of its full barrier
-    uint32_t next_ti = 0u;  // schedule entry of the next tile, fetched one tile ahead (thread 0)
-    auto ring_produce = [&]() {  // thread 0 only
-        mbar_wait(&bempty[l_slot], l_par ^ 1u);
-        const uint32_t ti = next_ti;
-        mbar_expect_tx(&bfull[l_slot], (uint32_t)C::TILEF * 4u);
-        bulk_g2s(stg + (size_t)l_slot * C::TILEF, p.blob + (size_t)ti * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[l_slot]);
-        if (g_load != 0xffffffffu) ++g_load;
-        if (++l_slot == NSTG) l_slot = 0, l_par ^= 1u;
-        if (++s_idx == (uint32_t)p.ntiles_frame) s_idx = 0;
-        next_ti = __ldg(&p.sched[s_idx]);  // latency overlaps the tile's compute
-    };
+    uint32_t g_cons = 0;                       // tiles consumed so far (saturating in a session)
+    uint32_t c_slot = 0, c_par = 0;            // current ring slot and the parity of its full barrier
+    uint32_t r_idx = (uint32_t)(p.ntiles_frame > 0 ? NSTG % p.ntiles_frame : 0);  // schedule position of tile g_cons + NSTG
+    uint32_t refill_ti = 0u;                   // its blob index, fetched at acquire time (lane 0)
     auto ring_acquire = [&]() -> const float * {
-        if (tid == 0 && (g_load < total_tiles || total_tiles == 0xffffffffu)) ring_produce();
+        if (lane == 0) refill_ti = __ldg(&p.sched[r_idx]);  // latency overlaps the tile's compute
         mbar_wait(&bfull[c_slot], c_par);
         return stg + (size_t)c_slot * C::TILEF;
     };
     auto ring_release = [&]() {
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bempty[c_slot]);
+        if (lane == 0) {
+            __threadfence_block();  // this warp's reads of the slot are done before the count says so
+            const uint32_t old = atomicAdd(&relcnt[c_slot], 1u);
+            if ((old + 1u) % (uint32_t)NWARP == 0u && (total_tiles == 0xffffffffu || g_cons + (uint32_t)NSTG < total_tiles)) {
+                fence_proxy_async();  // generic-proxy reads of the slot before the async-proxy write
+                mbar_expect_tx(&bfull[c_slot], (uint32_t)C::TILEF * 4u);
+                bulk_g2s(stg + (size_t)c_slot * C::TILEF, p.blob + (size_t)refill_ti * C::TILEF, (uint32_t)C::TILEF * 4u,
+                         &bfull[c_slot]);
+            }
+        }
+        if (g_cons != 0xffffffffu) ++g_cons;
         if (++c_slot == NSTG) c_slot = 0, c_par ^= 1u;
+        if (++r_idx == (uint32_t)p.ntiles_frame) r_idx = 0;
     };
 
-    // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts the first PFD operand tiles and
+    // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts the first NSTG operand tiles and
     // the first frame's raw rows in flight; the table copies of all threads overlap those copies; one cluster
     // barrier ends the setup.
     if (tid == 0) {
-        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), mbar_init(&bempty[i], NWARP);
+        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), relcnt[i] = 0u;
         mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
         mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1), mbar_init(cbar, 1);
         fence_mbar_init();
-        if (total_tiles > 0) {
-            uint32_t first[PFD];  // the first schedule entries ride in the kernel parameters: no load latency
-            uint32_t si = 0;
-#pragma unroll
-            for (int i = 0; i < PFD; ++i) {
-                first[i] = p.sched_head[i];
-                if (++si == (uint32_t)p.ntiles_frame) si = 0;
-            }
-            next_ti = __ldg(&p.sched[si]);
+        if (total_tiles > 0) {  // fill the ring; the first schedule entries ride in the kernel parameters: no load latency
             fence_proxy_async();
 #pragma unroll
-            for (int i = 0; i < PFD; ++i)
-                if (g_load < total_tiles) {
+            for (int i = 0; i < NSTG; ++i)
+                if ((uint32_t)i < total_tiles) {
                     mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
-                    bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)first[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
-                    ++g_load;
-                    ++l_slot;  // PFD < NSTG: no wrap during the burst
+                    bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)p.sched_head[i] * C::TILEF, (uint32_t)C::TILEF * 4u,
+                             &bfull[i]);
                 }
-            s_idx = si;  // == g_load % ntiles_frame whenever the burst was not cut short (otherwise unused)
         }
         if (!p.rt_cmd && cid < p.batch) issue_raw_head(p.frames, cid);
     }
@@ -508,7 +501,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         for (int e = 0; e < NI_W; ++e)
             if (tid + e * NT < W) rslot[tid + e * NT] = r_rs[e];
         if constexpr (C::LAT) {
-            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(cmdslot + 2) + 15) & ~(uintptr_t)15);
+            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(relcnt + NSTG) + 15) & ~(uintptr_t)15);
 #pragma unroll
             for (int e = 0; e < NI_W; ++e)
                 if (tid + e * NT < W) t64[tid + e * NT] = r_64[e];
@@ -1268,6 +1261,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                  (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * p.Emean)), wy, wx);
         }
         __syncthreads();  // U (polish scratch) is reused by the next frame's raw ring
+    }
+    if (RT && total_tiles > 0) {  // the ring ran ahead: let the outstanding operand copies land before the CTA leaves
+        for (int i = 0; i < NSTG; ++i) {
+            mbar_wait(&bfull[c_slot], c_par);
+            if (++c_slot == NSTG) c_slot = 0, c_par ^= 1u;
+        }
     }
     csync();  // no CTA of the cluster exits while peers may still address its shared memory
     if (RT && rank == 0 && tid == 0) {
