@@ -196,38 +196,41 @@ __device__ __forceinline__ int padi(int i) { return i + (i >> 4); }  // 1 float2
 template <int N, int NTW>
 struct RowTw {
     static constexpr int R0 = cc_radix_row(N, 0), R1 = cc_radix_row(N, 1), R2 = cc_radix_row(N, 2);
-    static constexpr int NB0 = (N / R0 + 31) / 32;               // pass-0 butterflies per lane, b = g
+    static constexpr int LP = 32 / cc_row_group(N);              // lanes that share one row pair
+    static constexpr int NB0 = (N / R0 + LP - 1) / LP;           // pass-0 butterflies per lane, b = g
     static constexpr int L1 = N / R0, ST1 = L1 / R1;
-    static constexpr int NB1 = (N / R1 + 31) / 32;
-    static constexpr int S1 = ST1 <= 1 ? 0 : (ST1 <= 32 ? 1 : NB1);  // pass-1 twiddle sets (b = g % ST1 repeats when ST1 | 32)
+    static constexpr int NB1 = (N / R1 + LP - 1) / LP;
+    static constexpr int S1 = ST1 <= 1 ? 0 : (ST1 <= LP ? 1 : NB1);  // pass-1 twiddle sets (b = g % ST1 repeats when ST1 | LP)
     float2 t0[NB0 * (R0 - 1)];
     float2 t1[S1 > 0 ? S1 * (R1 - 1) : 1];
     __device__ __forceinline__ void load(const float2 *tw, int lane)
     {
+        const int gl = lane % LP;
 #pragma unroll
         for (int n = 0; n < NB0; ++n) {
-            const int b = (lane + 32 * n) % (N / R0);
+            const int b = (gl + LP * n) % (N / R0);
 #pragma unroll
             for (int i = 1; i < R0; ++i) t0[n * (R0 - 1) + i - 1] = tw[(i * b * (NTW / N)) & (NTW - 1)];
         }
 #pragma unroll
         for (int n = 0; n < S1; ++n) {
-            const int b = (lane + 32 * n) % ST1;
+            const int b = (gl + LP * n) % ST1;
 #pragma unroll
             for (int i = 1; i < R1; ++i) t1[n * (R1 - 1) + i - 1] = tw[(i * b * (NTW / L1)) & (NTW - 1)];
         }
     }
 };
 
-// One pass (sub-FFT length L, radix R) of a length-N FFT held by one warp in a padded scratch row; rt = the
-// lane's twiddles (SETS sets of R-1), unused when the pass has none (L == R).
-template <int N, int L, int R, bool INV, int SETS>
-__device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int lane)
+// One pass (sub-FFT length L, radix R) of a length-N FFT held by LP lanes of a warp in a padded scratch row
+// (gl = lane % LP; the other lanes of the warp work on their own rows); rt = the lane's twiddles (SETS sets of
+// R-1), unused when the pass has none (L == R).
+template <int N, int L, int R, bool INV, int SETS, int LP>
+__device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int gl)
 {
-    constexpr int ST = L / R, NB = (N / R + 31) / 32;
+    constexpr int ST = L / R, NB = (N / R + LP - 1) / LP;
 #pragma unroll
     for (int n = 0; n < NB; ++n) {
-        const int g = lane + 32 * n;
+        const int g = gl + LP * n;
         if (g < N / R) {
             const int blk = g / ST, b = g % ST;
             const int base = blk * L + b;
@@ -239,18 +242,18 @@ __device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int 
 }
 
 template <int N, bool INV, int NTW>
-__device__ __forceinline__ void warp_fft(float2 *sc, const RowTw<N, NTW> &rt, int lane)
+__device__ __forceinline__ void warp_fft(float2 *sc, const RowTw<N, NTW> &rt, int gl)
 {
     using T = RowTw<N, NTW>;
-    constexpr int R0 = T::R0, R1 = T::R1, R2 = T::R2;
+    constexpr int R0 = T::R0, R1 = T::R1, R2 = T::R2, LP = T::LP;
     if (!INV) {
-        warp_fft_pass<N, N, R0, false, T::NB0>(sc, rt.t0, lane);
-        warp_fft_pass<N, N / R0, R1, false, T::S1>(sc, rt.t1, lane);
-        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, 1>(sc, rt.t1, lane);
+        warp_fft_pass<N, N, R0, false, T::NB0, LP>(sc, rt.t0, gl);
+        if constexpr (R1 > 1) warp_fft_pass<N, N / R0, R1, false, T::S1, LP>(sc, rt.t1, gl);
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, 1, LP>(sc, rt.t1, gl);
     } else {
-        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, 1>(sc, rt.t1, lane);
-        warp_fft_pass<N, N / R0, R1, true, T::S1>(sc, rt.t1, lane);
-        warp_fft_pass<N, N, R0, true, T::NB0>(sc, rt.t0, lane);
+        if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, 1, LP>(sc, rt.t1, gl);
+        if constexpr (R1 > 1) warp_fft_pass<N, N / R0, R1, true, T::S1, LP>(sc, rt.t1, gl);
+        warp_fft_pass<N, N, R0, true, T::NB0, LP>(sc, rt.t0, gl);
     }
 }
 
@@ -313,12 +316,14 @@ struct Cfg {
     static constexpr int NTW = H > W ? H : W;
     static constexpr int PADW = W + W / 16;
     static constexpr int rch0 = 16384 / (W * (int)sizeof(PIX));
-    static constexpr int rch1 = rch0 > 2 * NWARP ? rch0 : 2 * NWARP;
+    static constexpr int RG = cc_row_group(W);  // row pairs per warp in the row FFT phases
+    static constexpr int LP = 32 / RG;
+    static constexpr int rch1 = rch0 > 2 * NWARP * RG ? rch0 : 2 * NWARP * RG;
     static constexpr int RCH = NR < rch1 ? NR : rch1;  // rows per raw chunk
     static constexpr int NCHK = NR / RCH;
     static constexpr int CHB = RCH * W * (int)sizeof(PIX);
     static constexpr int RAWB = (NCHK > 1 ? 2 : 1) * CHB;
-    static constexpr int SCRB = NWARP * PADW * 8;
+    static constexpr int SCRB = NWARP * RG * PADW * 8;
     // stage 1: thread grid R1 (rows of [U|V]) x Cn1 (groups of TN1 spectrum floats) x KS1 (k-split); a warp covers
     // WR1 x WC1 threads of one k-slice
     static constexpr int Cn1 = 2 * NC / TN1;
@@ -348,7 +353,7 @@ struct Cfg {
     static constexpr size_t FIXED_BYTES =
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
-    static_assert(NR % RCH == 0 && RCH % 2 == 0, "bad raw chunking");
+    static_assert(NR % RCH == 0 && RCH % 2 == 0 && (RCH / 2) % RG == 0 && (NR / 2) % RG == 0, "bad raw chunking");
     static_assert((2 * NC) % TN1 == 0 && NT % (Cn1 * KS1) == 0 && TN1 % 4 == 0 && Cn1 % WC1 == 0 && 32 % WC1 == 0, "bad stage-1 tiling");
     static_assert(R1 % 4 == 0 && R1 % WR1 == 0 && (R1 / WR1) * WG1C * KS1 == NWARP && BK1 % KS1 == 0, "bad stage-1 warp grid");
     static_assert(TM1 == 1 || TM1 == 2 || TM1 == 3 || TM1 == 4 || TM1 == 5 || TM1 == 8 || TM1 == 10, "TM1 chunking");
@@ -393,7 +398,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
     uint32_t *const relcnt = reinterpret_cast<uint32_t *>(cmdslot + 2);  // [NSTG] releases of each ring slot (mod NWARP)
 
-    float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + warp * PADW;
+    constexpr int RG = C::RG, LP = C::LP;
+    const int gl = lane % LP, gp = lane / LP;  // lane within its row pair, row pair within the warp
+    float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + (warp * RG + gp) * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
 
     // local spectrum block S[y][ql], y in [0,H), ql in [0,NC)
@@ -707,10 +714,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 const int rb = ck & 1;
                 bar_wait(rb);
                 const PIX *rw = raw + (size_t)rb * C::RCH * W;
-                for (int jp = warp; jp < C::RCH / 2; jp += NWARP) {
+                for (int jp0 = warp * RG; jp0 < C::RCH / 2; jp0 += NWARP * RG) {
+                    const int jp = jp0 + gp;
                     const PIX *ra = rw + (size_t)jp * W;
                     const PIX *rbp = rw + (size_t)(jp + C::RCH / 2) * W;
-                    for (int x = lane; x < W; x += 32)
+                    for (int x = gl; x < W; x += LP)
                         if (p.sn) {  // CC-SN: I'^2 - c0 with I' = I + eps (Eq. (7)), one rounding
                             const double ta = (double)ra[x] + p.sn_eps, tb = (double)rbp[x] + p.sn_eps;
                             scr[padi(x)] = make_float2((float)fma(ta, ta, -p.sn_c0), (float)fma(tb, tb, -p.sn_c0));
@@ -718,10 +726,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                             scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
                         }
                     __syncwarp();
-                    warp_fft<W, false, NTW>(scr, rtw, lane);
+                    warp_fft<W, false, NTW>(scr, rtw, gl);
                     // untangle the two real rows and scatter to the column owners
                     const int ya = rank * NR + ck * C::RCH + jp, yb = ya + C::RCH / 2;
-                    for (int k = lane; k < W / 2; k += 32) {
+                    for (int k = gl; k < W / 2; k += LP) {
                         float2 A, B;
                         if (k == 0) {
                             const float2 z0 = scr[padi(rslot[0])], zn = scr[padi(rslot[W / 2])];
@@ -848,9 +856,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             RowTw<W, NTW> rtw;
             rtw.load(tw, lane);
             Best bst{-INFINITY, 0x7fffffff};
-            for (int jp = warp; jp < NR / 2; jp += NWARP) {
+            for (int jp0 = warp * RG; jp0 < NR / 2; jp0 += NWARP * RG) {
+                const int jp = jp0 + gp;
                 const int ya = rank * NR + jp, yb = ya + NR / 2;
-                for (int k = lane; k < W / 2; k += 32) {
+                for (int k = gl; k < W / 2; k += LP) {
                     const float2 *Sd = Sof(k / NC);
                     const float2 qa = Sd[(size_t)ya * NC + (k % NC)], qb = Sd[(size_t)yb * NC + (k % NC)];
                     if (k == 0) {
@@ -862,8 +871,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                 }
                 __syncwarp();
-                warp_fft<W, true, NTW>(scr, rtw, lane);
-                for (int x = lane; x < W; x += 32) {
+                warp_fft<W, true, NTW>(scr, rtw, gl);
+                for (int x = gl; x < W; x += LP) {
                     const float2 z = scr[padi(x)];
                     if (better(z.x, ya * W + x, bst.v, bst.i)) bst.v = z.x, bst.i = ya * W + x;
                     if (better(z.y, yb * W + x, bst.v, bst.i)) bst.v = z.y, bst.i = yb * W + x;
