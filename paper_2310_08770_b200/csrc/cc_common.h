@@ -21,15 +21,15 @@ __host__ __device__ constexpr int cc_radix_col(int N, int p)
 // all lanes busy instead of N/16 of them.
 __host__ __device__ constexpr int cc_radix_row(int N, int p)
 {
-    return N == 64   ? (p == 0 ? 4 : p == 1 ? 4 : 4)
+    return N == 64   ? (p == 0 ? 8 : p == 1 ? 8 : 1)   // four row pairs per warp, 8 lanes each
          : N == 128  ? (p == 0 ? 4 : p == 1 ? 4 : 8)
          : N == 256  ? (p == 0 ? 16 : p == 1 ? 16 : 1)  // two row pairs per warp, 16 lanes each (cc_row_group)
          : N == 512  ? (p == 0 ? 8 : p == 1 ? 8 : 8)
          : N == 1024 ? (p == 0 ? 16 : p == 1 ? 8 : 8)
                      : 0;
 }
-// Row pairs a warp transforms side by side (32 / cc_row_group lanes each): two passes instead of three at N = 256.
-__host__ __device__ constexpr int cc_row_group(int N) { return N == 256 ? 2 : 1; }
+// Row pairs a warp transforms side by side (32 / cc_row_group lanes each): two passes instead of three at N = 64, 256.
+__host__ __device__ constexpr int cc_row_group(int N) { return N == 256 ? 2 : N == 64 ? 4 : 1; }
 __host__ __device__ constexpr int cc_radix(int N, int p, bool row) { return row ? cc_radix_row(N, p) : cc_radix_col(N, p); }
 
 // Frequency held by slot p after the forward FFT of length N:
