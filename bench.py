@@ -268,7 +268,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2310_08770_b200 import Plan, fp32_peak_probe
+    from paper_2310_08770_b200 import Plan, fp32_peak_probe, fp32_tile_probe
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -356,6 +356,7 @@ def main():
     peak_tf = 148 * FP32_LANES_PER_SM * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12
     achieved_tf = flop * B / (kern_ms * 1e-3) / 1e12
     probe_tf = fp32_peak_probe()
+    tile_tf = fp32_tile_probe()
     hbm_gbs = None
     try:
         hbm_gbs = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
@@ -369,7 +370,8 @@ def main():
         "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
         "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,
-        "ffma_probe_tflops": probe_tf,
+        "ffma_probe_tflops": probe_tf, "ffma_register_tile_probe_tflops": tile_tf,
+        "frac_of_register_tile_rate": achieved_tf / tile_tf,
         "roofline_frames_per_s": 1.0 / max(t_alu, t_hbm), "hbm_leg_frames_per_s": 1.0 / t_hbm,
         "hbm_achieved_gbs": (frames[0].nbytes + 12) * B / (kern_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_gbs,
     }

@@ -218,6 +218,15 @@ cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info);
  */
 cc_status cc_fp32_peak_probe(double *tflops, void *stream);
 
+/*
+ * cc_fp32_tile_probe -- second measurement aid: an 8x8 register-tile FFMA loop with all three operands in
+ * registers (the instruction mix of a register-tiled FP32 GEMM inner loop, no memory traffic).  The rate it
+ * reaches is the practical ceiling of the upsampled-DFT GEMM loops; cc_fp32_peak_probe's loop (constant
+ * operands) reaches the nominal lane rate.
+ *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
+ */
+cc_status cc_fp32_tile_probe(double *tflops, void *stream);
+
 const char *cc_status_string(cc_status s);
 const char *cc_last_error(void); /* thread-local detail of the last failure */
 

@@ -20,7 +20,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_fp32_peak_probe", "cc_track_latency_probe",
+           "cc_plan_info", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -84,6 +84,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_plan_info.restype = ci
         lib.cc_fp32_peak_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         lib.cc_fp32_peak_probe.restype = ci
+        lib.cc_fp32_tile_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
+        lib.cc_fp32_tile_probe.restype = ci
         lib.cc_status_string.argtypes = [ci]
         lib.cc_status_string.restype = ctypes.c_char_p
         lib.cc_last_error.restype = ctypes.c_char_p
@@ -264,4 +266,11 @@ def fp32_peak_probe() -> float:
     _torch()
     v = ctypes.c_double()
     _check(load_library().cc_fp32_peak_probe(ctypes.byref(v), None))
+    return v.value
+
+
+def fp32_tile_probe() -> float:
+    _torch()
+    v = ctypes.c_double()
+    _check(load_library().cc_fp32_tile_probe(ctypes.byref(v), None))
     return v.value

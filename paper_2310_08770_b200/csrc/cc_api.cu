@@ -858,6 +858,63 @@ extern "C" cc_status cc_fp32_peak_probe(double *tflops, void *stream)
     return CC_OK;
 }
 
+__global__ void __launch_bounds__(256, 1) cc_ffma_tile_probe_kernel(float *out, const float *in, int iters)
+{
+    float a[8], b[8], acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = in[threadIdx.x + i], b[i] = in[threadIdx.x + 8 + i];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+        a[0] += 1e-9f, b[7] -= 1e-9f;  // keeps the loop from being hoisted (2 FADD per 64 FFMA)
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += acc[i][j];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" cc_status cc_fp32_tile_probe(double *tflops, void *stream)
+{
+    if (!tflops) return fail(CC_ERR_INVALID_ARG, "cc_fp32_tile_probe: null pointer");
+    cc_status st = check_device();
+    if (st != CC_OK) return st;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms, threads = 256, iters = 20000;  // 8 warps per SM, as the fused kernel runs
+    float *out = nullptr, *in = nullptr;
+    CK(cudaMalloc((void **)&out, (size_t)blocks * threads * sizeof(float)));
+    CK(cudaMalloc((void **)&in, 4096));
+    CK(cudaMemset(in, 0, 4096));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    cudaStream_t s = (cudaStream_t)stream;
+    cc_ffma_tile_probe_kernel<<<blocks, threads, 0, s>>>(out, in, 64);
+    float best = 1e30f;
+    for (int r = 0; r < 3; ++r) {
+        CK(cudaEventRecord(e0, s));
+        cc_ffma_tile_probe_kernel<<<blocks, threads, 0, s>>>(out, in, iters);
+        CK(cudaEventRecord(e1, s));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        best = std::min(best, ms);
+    }
+    cudaEventDestroy(e0), cudaEventDestroy(e1), cudaFree(out), cudaFree(in);
+    *tflops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads / ((double)best * 1e-3) / 1e12;
+    return CC_OK;
+}
+
 extern "C" const char *cc_status_string(cc_status s)
 {
     switch (s) {

@@ -232,6 +232,8 @@ def test_host_path_matches_device_path(gpu):
 def test_fp32_probe_reports_sane_rate(gpu):
     tf = gpu.fp32_peak_probe()
     assert 30.0 < tf < 80.0
+    tile = gpu.fp32_tile_probe()          # register-operand FFMA tiles: below the constant-operand loop
+    assert 20.0 < tile <= tf * 1.02
 
 
 @pytest.mark.parametrize("ci,n", [(2, 200), (1, 64), (4, 12)])
