@@ -74,6 +74,8 @@ def _load():
         lib.cco_track_sn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float),
                                      ctypes.c_double, ctypes.POINTER(_Result), ctypes.c_int]
+        lib.cco_drift_correct.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float), ctypes.c_int,
+                                          ctypes.c_double, ctypes.c_double, dp, dp, dp]
         lib.cco_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -224,3 +226,18 @@ def track(frames, reference, u: int, threads: int = 0, method: str = "u", epsilo
     return TrackResult(*(arr[k].copy() for k in
                          ("dy", "dx", "peak", "wy", "wx", "m", "n",
                           "cc_top1", "cc_top2", "up_top1", "up_top2")))
+
+
+def drift_correct(dx, dy, a0: float, max_step: float = 0.0, state=None):
+    """PAPER.md:L110-127, Eqs. (10)-(12): returns (dx', dy', state) with state = (Rx, Ry) after the last sample."""
+    dx = np.ascontiguousarray(dx, dtype=np.float32)
+    dy = np.ascontiguousarray(dy, dtype=np.float32)
+    n = dx.size
+    st = np.zeros(2) if state is None else np.array(state, dtype=np.float64)
+    ox, oy = np.empty(n), np.empty(n)
+    fp = ctypes.POINTER(ctypes.c_float)
+    rc = _load().cco_drift_correct(dx.ctypes.data_as(fp), dy.ctypes.data_as(fp), n, float(a0), float(max_step),
+                                   _d(st), _d(ox), _d(oy))
+    if rc:
+        raise ValueError("oracle cco_drift_correct failed: %d" % rc)
+    return ox, oy, st

@@ -444,3 +444,40 @@ int cco_track_sn(const void *frames, int dtype, int batch, int H, int W, int u,
     if (!(eps >= 0.0)) return -2;
     return track_impl(frames, dtype, batch, H, W, u, reference, 1, eps, out, threads);
 }
+
+/* Drift correction of the detected motion.
+ * Plain (max_step <= 0), Eq. (10):      R_n = a0 r_n + b1 R_{n-1},  b1 = 1 - a0
+ * Rate-limited (max_step = alpha/u), Eqs. (11)-(12):
+ *     dR_n = a0 r_n + (b1 - 1) R_{n-1}
+ *     R_n  = R_{n-1} + max_step * dR_n/|dR_n|   if |dR_n| > max_step,   else R_{n-1} + dR_n
+ * Output r'_n = r_n - R_n.  R_{-1} = (0, 0) (so R_0 = a0 r_0 in the plain case, as the paper states);
+ * state[2] = (Rx, Ry) carries R across calls. */
+int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double max_step,
+                      double state[2], double *out_dx, double *out_dy)
+{
+    if (!dx || !dy || !state || !out_dx || !out_dy || n < 0 || !(a0 >= 0.0 && a0 <= 1.0)) return -2;
+    const double b1 = 1.0 - a0;
+    double Rx = state[0], Ry = state[1];
+    for (int i = 0; i < n; ++i) {
+        const double rx = (double)dx[i], ry = (double)dy[i];
+        if (max_step > 0.0) {
+            const double ex = a0 * rx + (b1 - 1.0) * Rx;      /* Eq. (11) */
+            const double ey = a0 * ry + (b1 - 1.0) * Ry;
+            const double norm = sqrt(ex * ex + ey * ey);
+            if (norm > max_step) {                           /* Eq. (12), first case */
+                Rx = Rx + max_step * (ex / norm);
+                Ry = Ry + max_step * (ey / norm);
+            } else {
+                Rx = Rx + ex;
+                Ry = Ry + ey;
+            }
+        } else {
+            Rx = a0 * rx + b1 * Rx;                          /* Eq. (10) */
+            Ry = a0 * ry + b1 * Ry;
+        }
+        out_dx[i] = rx - Rx;
+        out_dy[i] = ry - Ry;
+    }
+    state[0] = Rx; state[1] = Ry;
+    return 0;
+}

@@ -106,6 +106,13 @@ int cco_track(const void *frames, int dtype, int batch, int H, int W, int u,
 int cco_track_sn(const void *frames, int dtype, int batch, int H, int W, int u,
                  const float *reference, double eps, cco_result *out, int threads);
 
+/* Drift correction: r'_n = r_n - R_n with the low-pass offset R_n of Eq. (10)
+ * (max_step <= 0) or its rate-limited form, Eqs. (11)-(12), with max_step = alpha/u.  b1 = 1 - a0,
+ * R_{-1} = 0; state[2] = (Rx, Ry) in/out.  Garbling: Eq. (12) prints "d\hat{R}_n" for the unit vector
+ * dR_n/|dR_n| (R14).  Returns 0 on success. */
+int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double max_step,
+                      double state[2], double *out_dx, double *out_dy);
+
 int cco_num_threads(void);
 
 #ifdef __cplusplus

@@ -443,3 +443,45 @@ def test_sn5_scaling_invariance(oracle_mod):
     b = oracle_mod.track((2 * fr).astype(np.uint16), 2 * ref, 10, method="sn", epsilon=12.0)   # I', E' both doubled
     assert np.array_equal(a.dx, b.dx) and np.array_equal(a.dy, b.dy)
     assert np.allclose(b.peak, 2 * a.peak, rtol=1e-12)
+
+
+# ---------------------------------------------------------------- drift correction (Eqs. (10)-(12))
+def test_d1_plain_filter_closed_forms(oracle_mod):
+    """Eq. (10) with R_0 = a0 r_0: a constant input c gives R_n = c (1 - b1^(n+1)); an impulse gives a0 b1^n."""
+    a0, n = 0.05, 200
+    c = np.float32(1.25)
+    ox, oy, st = oracle_mod.drift_correct(np.full(n, c), np.full(n, -2 * c), a0)
+    k = np.arange(1, n + 1)
+    assert np.allclose(ox, float(c) * (1 - a0) ** k, rtol=1e-12) and np.allclose(oy, -2 * float(c) * (1 - a0) ** k, rtol=1e-12)
+    assert np.allclose(st, [float(c) * (1 - (1 - a0) ** n), -2 * float(c) * (1 - (1 - a0) ** n)], rtol=1e-12)
+    imp = np.zeros(50, np.float32)
+    imp[0] = 1.0
+    ox, _, _ = oracle_mod.drift_correct(imp, imp, 0.2)
+    assert np.allclose(ox[1:], -0.2 * 0.8 ** np.arange(1, 50), rtol=1e-12) and abs(ox[0] - 0.8) < 1e-15
+
+
+def test_d2_rate_limited_steps_exactly_max_step(oracle_mod):
+    """Eq. (12): while |dR_n| > alpha/u the offset moves exactly alpha/u along dR_n; afterwards it follows Eq. (10)."""
+    a0, step, n = 0.5, 0.005, 40
+    rx, ry = np.full(n, 3.0, np.float32), np.full(n, 4.0, np.float32)         # direction (0.6, 0.8), |a0 r| = 2.5 >> step
+    ox, oy, st = oracle_mod.drift_correct(rx, ry, a0, step)
+    k = np.arange(1, n + 1)
+    assert np.allclose(3.0 - ox, 0.6 * step * k, rtol=1e-12) and np.allclose(4.0 - oy, 0.8 * step * k, rtol=1e-12)
+    # small input: never clamped -> identical to the plain filter
+    rng = np.random.default_rng(3)
+    sx, sy = (1e-3 * rng.standard_normal(100)).astype(np.float32), (1e-3 * rng.standard_normal(100)).astype(np.float32)
+    a = oracle_mod.drift_correct(sx, sy, 0.1, 0.005)
+    b = oracle_mod.drift_correct(sx, sy, 0.1, 0.0)
+    assert np.allclose(a[0], b[0], atol=1e-15) and np.allclose(a[1], b[1], atol=1e-15)
+
+
+def test_d3_state_carries_across_calls_and_linearity(oracle_mod):
+    rng = np.random.default_rng(4)
+    x, y = rng.standard_normal(300).astype(np.float32), rng.standard_normal(300).astype(np.float32)
+    for step in (0.0, 0.005):
+        full = oracle_mod.drift_correct(x, y, 0.02, step)
+        h1 = oracle_mod.drift_correct(x[:120], y[:120], 0.02, step)
+        h2 = oracle_mod.drift_correct(x[120:], y[120:], 0.02, step, state=h1[2])
+        assert np.array_equal(np.concatenate([h1[0], h2[0]]), full[0]) and np.array_equal(h2[2], full[2])
+    p = oracle_mod.drift_correct(2 * x, 2 * y, 0.02)[0]                       # plain filter is linear
+    assert np.allclose(p, 2 * oracle_mod.drift_correct(x, y, 0.02)[0], rtol=1e-12, atol=1e-15)
