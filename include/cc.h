@@ -205,6 +205,23 @@ cc_status cc_rt_close(cc_rt *rt);
 cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, float *dy, float *peak,
                               double *lat_us);
 
+/*
+ * cc_drift_correct -- PAPER.md:L110-127: removes the slowly drifting equilibrium position from a sequence of
+ * displacements, r'_n = r_n - R_n, with the low-pass offset of Eq. (10), R_n = a0 r_n + b1 R_{n-1}
+ * (b1 = 1 - a0; R_{-1} = 0, so R_0 = a0 r_0), or, when max_step > 0, its rate-limited form of Eqs. (11)-(12):
+ * the offset moves by at most max_step = alpha/u per sample (the paper suggests alpha = 0.5).  A sequential
+ * recurrence, evaluated in double precision by one warp on the device.
+ *   dx, dy     DEVICE pointers, n float32 each (e.g. the outputs of cc_track)
+ *   a0         1 - exp(-T/tau), in [0, 1]
+ *   max_step   alpha / upsample, or <= 0 for the plain filter
+ *   state      DEVICE pointer, 2 float64 (Rx, Ry), read and updated: zero it before the first call; consecutive
+ *              calls then continue the same filter
+ *   dxc, dyc   DEVICE pointers, n float32 each: the corrected displacements (may alias dx, dy)
+ * Only enqueues work on `stream`.  n == 0 -> CC_OK.
+ */
+cc_status cc_drift_correct(const float *dx, const float *dy, int n, double a0, double max_step,
+                           double *state, float *dxc, float *dyc, void *stream);
+
 /* Frees every device/host allocation of the plan.  NULL is a no-op. */
 cc_status cc_plan_destroy(cc_plan *plan);
 

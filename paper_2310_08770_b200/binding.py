@@ -20,7 +20,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
+           "cc_plan_info", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -84,6 +84,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_plan_info.restype = ci
         lib.cc_fp32_peak_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         lib.cc_fp32_peak_probe.restype = ci
+        lib.cc_drift_correct.argtypes = [vp, vp, ci, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp]
+        lib.cc_drift_correct.restype = ci
         lib.cc_fp32_tile_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         lib.cc_fp32_tile_probe.restype = ci
         lib.cc_status_string.argtypes = [ci]
@@ -274,3 +276,17 @@ def fp32_tile_probe() -> float:
     v = ctypes.c_double()
     _check(load_library().cc_fp32_tile_probe(ctypes.byref(v), None))
     return v.value
+
+
+def drift_correct(dx, dy, a0: float, max_step: float = 0.0, state=None, stream=None):
+    """cc_drift_correct on device tensors dx, dy (float32).  `state` = device float64 tensor (Rx, Ry), updated in
+    place (None: starts from zero).  Returns (dx', dy', state); nothing is synchronised."""
+    torch = _torch()
+    n = dx.numel()
+    if state is None:
+        state = torch.zeros(2, dtype=torch.float64, device=dx.device)
+    ox, oy = torch.empty_like(dx), torch.empty_like(dy)
+    s = (stream.cuda_stream if stream is not None else torch.cuda.current_stream(dx.device).cuda_stream)
+    _check(load_library().cc_drift_correct(dx.data_ptr(), dy.data_ptr(), n, float(a0), float(max_step), state.data_ptr(),
+                                           ox.data_ptr(), oy.data_ptr(), s))
+    return ox, oy, state

@@ -795,6 +795,59 @@ extern "C" cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, f
     return CC_OK;
 }
 
+// ------------------------------------------------------------------ drift correction
+// One warp: the lanes fetch 32 samples at a time (coalesced), lane 0 runs the recurrence of Eqs. (10)-(12) in fp64
+// with separately rounded multiplies and adds (no contraction: the same roundings as a plain C evaluation), the
+// lanes store the 32 corrected samples.
+__global__ void __launch_bounds__(32, 1) cc_drift_kernel(const float *dx, const float *dy, int n, double a0, double max_step,
+                                                         double *state, float *dxc, float *dyc)
+{
+    const int lane = threadIdx.x;
+    const double b1 = 1.0 - a0, b1m1 = b1 - 1.0;
+    double Rx = state[0], Ry = state[1];
+    for (int base = 0; base < n; base += 32) {
+        const int i = base + lane;
+        const float fx = i < n ? dx[i] : 0.f, fy = i < n ? dy[i] : 0.f;
+        float ox = 0.f, oy = 0.f;
+        const int cnt = min(32, n - base);
+        for (int k = 0; k < cnt; ++k) {
+            const double rx = (double)__shfl_sync(0xffffffffu, fx, k), ry = (double)__shfl_sync(0xffffffffu, fy, k);
+            if (max_step > 0.0) {
+                const double ex = __dadd_rn(__dmul_rn(a0, rx), __dmul_rn(b1m1, Rx));  // Eq. (11)
+                const double ey = __dadd_rn(__dmul_rn(a0, ry), __dmul_rn(b1m1, Ry));
+                const double norm = __dsqrt_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)));
+                if (norm > max_step) {  // Eq. (12), first case
+                    Rx = __dadd_rn(Rx, __dmul_rn(max_step, __ddiv_rn(ex, norm)));
+                    Ry = __dadd_rn(Ry, __dmul_rn(max_step, __ddiv_rn(ey, norm)));
+                } else {
+                    Rx = __dadd_rn(Rx, ex);
+                    Ry = __dadd_rn(Ry, ey);
+                }
+            } else {  // Eq. (10)
+                Rx = __dadd_rn(__dmul_rn(a0, rx), __dmul_rn(b1, Rx));
+                Ry = __dadd_rn(__dmul_rn(a0, ry), __dmul_rn(b1, Ry));
+            }
+            if (lane == k) ox = (float)(rx - Rx), oy = (float)(ry - Ry);
+        }
+        if (i < n) dxc[i] = ox, dyc[i] = oy;
+    }
+    if (lane == 0) state[0] = Rx, state[1] = Ry;
+}
+
+extern "C" cc_status cc_drift_correct(const float *dx, const float *dy, int n, double a0, double max_step, double *state,
+                                      float *dxc, float *dyc, void *stream)
+{
+    if (n < 0 || !(a0 >= 0.0 && a0 <= 1.0)) return fail(CC_ERR_INVALID_ARG, "cc_drift_correct: bad n or a0");
+    if (n == 0) return CC_OK;
+    if (!dx || !dy || !state || !dxc || !dyc) return fail(CC_ERR_INVALID_ARG, "cc_drift_correct: null pointer");
+    cc_status st = check_device();
+    if (st != CC_OK) return st;
+    cc_drift_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(dx, dy, n, a0, max_step, state, dxc, dyc);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "drift kernel launch");
+    return CC_OK;
+}
+
 extern "C" cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info)
 {
     if (!plan || !info) return fail(CC_ERR_INVALID_ARG, "cc_plan_info: null pointer");

@@ -340,3 +340,27 @@ def test_ccsn_argument_errors(gpu):
     assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 1, ctypes.c_float(0.0)) == 1
     assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 1, ctypes.c_float(-1.0)) == 1
     assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 7, ctypes.c_float(1.0)) == 1
+
+
+# ---------------------------------------------------------------- drift correction: cc_drift_correct
+@pytest.mark.parametrize("max_step", [0.0, 0.005])
+def test_drift_correction_matches_oracle(gpu, oracle_mod, max_step):
+    """Eqs. (10)-(12) on a slowly drifting, jittering track: every corrected sample equals the oracle's (same fp64
+    roundings, then one rounding to float32); two consecutive calls continue the filter of one call."""
+    import torch
+    rng = np.random.default_rng(8)
+    n = 10000                                                       # one batch of configs[2]; ragged tail: 10000 % 32 != 0
+    drift = np.cumsum(2e-4 * rng.standard_normal((n, 2)), axis=0) + np.linspace(0, 1.5, n)[:, None]
+    r = (np.round((drift + 0.05 * rng.standard_normal((n, 2))) * 100) / 100).astype(np.float32)   # 1/u grid, u = 100
+    ox, oy, st = oracle_mod.drift_correct(r[:, 1], r[:, 0], 0.01, max_step)
+    dx, dy = torch.from_numpy(r[:, 1].copy()).cuda(), torch.from_numpy(r[:, 0].copy()).cuda()
+    gx, gy, gs = gpu.drift_correct(dx, dy, 0.01, max_step)
+    assert np.array_equal(gx.cpu().numpy(), ox.astype(np.float32)) and np.array_equal(gy.cpu().numpy(), oy.astype(np.float32))
+    assert np.array_equal(gs.cpu().numpy(), st)
+    k = 4097
+    ax, ay, s1 = gpu.drift_correct(dx[:k], dy[:k], 0.01, max_step)
+    bx, by, s2 = gpu.drift_correct(dx[k:], dy[k:], 0.01, max_step, state=s1)
+    assert torch.equal(torch.cat([ax, bx]), gx) and torch.equal(torch.cat([ay, by]), gy) and torch.equal(s2, gs)
+    lib = gpu.load_library()
+    assert lib.cc_drift_correct(None, None, 0, 0.1, 0.0, None, None, None, None) == 0       # n == 0
+    assert lib.cc_drift_correct(dx.data_ptr(), dy.data_ptr(), 4, 1.5, 0.0, gs.data_ptr(), gx.data_ptr(), gy.data_ptr(), None) == 1
