@@ -206,6 +206,41 @@ def run_table(args):
         print(json.dumps(row), flush=True)
 
 
+def run_table1(args):
+    """--table1: the settings of the paper's Table I (CC-SN, one image per call, u = 128 ... 1024)
+    on synthetic 12-bit spot frames: images/s of sequential single-frame calls (the paper's mode) and of one batched
+    call.  Context for BASELINE.md section 1, not a target."""
+    import torch
+    from paper_2310_08770_b200 import Plan
+    rng = np.random.default_rng(7)
+    for (H, W) in ((128, 256), (256, 256), (256, 512), (512, 512), (128, 1024)):
+        y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+        spot = lambda sy, sx: 900.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 4.0 ** 2)) + 15.0
+        ref = spot(0.0, 0.0).astype(np.float32)
+        nb = 592
+        sh = rng.uniform(-9, 9, size=(16, 2))
+        fr16 = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 4095).astype(np.uint16)
+        fr = np.concatenate([fr16] * (nb // 16))
+        for u in (128, 256, 512, 1024):
+            plan = Plan(H, W, fr.dtype, u, ref, method="sn", epsilon=200.0)
+            d = plan.device_frames(fr)
+            out = tuple(torch.empty(nb, dtype=torch.float32, device="cuda") for _ in range(3))
+            plan.track(d, nb, out=out)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            plan.track(d, nb, out=out)
+            b.record()
+            torch.cuda.synchronize()
+            batched = nb / (a.elapsed_time(b) * 1e-3)
+            plan.latency_probe(d, 20)
+            lat = plan.latency_probe(d, 100)[3]
+            print(json.dumps({"rows_x_cols": "%dx%d" % (H, W), "u": u, "method": "CC-SN",
+                              "images_per_s_single_frame_calls": 1e6 / float(np.median(lat)),
+                              "single_frame_latency_us_median": float(np.median(lat)),
+                              "images_per_s_batched": batched, "batch": nb}), flush=True)
+            plan.close()
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -251,6 +286,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--table", action="store_true", help="per-config numbers for BASELINE.md section 3 and exit")
+    ap.add_argument("--table1", action="store_true", help="the paper's Table I settings (context numbers) and exit")
     ap.add_argument("--phases", action="store_true", help="print the per-phase cycle breakdown of every config and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -260,6 +296,9 @@ def main():
         return
     if args.table:
         run_table(args)
+        return
+    if args.table1:
+        run_table1(args)
         return
     cfg = wl.config(3)
     if args.impl == "reference":

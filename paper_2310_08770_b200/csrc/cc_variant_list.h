@@ -22,3 +22,10 @@ CCV(f512_u16,      512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false, 16,  8,  8,
 CCV(f512_u8,       512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false, 16,  8,  8,  4,  3,  2,  1)
 CCV(f1024_u16,    1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,  16,  8,  4,  4,  3,  2,  1)
 CCV(f1024_u8,     1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,  16,  8,  4,  4,  3,  2,  1)
+// non-square camera formats of the paper's Table I; H = rows, W = columns
+CCV(f128x256_u16,  128,  256, 1, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
+CCV(f256x128_u16,  256,  128, 1, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
+CCV(f256x512_u16,  256,  512, 4, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
+CCV(f512x256_u16,  512,  256, 4, uint16_t, 256, 10, 4,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
+CCV(f128x1024_u16, 128, 1024, 8, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
+CCV(f1024x128_u16, 1024, 128, 4, uint16_t, 256,  5, 4,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)

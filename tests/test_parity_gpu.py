@@ -364,3 +364,39 @@ def test_drift_correction_matches_oracle(gpu, oracle_mod, max_step):
     lib = gpu.load_library()
     assert lib.cc_drift_correct(None, None, 0, 0.1, 0.0, None, None, None, None) == 0       # n == 0
     assert lib.cc_drift_correct(dx.data_ptr(), dy.data_ptr(), 4, 1.5, 0.0, gs.data_ptr(), gx.data_ptr(), gy.data_ptr(), None) == 1
+
+
+@pytest.mark.parametrize("H,W", [(128, 256), (256, 128), (256, 512), (512, 256), (128, 1024), (1024, 128)])
+@pytest.mark.parametrize("method,eps", [("u", 0.0), ("sn", 200.0)])
+def test_non_square_formats(gpu, oracle_mod, H, W, method, eps):
+    """Non-square camera formats of the paper's Table I: Gaussian spot + Poisson noise,
+    shifts up to +-12 px per axis, u = 64; same bar as the square configs."""
+    rng = np.random.default_rng(H * 7 + W)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+    spot = lambda sy, sx: 800.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 3.5 ** 2)) + 12.0
+    ref = spot(0.0, 0.0).astype(np.float32)
+    sh = rng.uniform(-12, 12, size=(40 if H * W <= 32768 else 12, 2))
+    fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 65535).astype(np.uint16)
+    o = oracle_mod.track(fr, ref, 64, method=method, epsilon=eps)
+    plan = gpu.Plan(H, W, fr.dtype, 64, ref, method=method, epsilon=eps)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr), debug=True)]
+    plan.close()
+    _compare(o, dx, dy, pk, iy, ix, "%dx%d %s" % (H, W, method))
+    assert np.median(np.hypot(dx - sh[:, 1], dy - sh[:, 0])) < 0.1
+
+
+@pytest.mark.parametrize("H,W,u", [(256, 256, 128), (256, 256, 1024), (128, 256, 512)])
+def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
+    """The paper's benchmark settings (Table I: CC-SN, u = 128 ... 1024): grids of up to
+    1536 x 1536 samples, many super-blocks of the T buffer; same parity bar."""
+    rng = np.random.default_rng(u + H)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+    spot = lambda sy, sx: 900.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 4.0 ** 2)) + 15.0
+    ref = spot(0.0, 0.0).astype(np.float32)
+    sh = rng.uniform(-9, 9, size=(4, 2))
+    fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 4095).astype(np.uint16)   # 12-bit camera (L210)
+    o = oracle_mod.track(fr, ref, u, method="sn", epsilon=200.0)
+    plan = gpu.Plan(H, W, fr.dtype, u, ref, method="sn", epsilon=200.0)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr), debug=True)]
+    plan.close()
+    _compare(o, dx, dy, pk, iy, ix, "%dx%d u=%d CC-SN" % (H, W, u))
