@@ -1148,6 +1148,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                 ee[j] = ebase + (j < 4 ? tn2 * 4 + j : 4 * Cn2 + tn2);
                                 ny[j] = __ldg(&p.nyqc[ee[j]]);
                             }
+                            // C(m, c+e) = E - O and C(m, c-e) = E + O overwrite the accumulators (-inf outside the
+                            // grid); the chunk's maximum comes from an independent max tree, its smallest index from a
+                            // min tree over the equal entries -- no serial compare-select chain per output
+                            constexpr float NEG = -INFINITY;
+                            int mrow[TM2];
+                            float vmax = NEG;
 #pragma unroll
                             for (int i = 0; i < TM2; ++i) {
                                 const int r = rbase + i;
@@ -1155,18 +1161,31 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                 const int d = d0 + (lower ? r - DS : r);
                                 const int m = lower ? cM - d : cM + d;
                                 const bool rok = r < 2 * DS && d < nd && m >= 0 && m < M && !(lower && d == 0);
+                                mrow[i] = rok ? m * M + cM : -1;
                                 const float tny = Arow[i][1];         // Nyquist column of this T row
 #pragma unroll
                                 for (int j = 0; j < TN2; ++j) {
                                     const int e = ee[j];
                                     const float E = fmaf(tny, ny[j], aE[i][j]), O = aO[i][j];
-                                    if (rok && e < nd) {
-                                        const float cp = E - O, cm = E + O;
-                                        const int np = cM + e, nm = cM - e;
-                                        if (np < M && better(cp, m * M + np, sub.v, sub.i)) sub.v = cp, sub.i = m * M + np;
-                                        if (e > 0 && better(cm, m * M + nm, sub.v, sub.i)) sub.v = cm, sub.i = m * M + nm;
-                                    }
+                                    const bool ok = rok && e < nd;
+                                    aE[i][j] = (ok && cM + e < M) ? E - O : NEG;   // column c + e
+                                    aO[i][j] = (ok && e > 0) ? E + O : NEG;        // column c - e
                                 }
+                                float rm = NEG;
+#pragma unroll
+                                for (int j = 0; j < TN2; ++j) rm = fmaxf(rm, fmaxf(aE[i][j], aO[i][j]));
+                                vmax = fmaxf(vmax, rm);
+                            }
+                            if (vmax > sub.v || (vmax == sub.v && vmax > NEG)) {
+                                int imin = 0x7fffffff;
+#pragma unroll
+                                for (int i = 0; i < TM2; ++i)
+#pragma unroll
+                                    for (int j = 0; j < TN2; ++j) {
+                                        if (aO[i][j] == vmax) imin = min(imin, mrow[i] - ee[j]);
+                                        if (aE[i][j] == vmax) imin = min(imin, mrow[i] + ee[j]);
+                                    }
+                                if (better(vmax, imin, sub.v, sub.i)) sub.v = vmax, sub.i = imin;
                             }
                         }
                     }
