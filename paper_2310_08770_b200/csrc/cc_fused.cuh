@@ -13,7 +13,7 @@
 //                  stage 1  [T(c+d) + T(c-d), T(c+d) - T(c-d)] = [Ee, Eo] * [Q(y0+j) + Q(y0-j), Q(y0+j) - Q(y0-j)]
 //                  stage 2  [C(m,c+e) + C(m,c-e), C(m,c-e) - C(m,c+e)] / 2 = [T_re * cos, T_im * sin]
 //                  (FP32 register-tiled GEMMs with half the multiply-adds of the plain products);
-//                  operand tiles stream L2 -> smem through a TMA ring with full/empty mbarriers
+//                  operand tiles stream L2 -> smem through a TMA ring refilled by the last warp to release a slot
 //   a7 argmax    : streamed out of stage 2, fp64 3x3 hill-climb polish, compose
 // Product code: shares nothing with oracle/.
 #pragma once
@@ -38,10 +38,6 @@ __device__ __forceinline__ void mbar_init(uint64_t *b, uint32_t cnt)
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *b)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity)
 {
@@ -277,27 +273,6 @@ __device__ __forceinline__ Best warp_best(Best b)
     return b;
 }
 
-template <int n>
-__device__ __forceinline__ void load_vec(float (&d)[n], const float *s)
-{
-    if constexpr (n % 4 == 0) {
-#pragma unroll
-        for (int i = 0; i < n / 4; ++i) {
-            const float4 t = reinterpret_cast<const float4 *>(s)[i];
-            d[4 * i] = t.x, d[4 * i + 1] = t.y, d[4 * i + 2] = t.z, d[4 * i + 3] = t.w;
-        }
-    } else if constexpr (n % 2 == 0) {
-#pragma unroll
-        for (int i = 0; i < n / 2; ++i) {
-            const float2 t = reinterpret_cast<const float2 *>(s)[i];
-            d[2 * i] = t.x, d[2 * i + 1] = t.y;
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < n; ++i) d[i] = s[i];
-    }
-}
-
 // ------------------------------------------------------------------ the kernel
 template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
           int R2_, int KS2_, int NSTG_, int PFD_, int KS1_>
@@ -349,7 +324,7 @@ struct Cfg {
     static constexpr int RED_FLOATS = RED1_FLOATS > RED2_FLOATS ? RED1_FLOATS : RED2_FLOATS;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
-    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN + XN) + 16 * NWARP + 64 + 16 + 4 * NSTG;
+    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN) + 16 * NWARP + 64 + 16 + 4 * NSTG;
     static constexpr size_t FIXED_BYTES =
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
@@ -391,8 +366,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
     uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
-    double *const xsrc = xchg + 2 * CS * XN;                           // [XN]
-    float *const wv = reinterpret_cast<float *>(xsrc + XN);            // [NWARP]
+    float *const wv = reinterpret_cast<float *>(xchg + 2 * CS * XN);    // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
     uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
