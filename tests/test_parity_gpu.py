@@ -400,3 +400,25 @@ def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
     dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr), debug=True)]
     plan.close()
     _compare(o, dx, dy, pk, iy, ix, "%dx%d u=%d CC-SN" % (H, W, u))
+
+
+@pytest.mark.parametrize("ci,n", [(3, 24), (4, 12)])
+def test_single_frame_variants_match_oracle(gpu, oracle_mod, ci, n):
+    """Sequential batch-1 calls select the small-batch cluster variants (8 CTAs at 256x256, 16 CTAs at 512x512);
+    they return the oracle's grid points and the same displacements as the batched variant."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    fr = wl.frames(cfg, np.arange(n))
+    ref = wl.reference(cfg)
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+    info = plan.info()
+    assert info["lat_cluster_size"] > info["cluster_size"]
+    d = plan.device_frames(fr)
+    big = np.concatenate([fr] * (info["lat_max_clusters"] // n + 2))           # more frames than the latency variant takes
+    bx, by, _ = [t.cpu().numpy()[:n] for t in plan.track(plan.device_frames(big))]
+    s = np.array([[t.item() for t in plan.track(d[i], 1)] for i in range(n)], dtype=np.float32)
+    plan.close()
+    o = oracle_mod.track(fr, ref, cfg.upsample)
+    assert np.array_equal(s[:, 0], bx) and np.array_equal(s[:, 1], by)
+    assert np.max(np.abs(s[:, 0] - o.dx)) <= TOL_PX and np.max(np.abs(s[:, 1] - o.dy)) <= TOL_PX
+    assert np.max(np.abs(s[:, 2] / o.peak - 1)) <= TOL_PEAK
