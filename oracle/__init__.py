@@ -76,6 +76,8 @@ def _load():
                                      ctypes.c_double, ctypes.POINTER(_Result), ctypes.c_int]
         lib.cco_drift_correct.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float), ctypes.c_int,
                                           ctypes.c_double, ctypes.c_double, dp, dp, dp]
+        lib.cco_track_rt.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.POINTER(ctypes.c_float), ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
         lib.cco_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -241,3 +243,28 @@ def drift_correct(dx, dy, a0: float, max_step: float = 0.0, state=None):
     if rc:
         raise ValueError("oracle cco_drift_correct failed: %d" % rc)
     return ox, oy, st
+
+
+_RES_DT = np.dtype([("dy", "f8"), ("dx", "f8"), ("peak", "f8"), ("wy", "i4"), ("wx", "i4"), ("m", "i4"), ("n", "i4"),
+                    ("cc_top1", "f8"), ("cc_top2", "f8"), ("up_top1", "f8"), ("up_top2", "f8")], align=True)
+
+
+def track_rt(frames, reference, u: int, a0: float):
+    """PAPER.md:L102-108, Eq. (9): sequential tracking with the running reference image.  Returns
+    (TrackResult, G) with G the complex spectrum (H, W) of the last reference image."""
+    frames = np.ascontiguousarray(frames)
+    if frames.ndim == 2:
+        frames = frames[None]
+    dt = {np.dtype(np.uint8): 0, np.dtype(np.uint16): 1}[frames.dtype]
+    B, H, W = frames.shape
+    ref = np.ascontiguousarray(reference, dtype=np.float32)
+    out = (_Result * max(B, 1))()
+    gr, gi = np.empty((H, W)), np.empty((H, W))
+    rc = _load().cco_track_rt(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                              ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(a0), out, _d(gr), _d(gi))
+    if rc:
+        raise RuntimeError("oracle cco_track_rt failed: %d" % rc)
+    arr = np.frombuffer(out, dtype=_RES_DT)[:B]
+    res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
+                                                "up_top1", "up_top2")))
+    return res, gr + 1j * gi

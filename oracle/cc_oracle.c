@@ -481,3 +481,86 @@ int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double
     state[0] = Rx; state[1] = Ry;
     return 0;
 }
+
+/* Real-time analysis with a running reference image, Eq. (9):
+ *     F[E_i] = a0 F[I_i(r - r0)] + b1 F[E_{i-1}],   b1 = 1 - a0,
+ * "I(r - r0)" being the new image translated by its detected displacement so that it lines up with the RI
+ * (Eq. (1)).  With this build's sign (frame(r) ~ reference(r - d), R1) the aligned
+ * image is J(r) = I(r + d), i.e. F[J](k) = F[I](k) exp(+2 pi i (fy dy / H + fx dx / W)) with signed
+ * frequencies; d is fractional, and on the Nyquist bins (even H, W) the real minimal-bandwidth interpolant
+ * multiplies by cos(pi d) instead (R18).  Frames are processed strictly in order: frame i is
+ * measured against E_{i-1} (the RI given by the caller is E_{-1}), then E_i is formed.  CC-U only.
+ * G_re/G_im (H*W each, may be NULL) receive the spectrum of the last RI. */
+int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
+                 const float *reference, double a0, cco_result *out, double *G_out_re, double *G_out_im)
+{
+    if (!frames || !reference || !out || batch < 0 || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) ||
+        !(a0 >= 0.0 && a0 <= 1.0))
+        return -2;
+    const size_t n = (size_t)H * W;
+    const double b1 = 1.0 - a0;
+    double *buf = (double *)malloc(sizeof(double) * n * 10);
+    if (!buf) return -1;
+    double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
+           *P_re = buf + 6 * n, *P_im = buf + 7 * n, *cc = buf + 8 * n, *cc_im = buf + 9 * n;
+    for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    int rc = cco_dft2_real(E, H, W, G_re, G_im);
+    for (int b = 0; b < batch && !rc; ++b) {
+        if (dtype == 0) {
+            const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
+            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+        } else {
+            const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
+            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+        }
+        rc = cco_dft2_real(I, H, W, F_re, F_im);
+        conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);
+        if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);
+        cco_result r;
+        memset(&r, 0, sizeof r);
+        long idx;
+        top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
+        int y0 = (int)(idx / W), x0 = (int)(idx % W);
+        r.wy = (2 * y0 >= H) ? y0 - H : y0;
+        r.wx = (2 * x0 >= W) ? x0 - W : x0;
+        if (u == 1) {
+            r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
+            r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
+        } else {
+            int M = cco_grid_size(u), c = M / 2;
+            if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL, &r.m, &r.n, &r.up_top1, &r.up_top2);
+            r.dy = (double)r.wy + (double)(r.m - c) / (double)u;
+            r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
+            r.peak = r.up_top1;
+        }
+        out[b] = r;
+        /* Eq. (9): G <- a0 F[I(r + d)] + b1 G */
+        for (int ky = 0; ky < H; ++ky) {
+            double wyr, wyi;
+            if (H % 2 == 0 && 2 * ky == H) { wyr = cos(M_PI * r.dy); wyi = 0.0; }
+            else {
+                double fy = (2 * ky < H) ? ky : (double)ky - H;
+                wyr = cos(2.0 * M_PI * fy * r.dy / H); wyi = sin(2.0 * M_PI * fy * r.dy / H);
+            }
+            for (int kx = 0; kx < W; ++kx) {
+                double wxr, wxi;
+                if (W % 2 == 0 && 2 * kx == W) { wxr = cos(M_PI * r.dx); wxi = 0.0; }
+                else {
+                    double fx = (2 * kx < W) ? kx : (double)kx - W;
+                    wxr = cos(2.0 * M_PI * fx * r.dx / W); wxi = sin(2.0 * M_PI * fx * r.dx / W);
+                }
+                const double wr = wyr * wxr - wyi * wxi, wi = wyr * wxi + wyi * wxr;
+                const size_t k = (size_t)ky * W + kx;
+                const double sr = F_re[k] * wr - F_im[k] * wi, si = F_re[k] * wi + F_im[k] * wr;
+                G_re[k] = a0 * sr + b1 * G_re[k];
+                G_im[k] = a0 * si + b1 * G_im[k];
+            }
+        }
+    }
+    if (!rc && G_out_re && G_out_im) {
+        memcpy(G_out_re, G_re, sizeof(double) * n);
+        memcpy(G_out_im, G_im, sizeof(double) * n);
+    }
+    free(buf);
+    return rc ? -1 : 0;
+}

@@ -113,6 +113,13 @@ int cco_track_sn(const void *frames, int dtype, int batch, int H, int W, int u,
 int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double max_step,
                       double state[2], double *out_dx, double *out_dy);
 
+/* Real-time analysis, Eq. (9): frames in order, frame i measured against the running RI
+ * E_{i-1} (reference = E_{-1}), then F[E_i] = a0 F[I_i aligned] + (1 - a0) F[E_{i-1}], the aligned image being
+ * I_i(r + d_i) by the Fourier shift theorem (cos(pi d) on the Nyquist bins; R18).  CC-U.  G_out_re/im
+ * (H*W each, may be NULL): spectrum of the last RI.  Sequential (no OpenMP). */
+int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
+                 const float *reference, double a0, cco_result *out, double *G_out_re, double *G_out_im);
+
 int cco_num_threads(void);
 
 #ifdef __cplusplus

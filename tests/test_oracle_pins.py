@@ -485,3 +485,66 @@ def test_d3_state_carries_across_calls_and_linearity(oracle_mod):
         assert np.array_equal(np.concatenate([h1[0], h2[0]]), full[0]) and np.array_equal(h2[2], full[2])
     p = oracle_mod.drift_correct(2 * x, 2 * y, 0.02)[0]                       # plain filter is linear
     assert np.allclose(p, 2 * oracle_mod.drift_correct(x, y, 0.02)[0], rtol=1e-12, atol=1e-15)
+
+
+# ---------------------------------------------------------------- real-time RI update (Eq. (9))
+def test_ri1_a0_zero_is_the_fixed_reference(oracle_mod):
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr, ref = wl.frames(cfg, np.arange(6)), wl.reference(cfg)
+    a = oracle_mod.track(fr, ref, 20)
+    b, G = oracle_mod.track_rt(fr, ref, 20, 0.0)
+    assert np.array_equal(a.dx, b.dx) and np.array_equal(a.dy, b.dy) and np.array_equal(a.peak, b.peak)
+    assert np.allclose(G, np.fft.fft2(ref.astype(np.float64)), rtol=1e-10, atol=1e-6)
+
+
+def test_ri2_aligned_copies_leave_the_reference_unchanged(oracle_mod):
+    """Frames that are exact translations of the RI (integer circular shifts; fractional shifts of a band-limited
+    image by the phase ramp) are shifted back onto it: E_i = a0 E + b1 E = E for every a0.  Fails if the sign of the
+    alignment, the Nyquist rule or the filter weights are wrong."""
+    rng = _rng(41)
+    H, W = 16, 24
+    ref = rng.integers(0, 200, size=(H, W)).astype(np.float32)
+    shifts = [(3, -5), (0, 7), (-6, 0), (8, 12), (1, 1)]
+    fr = np.stack([np.roll(ref, s, axis=(0, 1)) for s in shifts]).astype(np.uint16)
+    res, G = oracle_mod.track_rt(fr, ref, 4, 0.3)
+    G0 = np.fft.fft2(ref.astype(np.float64))
+    assert np.max(np.abs(G - G0)) < 1e-9 * np.max(np.abs(G0))
+    for k, (a, b) in enumerate(shifts):
+        assert (res.dy[k], res.dx[k]) == (a - H if 2 * a >= H else a, b - W if 2 * b >= W else b)
+    # fractional: band-limited reference (Nyquist row/column removed), frames = phase-ramp shifts on the 1/u grid
+    u = 8
+    B0 = np.fft.fft2(rng.standard_normal((H, W)))
+    B0[H // 2, :] = 0
+    B0[:, W // 2] = 0
+    base = np.real(np.fft.ifft2(B0))
+    fy, fx = np.fft.fftfreq(H)[:, None], np.fft.fftfreq(W)[None, :]
+    scale = 2000.0 / np.abs(base).max()
+    ref2 = np.round(base * scale) + 3000.0                                # integer pixels: quantisation breaks exact
+    frames2 = []                                                           # band-limitedness by ~1e-4 relative
+    for dy, dx in [(0.375, -0.25), (-1.5, 2.125)]:
+        sh = np.real(np.fft.ifft2(np.fft.fft2(ref2) * np.exp(-2j * np.pi * (fy * dy + fx * dx))))
+        frames2.append(np.round(sh))
+    fr2 = np.stack(frames2).astype(np.uint16)
+    res2, G2 = oracle_mod.track_rt(fr2, ref2.astype(np.float32), u, 0.5)
+    assert np.allclose(res2.dy, [0.375, -1.5]) and np.allclose(res2.dx, [-0.25, 2.125])
+    Gr = np.fft.fft2(ref2)
+    err = np.max(np.abs(G2 - Gr))                                          # only the +-0.5 rounding of the pixels remains:
+    assert err < 5 * np.sqrt(H * W / 12.0) and err < 1e-2 * np.median(np.abs(Gr))   # ~sqrt(HW/12) per bin, << |G|
+
+
+def test_ri3_filter_weights_closed_form(oracle_mod):
+    """Frames with zero displacement (the RI plus zero-mean noise): no alignment phase, so
+    G_n = b1^(n+1) G_ref + a0 sum_k b1^(n-k) F[I_k] -- the low-pass filter of Eq. (9) written out."""
+    rng = _rng(42)
+    H = W = 16
+    y, x = np.mgrid[0:H, 0:W]
+    ref = (500.0 * np.exp(-((y - 8) ** 2 + (x - 8) ** 2) / 8.0) + 20.0).astype(np.float32)
+    fr = np.clip(np.round(ref[None] + rng.normal(0, 1.0, size=(5, H, W))), 0, 65535).astype(np.uint16)
+    a0 = 0.25
+    res, G = oracle_mod.track_rt(fr, ref, 2, a0)
+    assert np.all(res.dx == 0) and np.all(res.dy == 0)
+    expect = (1 - a0) ** 5 * np.fft.fft2(ref.astype(np.float64))
+    for k in range(5):
+        expect = expect + a0 * (1 - a0) ** (4 - k) * np.fft.fft2(fr[k].astype(np.float64))
+    assert np.max(np.abs(G - expect)) < 1e-9 * np.max(np.abs(expect))
