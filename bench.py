@@ -450,6 +450,18 @@ def main():
                 rt.latency_probe(d2.data_ptr(), min(100, nlat))
                 rx, ry, _, lat_rt = rt.latency_probe(d2.data_ptr(), nlat)
                 leg["rt_session"] = stat(lat_rt)
+                if ci == 2:  # the paper's full real-time loop: running reference image, Eq. (9), inside the session
+                    rt.close()
+                    rt = None
+                    p2.enable_reference_update(0.02)
+                    rt = RtSession(p2, 1000)
+                    rt.latency_probe(d2.data_ptr(), min(100, nlat))
+                    leg["rt_session_with_reference_update"] = stat(rt.latency_probe(d2.data_ptr(), nlat)[3])
+                    rt.close()
+                    rt = None
+                    p2.close()
+                    p2 = Plan(c2.H, c2.W, f2.dtype, c2.upsample, wl.reference(c2))
+                    rt = RtSession(p2, 1000)
                 h2 = torch.from_numpy(f2.view(np.uint8).reshape(nlat, -1)).pin_memory()
                 rt.latency_probe(h2.data_ptr(), min(100, nlat))
                 leg["rt_session_frame_in_pinned_host_memory"] = stat(rt.latency_probe(h2.data_ptr(), nlat)[3])

@@ -206,6 +206,23 @@ cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, f
                               double *lat_us);
 
 /*
+ * cc_plan_enable_reference_update -- the paper's real-time analysis (Eq. (9)): after every
+ * frame the plan's reference image is replaced by  F[E_i] = a0 F[I_i aligned] + (1 - a0) F[E_{i-1}],  the aligned
+ * image being the frame translated by its detected displacement (Fourier shift theorem; cos(pi d) on the Nyquist
+ * bins -- DESIGN.md R18).  a0 = 1 - exp(-T/tau) in (0, 1]; a0 == 0 switches the update off again.  CC-U plans only
+ * (CC_ERR_UNSUPPORTED otherwise).  Frames are then processed strictly in order by ONE cluster (the largest-cluster
+ * variant of the shape): frame i of a cc_track batch is measured against the reference left by frame i-1, and
+ * consecutive cc_track / cc_rt_track calls continue the sequence.  cc_track thereby MODIFIES the plan: calls on
+ * one plan must be serialised (same stream).  May synchronise the device.
+ *
+ * cc_plan_get_reference_spectrum -- debugging / checkpoint aid: the spectrum F[E] the plan currently holds.
+ *   out   HOST pointer, H * (W/2 + 1) complex float32 (re, im interleaved), row ky, column kx = 0..W/2,
+ *         natural frequency order, unnormalised (sum over pixels).  Synchronises the device.
+ */
+cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0);
+cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *out);
+
+/*
  * cc_drift_correct -- PAPER.md:L110-127: removes the slowly drifting equilibrium position from a sequence of
  * displacements, r'_n = r_n - R_n, with the low-pass offset of Eq. (10), R_n = a0 r_n + b1 R_{n-1}
  * (b1 = 1 - a0; R_{-1} = 0, so R_0 = a0 r_0), or, when max_step > 0, its rate-limited form of Eqs. (11)-(12):

@@ -20,7 +20,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
+           "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -78,6 +78,10 @@ def load_library() -> ctypes.CDLL:
         lib.cc_rt_close.restype = ci
         lib.cc_rt_latency_probe.argtypes = [vp, vp, ci, vp, vp, vp, vp]
         lib.cc_rt_latency_probe.restype = ci
+        lib.cc_plan_enable_reference_update.argtypes = [vp, ctypes.c_double]
+        lib.cc_plan_enable_reference_update.restype = ci
+        lib.cc_plan_get_reference_spectrum.argtypes = [vp, vp]
+        lib.cc_plan_get_reference_spectrum.restype = ci
         lib.cc_plan_destroy.argtypes = [vp]
         lib.cc_plan_destroy.restype = ci
         lib.cc_plan_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
@@ -137,6 +141,16 @@ class Plan:
             self._h = None
 
     __del__ = close
+
+    def enable_reference_update(self, a0: float):
+        """cc_plan_enable_reference_update: running reference image of PAPER.md Eq. (9); a0 = 0 switches it off."""
+        _check(load_library().cc_plan_enable_reference_update(self._h, float(a0)))
+
+    def reference_spectrum(self) -> np.ndarray:
+        """cc_plan_get_reference_spectrum: complex64 (H, W/2 + 1), the spectrum F[E] the plan currently holds."""
+        out = np.empty((self.H, self.W // 2 + 1), np.complex64)
+        _check(load_library().cc_plan_get_reference_spectrum(self._h, out.ctypes.data_as(ctypes.c_void_p)))
+        return out
 
     def info(self) -> dict:
         inf = PlanInfo()

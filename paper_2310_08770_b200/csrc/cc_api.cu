@@ -76,6 +76,12 @@ struct cc_plan {
     float4 *ab = nullptr;
     double2 *tw64 = nullptr, *Xpol = nullptr;  // fp64 tables of the argmax polish steps
     double *Dpol = nullptr, *nyq64 = nullptr;
+    // running reference image (Eq. (9)): scratch spectrum of the current frame, running mean, slot -> frequency table
+    float2 *ri_Fs = nullptr;
+    float4 *ri_Fab = nullptr;
+    double *ri_emean = nullptr;
+    int16_t *col_freq = nullptr;
+    double ri_a0 = 0.0;
     size_t table_bytes = 0;
     VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
     bool has_lat = false;
@@ -319,6 +325,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     cudaFree(plan->tw), cudaFree(plan->Gt), cudaFree(plan->row_slot), cudaFree(plan->col_partner);
     cudaFree(plan->ab);
     cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
+    cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab), cudaFree(plan->ri_emean), cudaFree(plan->col_freq);
     for (VarPlan *vp : {&plan->thr, &plan->lat}) cudaFree(vp->Sg), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
@@ -513,6 +520,9 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
     p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.Emean = pl->Emean;
+    if (pl->ri_a0 > 0.0) {
+        p.ri_Fs = pl->ri_Fs, p.ri_Fab = pl->ri_Fab, p.ri_emean = pl->ri_emean, p.col_freq = pl->col_freq, p.ri_a0 = pl->ri_a0;
+    }
     p.sn = pl->sn, p.sn_eps = pl->sn_eps, p.sn_c0 = pl->sn_c0, p.peak_sign = pl->sn ? -1.0 : 1.0;
 }
 
@@ -524,12 +534,13 @@ static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, 
     if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track: null pointer");
     if (((uintptr_t)frames & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_track: frames must be 16-byte aligned");
     const VarPlan *vp = &plan->thr;
-    if (plan->has_lat && batch <= plan->lat.max_clusters && batch * plan->lat.v.CS <= plan->thr.max_clusters * plan->thr.v.CS)
+    const bool ri = plan->ri_a0 > 0.0;  // running reference image: frames strictly in order, one cluster
+    if (plan->has_lat && (ri || (batch <= plan->lat.max_clusters && batch * plan->lat.v.CS <= plan->thr.max_clusters * plan->thr.v.CS)))
         vp = &plan->lat;
     CcParams p{};
     fill_params(plan, *vp, p);
     p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix, p.phase_clk = phase_clk;
-    const int ncl = std::min(batch, vp->max_clusters);
+    const int ncl = ri ? 1 : std::min(batch, vp->max_clusters);
     cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
     return CC_OK;
@@ -791,6 +802,62 @@ extern "C" cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, f
         cc_status s = cc_rt_track(rt, (const unsigned char *)frames + (size_t)i * fbytes, dx + i, dy + i, peak ? peak + i : nullptr);
         lat_us[i] = mono_us() - t0;
         if (s != CC_OK) return s;
+    }
+    return CC_OK;
+}
+
+// ------------------------------------------------------------------ running reference image
+extern "C" cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0)
+{
+    if (!plan || !(a0 >= 0.0 && a0 <= 1.0)) return fail(CC_ERR_INVALID_ARG, "cc_plan_enable_reference_update: bad plan or a0");
+    if (plan->sn) return fail(CC_ERR_UNSUPPORTED, "the reference update of Eq. (9) is built for CC-U plans only");
+    CK(cudaDeviceSynchronize());
+    if (a0 == 0.0) {
+        plan->ri_a0 = 0.0;
+        return CC_OK;
+    }
+    const int H = plan->H, W = plan->W;
+    if (!plan->ri_Fs) {
+        std::vector<int16_t> cf(H);
+        for (int p = 0; p < H; ++p) {
+            const int ky = cc_freq_of_slot(H, p, false);
+            cf[p] = (int16_t)(2 * ky < H ? ky : ky - H);  // Nyquist slot: -H/2
+        }
+        cudaError_t e = upload(&plan->col_freq, cf, &plan->table_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_Fs, (size_t)H * (W / 2) * sizeof(float2));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_Fab, (size_t)H * sizeof(float4));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_emean, sizeof(double));
+        if (e == cudaSuccess) e = cudaMemset(plan->ri_Fs, 0, (size_t)H * (W / 2) * sizeof(float2));
+        if (e == cudaSuccess) e = cudaMemcpy(plan->ri_emean, &plan->Emean, sizeof(double), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "reference-update setup");
+    }
+    plan->ri_a0 = a0;
+    return CC_OK;
+}
+
+extern "C" cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *out)
+{
+    if (!plan || !out) return fail(CC_ERR_INVALID_ARG, "cc_plan_get_reference_spectrum: null pointer");
+    const int H = plan->H, W = plan->W, Wh = W / 2;
+    CK(cudaDeviceSynchronize());
+    std::vector<float2> Gt((size_t)H * Wh);
+    std::vector<float4> ab(H);
+    double emean = plan->Emean;
+    CK(cudaMemcpy(Gt.data(), plan->Gt, Gt.size() * sizeof(float2), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ab.data(), plan->ab, ab.size() * sizeof(float4), cudaMemcpyDeviceToHost));
+    if (plan->ri_emean) CK(cudaMemcpy(&emean, plan->ri_emean, sizeof(double), cudaMemcpyDeviceToHost));
+    const double HW = (double)H * (double)W;
+    for (int p = 0; p < H; ++p) {
+        const int ky = cc_freq_of_slot(H, p, false);
+        float *row = out + (size_t)ky * (Wh + 1) * 2;
+        for (int q = 1; q < Wh; ++q) {  // stored: conj(G) / (HW)
+            row[2 * q] = (float)((double)Gt[(size_t)p * Wh + q].x * HW);
+            row[2 * q + 1] = (float)(-(double)Gt[(size_t)p * Wh + q].y * HW);
+        }
+        row[0] = ky == 0 ? (float)(emean * HW) : (float)((double)ab[p].x * HW);  // the DC bin is kept as the mean
+        row[1] = ky == 0 ? 0.f : (float)(-(double)ab[p].y * HW);
+        row[2 * Wh] = (float)((double)ab[p].z * HW);
+        row[2 * Wh + 1] = (float)(-(double)ab[p].w * HW);
     }
     return CC_OK;
 }

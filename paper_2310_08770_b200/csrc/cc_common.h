@@ -99,6 +99,14 @@ struct CcParams {
     int *rt_alive;                              // cleared by the kernel when it exits
     unsigned long long rt_timeout_ns;           // the kernel exits after this long without a command
 
+    // running reference image (Eq. (9)); ri_Fs == null outside that mode.  The kernel then
+    // reads Gt / ab / the reference mean through L2 (ld.cg) and rewrites them after every frame.
+    float2 *ri_Fs;             // [H][W/2] forward spectrum of the current frame, column-slot order (scratch)
+    float4 *ri_Fab;            // [H] (DC column, Nyquist column) of the current frame's spectrum, by slot
+    double *ri_emean;          // mean of the running reference image
+    const int16_t *col_freq;   // [H] signed row frequency ky of column-FFT slot p (-H/2 at the Nyquist slot)
+    double ri_a0;              // a0 = 1 - exp(-T/tau); b1 = 1 - a0
+
     int u, M, c;        // upsample factor, grid size ceil(1.5 u), centre floor(M/2)
     int nd;             // c + 1: number of |offsets| d (and e) evaluated per axis
     int DS;             // offsets d owned per CTA per super-block (T holds 2*DS rows)

@@ -612,6 +612,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     // results of one frame (rank 0, thread 0): batch arrays, or the session's mapped host record
     const bool RT = p.rt_cmd != nullptr;
+    const bool RI = p.ri_Fs != nullptr;  // running reference image (Eq. (9))
     uint64_t rt_seq = 0;    // sequence number of the command being served
     uint32_t cph = 0;       // phase parity of the command barrier
     auto emit = [&](int f, float dyv, float dxv, float pkv, int wyv, int wxv) {
@@ -627,6 +628,55 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             if (p.iy) p.iy[f] = wyv;
             if (p.ix) p.ix[f] = wxv;
         }
+    };
+
+    // ---- running reference image, Eq. (9): F[E_i] = a0 F[I_i(r + d_i)] + b1 F[E_{i-1}] (R18).  d = (ny, nx) / u.
+    // In the plan's storage (conj(G)/(HW), column-slot order): Gt <- b1 Gt + (a0/HW) conj(F exp(i theta)),
+    // theta = 2 pi (fy ny / (u H) + kx nx / (u W)); cos(pi d) replaces the phase factor on the Nyquist row / column.
+    // Every CTA rewrites exactly the columns it reads in the product, so no cluster barrier is involved.
+    auto ri_update = [&](long long ny, long long nx) {
+        const double a0 = p.ri_a0, b1 = 1.0 - a0;
+        const float b1f = (float)b1, scf = (float)(a0 / ((double)H * (double)W));
+        const long long den = (long long)u * H * W;
+        const double cnx = cospi((double)(((nx % (2LL * u)) + 2LL * u) % (2LL * u)) / (double)u);  // cos(pi dx)
+        const double cny = cospi((double)(((ny % (2LL * u)) + 2LL * u) % (2LL * u)) / (double)u);  // cos(pi dy)
+        auto phase = [&](int fy, int kx) -> float2 {  // exp(i theta), the y factor real (cos(pi dy)) at the Nyquist row
+            const bool nyq = (2 * fy == -H);
+            long long num = ((nyq ? 0LL : (long long)fy * ny * W) + (long long)kx * nx * H) % den;
+            if (num < 0) num += den;
+            double sn, cs;
+            sincospi(2.0 * (double)num / (double)den, &sn, &cs);
+            if (nyq) cs *= cny, sn *= cny;
+            return make_float2((float)cs, (float)sn);
+        };
+        for (int idx = tid; idx < H * NC; idx += NT) {
+            const int ps = idx / NC, q = rank * NC + idx % NC;
+            if (q == 0) continue;
+            const size_t gi = (size_t)ps * (W / 2) + q;
+            const float2 Fv = __ldcg(&p.ri_Fs[gi]), Gv = __ldcg(&p.Gt[gi]);
+            const float2 Fp = cmul(Fv, phase((int)p.col_freq[ps], q));
+            __stcg(const_cast<float2 *>(&p.Gt[gi]), make_float2(fmaf(b1f, Gv.x, scf * Fp.x), fmaf(b1f, Gv.y, -scf * Fp.y)));
+        }
+        if (rank == 0) {
+            for (int ps = tid; ps < H; ps += NT) {
+                const int fy = (int)p.col_freq[ps];
+                const float4 Fv = __ldcg(&p.ri_Fab[ps]), Gv = __ldcg(&p.ab[ps]);
+                const float2 wy = phase(fy, 0);
+                const float2 Fa = cmul(make_float2(Fv.x, Fv.y), wy);
+                const float2 Fb = cmul(make_float2(Fv.z, Fv.w), make_float2(wy.x * (float)cnx, wy.y * (float)cnx));
+                float4 o;
+                o.x = fy == 0 ? 0.f : fmaf(b1f, Gv.x, scf * Fa.x);  // the DC bin of the reference stays zero (R10)
+                o.y = fy == 0 ? 0.f : fmaf(b1f, Gv.y, -scf * Fa.y);
+                o.z = fmaf(b1f, Gv.z, scf * Fb.x);
+                o.w = fmaf(b1f, Gv.w, -scf * Fb.y);
+                __stcg(const_cast<float4 *>(&p.ab[ps]), o);
+            }
+            if (tid == 0) {
+                const double mean_i = ((double)*f00 + c0d * H * W) / ((double)H * (double)W);
+                __stcg(p.ri_emean, b1 * __ldcg(p.ri_emean) + a0 * mean_i);
+            }
+        }
+        __threadfence();
     };
 
     for (int f = cid; RT || f < p.batch; f += ncl) {
@@ -767,7 +817,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 } else {
                     float2 w[RL];
 #pragma unroll
-                    for (int k = 0; k < RL; ++k) w[k] = cmul(v[brev(k, bits)], __ldg(&p.Gt[(size_t)(g * RL + k) * (W / 2) + q]));
+                    for (int k = 0; k < RL; ++k) {
+                        const size_t gi = (size_t)(g * RL + k) * (W / 2) + q;
+                        if (RI) __stcg(&p.ri_Fs[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
+                        w[k] = cmul(v[brev(k, bits)], RI ? __ldcg(&p.Gt[gi]) : __ldg(&p.Gt[gi]));
+                    }
                     dft_reg<RL, true>(w);
 #pragma unroll
                     for (int n = 0; n < RL; ++n) Sl[(size_t)(g * RL + n) * NC + ql] = w[brev(n, bits)];
@@ -785,9 +839,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     const int s = tid + e * NT;
                     if (s < H) {
                         const float2 z = Sl[(size_t)s * NC], zp = Sl[(size_t)p.col_partner[s] * NC];
-                        const float4 g = p.ab[s];  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
+                        const float4 g = RI ? __ldcg(&p.ab[s]) : p.ab[s];  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
+                        if (RI) __stcg(&p.ri_Fab[s], make_float4(fa.x, fa.y, fb.x, fb.y));
                         const float2 pa = cmul(fa, make_float2(g.x, g.y)), pb = cmul(fb, make_float2(g.z, g.w));
                         o[e] = make_float2(pa.x - pb.y, pa.y + pb.x);
                         if (s == 0) *f00 = z.x;  // sum of (I - c0): DC add-back for `peak`
@@ -890,7 +945,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
         if (u == 1) {
             if (rank == 0 && tid == 0) {
-                emit(f, (float)wy, (float)wx, (float)(p.peak_sign * (cc_peak + ((double)*f00 + c0d * H * W) * p.Emean)), wy, wx);
+                const double Em = RI ? __ldcg(p.ri_emean) : p.Emean;
+                emit(f, (float)wy, (float)wx, (float)(p.peak_sign * (cc_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
+            }
+            if (RI) {
+                __syncthreads();  // the reference mean was read before it is rewritten
+                ri_update((long long)wy, (long long)wx);
             }
             csync();
             continue;
@@ -1259,8 +1319,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
         stamp(7, f);
         if (rank == 0 && tid == 0) {
+            const double Em = RI ? __ldcg(p.ri_emean) : p.Emean;
             emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
-                 (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * p.Emean)), wy, wx);
+                 (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
+        }
+        if (RI) {
+            __syncthreads();  // the reference mean was read before it is rewritten
+            ri_update((long long)wy * u + (ms - cM), (long long)wx * u + (ns - cM));
         }
         __syncthreads();  // U (polish scratch) is reused by the next frame's raw ring
     }
