@@ -637,31 +637,46 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     auto ri_update = [&](long long ny, long long nx) {
         const double a0 = p.ri_a0, b1 = 1.0 - a0;
         const float b1f = (float)b1, scf = (float)(a0 / ((double)H * (double)W));
-        const long long den = (long long)u * H * W;
         const double cnx = cospi((double)(((nx % (2LL * u)) + 2LL * u) % (2LL * u)) / (double)u);  // cos(pi dx)
         const double cny = cospi((double)(((ny % (2LL * u)) + 2LL * u) % (2LL * u)) / (double)u);  // cos(pi dy)
-        auto phase = [&](int fy, int kx) -> float2 {  // exp(i theta), the y factor real (cos(pi dy)) at the Nyquist row
-            const bool nyq = (2 * fy == -H);
-            long long num = ((nyq ? 0LL : (long long)fy * ny * W) + (long long)kx * nx * H) % den;
-            if (num < 0) num += den;
+        // exp(i theta) = wy(slot) * wx(kx): H + W/2 phase factors per frame (exactly reduced phase numerators, fp64
+        // sincospi, rounded once) in the free U region instead of one evaluation per spectrum element
+        float2 *const wyt = reinterpret_cast<float2 *>(U), *const wxt = wyt + H;
+        for (int i = tid; i < H + W / 2; i += NT) {
             double sn, cs;
-            sincospi(2.0 * (double)num / (double)den, &sn, &cs);
-            if (nyq) cs *= cny, sn *= cny;
-            return make_float2((float)cs, (float)sn);
-        };
+            if (i < H) {
+                const int fy = (int)p.col_freq[i];
+                if (2 * fy == -H) {  // Nyquist row: the real interpolant multiplies by cos(pi dy)
+                    cs = cny, sn = 0.0;
+                } else {
+                    const long long dy_den = (long long)u * H;
+                    long long num = ((long long)fy * ny) % dy_den;
+                    if (num < 0) num += dy_den;
+                    sincospi(2.0 * (double)num / (double)dy_den, &sn, &cs);
+                }
+                wyt[i] = make_float2((float)cs, (float)sn);
+            } else {
+                const long long dx_den = (long long)u * W;
+                long long num = ((long long)(i - H) * nx) % dx_den;
+                if (num < 0) num += dx_den;
+                sincospi(2.0 * (double)num / (double)dx_den, &sn, &cs);
+                wxt[i - H] = make_float2((float)cs, (float)sn);
+            }
+        }
+        __syncthreads();
         for (int idx = tid; idx < H * NC; idx += NT) {
             const int ps = idx / NC, q = rank * NC + idx % NC;
             if (q == 0) continue;
             const size_t gi = (size_t)ps * (W / 2) + q;
             const float2 Fv = __ldcg(&p.ri_Fs[gi]), Gv = __ldcg(&p.Gt[gi]);
-            const float2 Fp = cmul(Fv, phase((int)p.col_freq[ps], q));
+            const float2 Fp = cmul(Fv, cmul(wyt[ps], wxt[q]));
             __stcg(const_cast<float2 *>(&p.Gt[gi]), make_float2(fmaf(b1f, Gv.x, scf * Fp.x), fmaf(b1f, Gv.y, -scf * Fp.y)));
         }
         if (rank == 0) {
             for (int ps = tid; ps < H; ps += NT) {
                 const int fy = (int)p.col_freq[ps];
                 const float4 Fv = __ldcg(&p.ri_Fab[ps]), Gv = __ldcg(&p.ab[ps]);
-                const float2 wy = phase(fy, 0);
+                const float2 wy = wyt[ps];
                 const float2 Fa = cmul(make_float2(Fv.x, Fv.y), wy);
                 const float2 Fb = cmul(make_float2(Fv.z, Fv.w), make_float2(wy.x * (float)cnx, wy.y * (float)cnx));
                 float4 o;
@@ -820,7 +835,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     for (int k = 0; k < RL; ++k) {
                         const size_t gi = (size_t)(g * RL + k) * (W / 2) + q;
                         if (RI) __stcg(&p.ri_Fs[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
-                        w[k] = cmul(v[brev(k, bits)], RI ? __ldcg(&p.Gt[gi]) : __ldg(&p.Gt[gi]));
+                        w[k] = cmul(v[brev(k, bits)], __ldcg(&p.Gt[gi]));  // through L2: the RI update rewrites Gt
                     }
                     dft_reg<RL, true>(w);
 #pragma unroll
@@ -839,7 +854,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     const int s = tid + e * NT;
                     if (s < H) {
                         const float2 z = Sl[(size_t)s * NC], zp = Sl[(size_t)p.col_partner[s] * NC];
-                        const float4 g = RI ? __ldcg(&p.ab[s]) : p.ab[s];  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
+                        const float4 g = __ldcg(&p.ab[s]);  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
                         if (RI) __stcg(&p.ri_Fab[s], make_float4(fa.x, fa.y, fb.x, fb.y));
