@@ -78,6 +78,8 @@ def _load():
                                           ctypes.c_double, ctypes.c_double, dp, dp, dp]
         lib.cco_track_rt.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.POINTER(ctypes.c_float), ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
+        lib.cco_iterate_reference.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                              ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.POINTER(_Result), dp, dp]
         lib.cco_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -264,6 +266,24 @@ def track_rt(frames, reference, u: int, a0: float):
                               ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(a0), out, _d(gr), _d(gi))
     if rc:
         raise RuntimeError("oracle cco_track_rt failed: %d" % rc)
+    arr = np.frombuffer(out, dtype=_RES_DT)[:B]
+    res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
+                                                "up_top1", "up_top2")))
+    return res, gr + 1j * gi
+
+
+def iterate_reference(frames, reference, u: int, n_iter: int):
+    """PAPER.md:L94-100, Eq. (8): n_iter passes of the offline analysis.  Returns (TrackResult of the last pass, G)."""
+    frames = np.ascontiguousarray(frames)
+    dt = {np.dtype(np.uint8): 0, np.dtype(np.uint16): 1}[frames.dtype]
+    B, H, W = frames.shape
+    ref = np.ascontiguousarray(reference, dtype=np.float32)
+    out = (_Result * B)()
+    gr, gi = np.empty((H, W)), np.empty((H, W))
+    rc = _load().cco_iterate_reference(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                       ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), int(n_iter), out, _d(gr), _d(gi))
+    if rc:
+        raise RuntimeError("oracle cco_iterate_reference failed: %d" % rc)
     arr = np.frombuffer(out, dtype=_RES_DT)[:B]
     res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
                                                 "up_top1", "up_top2")))

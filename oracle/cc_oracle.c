@@ -564,3 +564,84 @@ int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
     free(buf);
     return rc ? -1 : 0;
 }
+
+/* Offline analysis, Eq. (8): for each complete pass through the images,
+ *     F[E_n] = (1/N) sum_i F[I_i(r - r0_i)],
+ * every displacement r0_i of the pass being measured against the constant RI E_{n-1}; the aligned image is
+ * I_i(r + d_i) as in cco_track_rt (R18).  n_iter passes are made, starting from the caller's reference
+ * (the paper starts from E_0 = I_0: pass the first frame).  `out` receives the displacements measured in the LAST
+ * pass (against E_{n_iter-1}), G_out the spectrum of E_{n_iter}.  CC-U.  Sequential. */
+int cco_iterate_reference(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
+                          int n_iter, cco_result *out, double *G_out_re, double *G_out_im)
+{
+    if (!frames || !reference || !out || batch <= 0 || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) || n_iter < 1)
+        return -2;
+    const size_t n = (size_t)H * W;
+    double *buf = (double *)malloc(sizeof(double) * n * 12);
+    if (!buf) return -1;
+    double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
+           *P_re = buf + 6 * n, *P_im = buf + 7 * n, *cc = buf + 8 * n, *cc_im = buf + 9 * n, *A_re = buf + 10 * n,
+           *A_im = buf + 11 * n;
+    for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    int rc = cco_dft2_real(E, H, W, G_re, G_im);
+    for (int it = 0; it < n_iter && !rc; ++it) {
+        for (size_t i = 0; i < n; ++i) A_re[i] = A_im[i] = 0.0;
+        for (int b = 0; b < batch && !rc; ++b) {
+            if (dtype == 0) {
+                const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
+                for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+            } else {
+                const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
+                for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+            }
+            rc = cco_dft2_real(I, H, W, F_re, F_im);
+            conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);
+            if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);
+            cco_result r;
+            memset(&r, 0, sizeof r);
+            long idx;
+            top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
+            int y0 = (int)(idx / W), x0 = (int)(idx % W);
+            r.wy = (2 * y0 >= H) ? y0 - H : y0;
+            r.wx = (2 * x0 >= W) ? x0 - W : x0;
+            if (u == 1) {
+                r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
+                r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
+            } else {
+                int M = cco_grid_size(u), c = M / 2;
+                if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL, &r.m, &r.n, &r.up_top1, &r.up_top2);
+                r.dy = (double)r.wy + (double)(r.m - c) / (double)u;
+                r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
+                r.peak = r.up_top1;
+            }
+            out[b] = r;
+            for (int ky = 0; ky < H; ++ky) {          /* A += F[I_b(r + d_b)] */
+                double wyr, wyi;
+                if (H % 2 == 0 && 2 * ky == H) { wyr = cos(M_PI * r.dy); wyi = 0.0; }
+                else {
+                    double fy = (2 * ky < H) ? ky : (double)ky - H;
+                    wyr = cos(2.0 * M_PI * fy * r.dy / H); wyi = sin(2.0 * M_PI * fy * r.dy / H);
+                }
+                for (int kx = 0; kx < W; ++kx) {
+                    double wxr, wxi;
+                    if (W % 2 == 0 && 2 * kx == W) { wxr = cos(M_PI * r.dx); wxi = 0.0; }
+                    else {
+                        double fx = (2 * kx < W) ? kx : (double)kx - W;
+                        wxr = cos(2.0 * M_PI * fx * r.dx / W); wxi = sin(2.0 * M_PI * fx * r.dx / W);
+                    }
+                    const double wr = wyr * wxr - wyi * wxi, wi = wyr * wxi + wyi * wxr;
+                    const size_t k = (size_t)ky * W + kx;
+                    A_re[k] += F_re[k] * wr - F_im[k] * wi;
+                    A_im[k] += F_re[k] * wi + F_im[k] * wr;
+                }
+            }
+        }
+        for (size_t i = 0; i < n; ++i) { G_re[i] = A_re[i] / batch; G_im[i] = A_im[i] / batch; }   /* Eq. (8) */
+    }
+    if (!rc && G_out_re && G_out_im) {
+        memcpy(G_out_re, G_re, sizeof(double) * n);
+        memcpy(G_out_im, G_im, sizeof(double) * n);
+    }
+    free(buf);
+    return rc ? -1 : 0;
+}

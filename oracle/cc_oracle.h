@@ -120,6 +120,12 @@ int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double
 int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
                  const float *reference, double a0, cco_result *out, double *G_out_re, double *G_out_im);
 
+/* Offline analysis, Eq. (8): n_iter complete passes; in each, every frame is measured against the
+ * constant RI of the previous pass and the new RI is the mean of the aligned images, F[E_n] = (1/N) sum_i
+ * F[I_i(r + d_i)] (alignment as in cco_track_rt).  out: displacements of the last pass; G_out: spectrum of E_{n_iter}. */
+int cco_iterate_reference(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
+                          int n_iter, cco_result *out, double *G_out_re, double *G_out_im);
+
 int cco_num_threads(void);
 
 #ifdef __cplusplus

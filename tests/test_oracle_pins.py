@@ -548,3 +548,39 @@ def test_ri3_filter_weights_closed_form(oracle_mod):
     for k in range(5):
         expect = expect + a0 * (1 - a0) ** (4 - k) * np.fft.fft2(fr[k].astype(np.float64))
     assert np.max(np.abs(G - expect)) < 1e-9 * np.max(np.abs(expect))
+
+
+# ---------------------------------------------------------------- offline iterative RI (Eq. (8))
+def test_it1_mean_of_aligned_images(oracle_mod):
+    """Frames = integer circular shifts of one image plus independent noise: after one pass the RI is the plain mean
+    of the frames rolled back by their shifts (np.roll + np.mean, no Fourier arithmetic); a second pass keeps d."""
+    rng = _rng(61)
+    H, W, N = 16, 16, 12
+    y, x = np.mgrid[0:H, 0:W]
+    base = 400.0 * np.exp(-((y - 8) ** 2 + (x - 8) ** 2) / 6.0) + 30.0
+    shifts = rng.integers(-3, 4, size=(N, 2))
+    shifts[0] = 0                                                     # E_0 = I_0 (PAPER.md:L98)
+    fr = np.stack([np.roll(rng.poisson(base), tuple(s), axis=(0, 1)) for s in shifts]).astype(np.uint16)
+    res, G = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 1, 1)
+    assert np.array_equal(res.wy, shifts[:, 0]) and np.array_equal(res.wx, shifts[:, 1])
+    mean = np.mean([np.roll(f.astype(np.float64), tuple(-s), axis=(0, 1)) for f, s in zip(fr, shifts)], axis=0)
+    assert np.max(np.abs(G - np.fft.fft2(mean))) < 1e-9 * np.abs(G[0, 0])
+    res2, G2 = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 1, 2)
+    assert np.array_equal(res2.wy, shifts[:, 0]) and np.max(np.abs(G2 - G)) < 1e-9 * np.abs(G[0, 0])
+
+
+def test_it2_iterations_sharpen_the_reference(oracle_mod):
+    """The point of Eq. (8): starting from one noisy frame, the averaged RI approaches the noiseless spot, and the
+    rms error of the displacements does not get worse from the first pass to the third."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(40))
+    truth = wl.shifts(cfg)[:40]
+    clean = wl.reference(cfg).astype(np.float64)
+    r1, G1 = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 10, 1)
+    r3, G3 = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 10, 3)
+    rel = lambda r: np.hypot((r.dx - r.dx[0]) - (truth[:, 1] - truth[0, 1]), (r.dy - r.dy[0]) - (truth[:, 0] - truth[0, 0]))
+    assert np.sqrt(np.mean(rel(r3) ** 2)) <= np.sqrt(np.mean(rel(r1) ** 2)) + 1e-12
+    # the averaged RI sits at frame 0's position: compare its spectrum modulus with the clean template's
+    noisy = np.abs(np.fft.fft2(fr[0].astype(np.float64)))
+    assert np.sum((np.abs(G3) - np.abs(np.fft.fft2(clean))) ** 2) < 0.2 * np.sum((noisy - np.abs(np.fft.fft2(clean))) ** 2)
