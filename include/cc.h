@@ -223,6 +223,23 @@ cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0);
 cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *out);
 
 /*
+ * Offline analysis -- PAPER.md:L94-100, Eq. (8): the reference image of pass n is the mean of all images of the
+ * data set, each aligned by its displacement against the reference of pass n-1:
+ *     F[E_n] = (1/N) sum_i F[I_i aligned]        (alignment as in cc_plan_enable_reference_update).
+ * cc_track_accumulate   cc_track over a batch (all clusters in parallel: "embarrassingly parallel", L100) that also
+ *                       adds every frame's aligned spectrum to plan-owned per-cluster accumulators.  May be called
+ *                       several times per pass (chunks of a data set).  CC-U plans without the Eq. (9) update.
+ *                       Allocates on first use; arguments as cc_track.
+ * cc_plan_update_reference_from_accumulator
+ *                       ends a pass: reduces the accumulators in a fixed order (deterministic), replaces the plan's
+ *                       reference by the mean over all frames accumulated since the last call and clears them.
+ *                       Enqueues on `stream` (use the stream of the cc_track_accumulate calls).
+ *                       CC_ERR_INVALID_ARG if nothing was accumulated.
+ */
+cc_status cc_track_accumulate(cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak, void *stream);
+cc_status cc_plan_update_reference_from_accumulator(cc_plan *plan, void *stream);
+
+/*
  * cc_drift_correct -- PAPER.md:L110-127: removes the slowly drifting equilibrium position from a sequence of
  * displacements, r'_n = r_n - R_n, with the low-pass offset of Eq. (10), R_n = a0 r_n + b1 R_{n-1}
  * (b1 = 1 - a0; R_{-1} = 0, so R_0 = a0 r_0), or, when max_step > 0, its rate-limited form of Eqs. (11)-(12):

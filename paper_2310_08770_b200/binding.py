@@ -20,7 +20,8 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
-           "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
+           "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_track_accumulate",
+           "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -82,6 +83,10 @@ def load_library() -> ctypes.CDLL:
         lib.cc_plan_enable_reference_update.restype = ci
         lib.cc_plan_get_reference_spectrum.argtypes = [vp, vp]
         lib.cc_plan_get_reference_spectrum.restype = ci
+        lib.cc_track_accumulate.argtypes = [vp, vp, ci, vp, vp, vp, vp]
+        lib.cc_track_accumulate.restype = ci
+        lib.cc_plan_update_reference_from_accumulator.argtypes = [vp, vp]
+        lib.cc_plan_update_reference_from_accumulator.restype = ci
         lib.cc_plan_destroy.argtypes = [vp]
         lib.cc_plan_destroy.restype = ci
         lib.cc_plan_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
@@ -151,6 +156,25 @@ class Plan:
         out = np.empty((self.H, self.W // 2 + 1), np.complex64)
         _check(load_library().cc_plan_get_reference_spectrum(self._h, out.ctypes.data_as(ctypes.c_void_p)))
         return out
+
+    def track_accumulate(self, frames_dev, batch: int | None = None):
+        """cc_track_accumulate (offline analysis, Eq. (8)): cc_track that also sums the aligned spectra."""
+        torch = _torch()
+        fb = self.H * self.W * self.np_dtype.itemsize
+        if batch is None:
+            batch = frames_dev.numel() * frames_dev.element_size() // fb
+        dev = frames_dev.device
+        dx = torch.empty(batch, dtype=torch.float32, device=dev)
+        dy = torch.empty(batch, dtype=torch.float32, device=dev)
+        pk = torch.empty(batch, dtype=torch.float32, device=dev)
+        _check(load_library().cc_track_accumulate(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(),
+                                                  pk.data_ptr(), torch.cuda.current_stream(dev).cuda_stream))
+        return dx, dy, pk
+
+    def update_reference_from_accumulator(self):
+        """cc_plan_update_reference_from_accumulator: the reference becomes the mean of the aligned frames."""
+        torch = _torch()
+        _check(load_library().cc_plan_update_reference_from_accumulator(self._h, torch.cuda.current_stream().cuda_stream))
 
     def info(self) -> dict:
         inf = PlanInfo()

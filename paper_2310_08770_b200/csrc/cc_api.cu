@@ -82,6 +82,13 @@ struct cc_plan {
     double *ri_emean = nullptr;
     int16_t *col_freq = nullptr;
     double ri_a0 = 0.0;
+    int keep_clusters = 0;        // copies of ri_Fs / ri_Fab allocated
+    // offline iteration (Eq. (8)): per-cluster accumulators of the aligned spectra
+    float2 *acc_G = nullptr;
+    float4 *acc_ab = nullptr;
+    double *acc_mean = nullptr;
+    int acc_clusters = 0;
+    long long acc_count = 0;      // frames accumulated since the last reference update
     size_t table_bytes = 0;
     VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
     bool has_lat = false;
@@ -326,6 +333,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     cudaFree(plan->ab);
     cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
     cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab), cudaFree(plan->ri_emean), cudaFree(plan->col_freq);
+    cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
     for (VarPlan *vp : {&plan->thr, &plan->lat}) cudaFree(vp->Sg), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
@@ -520,8 +528,9 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
     p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.Emean = pl->Emean;
+    p.ri_emean = pl->ri_emean;  // null while the reference mean is the host constant Emean
     if (pl->ri_a0 > 0.0) {
-        p.ri_Fs = pl->ri_Fs, p.ri_Fab = pl->ri_Fab, p.ri_emean = pl->ri_emean, p.col_freq = pl->col_freq, p.ri_a0 = pl->ri_a0;
+        p.ri_Fs = pl->ri_Fs, p.ri_Fab = pl->ri_Fab, p.col_freq = pl->col_freq, p.ri_a0 = pl->ri_a0;
     }
     p.sn = pl->sn, p.sn_eps = pl->sn_eps, p.sn_c0 = pl->sn_c0, p.peak_sign = pl->sn ? -1.0 : 1.0;
 }
@@ -807,6 +816,33 @@ extern "C" cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, f
 }
 
 // ------------------------------------------------------------------ running reference image
+// scratch for the frames' forward spectra (one copy per cluster), the slot -> frequency table, the device-resident mean
+static cc_status ensure_spectrum_scratch(cc_plan *plan, int clusters)
+{
+    const int H = plan->H, W = plan->W;
+    cudaError_t e = cudaSuccess;
+    if (!plan->col_freq) {
+        std::vector<int16_t> cf(H);
+        for (int p = 0; p < H; ++p) {
+            const int ky = cc_freq_of_slot(H, p, false);
+            cf[p] = (int16_t)(2 * ky < H ? ky : ky - H);  // Nyquist slot: -H/2
+        }
+        e = upload(&plan->col_freq, cf, &plan->table_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_emean, sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(plan->ri_emean, &plan->Emean, sizeof(double), cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess && clusters > plan->keep_clusters) {
+        cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab);
+        plan->ri_Fs = nullptr, plan->ri_Fab = nullptr, plan->keep_clusters = 0;
+        e = cudaMalloc((void **)&plan->ri_Fs, (size_t)clusters * H * (W / 2) * sizeof(float2));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_Fab, (size_t)clusters * H * sizeof(float4));
+        if (e == cudaSuccess) plan->keep_clusters = clusters;
+    }
+    if (e != cudaSuccess)
+        return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "spectrum scratch setup");
+    return CC_OK;
+}
+
 extern "C" cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0)
 {
     if (!plan || !(a0 >= 0.0 && a0 <= 1.0)) return fail(CC_ERR_INVALID_ARG, "cc_plan_enable_reference_update: bad plan or a0");
@@ -816,21 +852,8 @@ extern "C" cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0)
         plan->ri_a0 = 0.0;
         return CC_OK;
     }
-    const int H = plan->H, W = plan->W;
-    if (!plan->ri_Fs) {
-        std::vector<int16_t> cf(H);
-        for (int p = 0; p < H; ++p) {
-            const int ky = cc_freq_of_slot(H, p, false);
-            cf[p] = (int16_t)(2 * ky < H ? ky : ky - H);  // Nyquist slot: -H/2
-        }
-        cudaError_t e = upload(&plan->col_freq, cf, &plan->table_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_Fs, (size_t)H * (W / 2) * sizeof(float2));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_Fab, (size_t)H * sizeof(float4));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->ri_emean, sizeof(double));
-        if (e == cudaSuccess) e = cudaMemset(plan->ri_Fs, 0, (size_t)H * (W / 2) * sizeof(float2));
-        if (e == cudaSuccess) e = cudaMemcpy(plan->ri_emean, &plan->Emean, sizeof(double), cudaMemcpyHostToDevice);
-        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "reference-update setup");
-    }
+    cc_status st = ensure_spectrum_scratch(plan, 1);
+    if (st != CC_OK) return st;
     plan->ri_a0 = a0;
     return CC_OK;
 }
@@ -859,6 +882,94 @@ extern "C" cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *
         row[2 * Wh] = (float)((double)ab[p].z * HW);
         row[2 * Wh + 1] = (float)(-(double)ab[p].w * HW);
     }
+    return CC_OK;
+}
+
+// ------------------------------------------------------------------ offline iteration (Eq. (8))
+extern "C" cc_status cc_track_accumulate(cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                                         void *stream)
+{
+    if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: bad plan or batch");
+    if (plan->sn) return fail(CC_ERR_UNSUPPORTED, "the offline iteration of Eq. (8) is built for CC-U plans only");
+    if (plan->ri_a0 > 0.0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: switch the Eq. (9) update off first");
+    if (batch == 0) return CC_OK;
+    if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: null pointer");
+    if (((uintptr_t)frames & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: frames must be 16-byte aligned");
+    const VarPlan *vp = &plan->thr;
+    const int H = plan->H, W = plan->W, ncmax = vp->max_clusters;
+    if (plan->acc_clusters < ncmax) {  // first use: may synchronise
+        CK(cudaDeviceSynchronize());
+        cc_status st = ensure_spectrum_scratch(plan, ncmax);
+        if (st != CC_OK) return st;
+        cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
+        plan->acc_G = nullptr, plan->acc_ab = nullptr, plan->acc_mean = nullptr, plan->acc_clusters = 0, plan->acc_count = 0;
+        cudaError_t e = cudaMalloc((void **)&plan->acc_G, (size_t)ncmax * H * (W / 2) * sizeof(float2));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->acc_ab, (size_t)ncmax * H * sizeof(float4));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&plan->acc_mean, (size_t)ncmax * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemset(plan->acc_G, 0, (size_t)ncmax * H * (W / 2) * sizeof(float2));
+        if (e == cudaSuccess) e = cudaMemset(plan->acc_ab, 0, (size_t)ncmax * H * sizeof(float4));
+        if (e == cudaSuccess) e = cudaMemset(plan->acc_mean, 0, (size_t)ncmax * sizeof(double));
+        if (e != cudaSuccess)
+            return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "accumulator setup");
+        plan->acc_clusters = ncmax;
+    }
+    CcParams p{};
+    fill_params(plan, *vp, p);
+    p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak;
+    p.ri_Fs = plan->ri_Fs, p.ri_Fab = plan->ri_Fab, p.col_freq = plan->col_freq, p.ri_a0 = 0.0;
+    p.acc_G = plan->acc_G, p.acc_ab = plan->acc_ab, p.acc_mean = plan->acc_mean;
+    const int ncl = std::min(batch, ncmax);
+    cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
+    plan->acc_count += batch;
+    return CC_OK;
+}
+
+// Gt <- conj(sum over clusters) / (N HW), clusters in index order (deterministic); accumulators cleared
+__global__ void cc_reduce_reference_kernel(float2 *acc_G, float4 *acc_ab, double *acc_mean, int ncl, int H, int Wh,
+                                           const int16_t *col_freq, float2 *Gt, float4 *ab, double *emean, double inv, double invN)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t plane = (size_t)H * Wh;
+    if (idx < H * Wh && idx % Wh != 0) {
+        double sx = 0.0, sy = 0.0;
+        for (int c = 0; c < ncl; ++c) {
+            const float2 v = acc_G[c * plane + idx];
+            sx += (double)v.x, sy += (double)v.y;
+            acc_G[c * plane + idx] = make_float2(0.f, 0.f);
+        }
+        Gt[idx] = make_float2((float)(sx * inv), (float)(-sy * inv));
+    }
+    if (idx < H) {
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        for (int c = 0; c < ncl; ++c) {
+            const float4 v = acc_ab[(size_t)c * H + idx];
+            a0 += (double)v.x, a1 += (double)v.y, a2 += (double)v.z, a3 += (double)v.w;
+            acc_ab[(size_t)c * H + idx] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        const bool dc = col_freq[idx] == 0;  // the DC bin of the reference stays zero (R10)
+        ab[idx] = make_float4(dc ? 0.f : (float)(a0 * inv), dc ? 0.f : (float)(-a1 * inv), (float)(a2 * inv), (float)(-a3 * inv));
+    }
+    if (idx == 0) {
+        double m = 0.0;
+        for (int c = 0; c < ncl; ++c) m += acc_mean[c], acc_mean[c] = 0.0;
+        *emean = m * invN;
+    }
+}
+
+extern "C" cc_status cc_plan_update_reference_from_accumulator(cc_plan *plan, void *stream)
+{
+    if (!plan) return fail(CC_ERR_INVALID_ARG, "cc_plan_update_reference_from_accumulator: null plan");
+    if (plan->acc_count <= 0 || !plan->acc_G) return fail(CC_ERR_INVALID_ARG, "nothing accumulated: call cc_track_accumulate first");
+    const int H = plan->H, Wh = plan->W / 2;
+    const double invN = 1.0 / (double)plan->acc_count, inv = invN / ((double)H * (double)plan->W);
+    const int threads = 256, blocks = (H * Wh + threads - 1) / threads;
+    cc_reduce_reference_kernel<<<blocks, threads, 0, (cudaStream_t)stream>>>(plan->acc_G, plan->acc_ab, plan->acc_mean,
+                                                                             plan->acc_clusters, H, Wh, plan->col_freq, plan->Gt,
+                                                                             plan->ab, plan->ri_emean, inv, invN);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "reference reduction launch");
+    plan->acc_count = 0;
     return CC_OK;
 }
 

@@ -103,7 +103,12 @@ struct CcParams {
     // reads Gt / ab / the reference mean through L2 (ld.cg) and rewrites them after every frame.
     float2 *ri_Fs;             // [H][W/2] forward spectrum of the current frame, column-slot order (scratch)
     float4 *ri_Fab;            // [H] (DC column, Nyquist column) of the current frame's spectrum, by slot
-    double *ri_emean;          // mean of the running reference image
+    double *ri_emean;          // mean of the reference image when it lives on the device (else null: Emean below)
+    // offline iteration (Eq. (8)): per-cluster sums of the aligned frame spectra; acc_G == null
+    // outside that mode.  ri_Fs / ri_Fab then hold one copy per cluster and the reference is not rewritten.
+    float2 *acc_G;             // [clusters][H][W/2]
+    float4 *acc_ab;            // [clusters][H]
+    double *acc_mean;          // [clusters] sum of the frame means
     const int16_t *col_freq;   // [H] signed row frequency ky of column-FFT slot p (-H/2 at the Nyquist slot)
     double ri_a0;              // a0 = 1 - exp(-T/tau); b1 = 1 - a0
 

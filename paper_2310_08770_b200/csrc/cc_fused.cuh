@@ -612,7 +612,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     // results of one frame (rank 0, thread 0): batch arrays, or the session's mapped host record
     const bool RT = p.rt_cmd != nullptr;
-    const bool RI = p.ri_Fs != nullptr;  // running reference image (Eq. (9))
+    const bool ACC = p.acc_G != nullptr;              // offline iteration, Eq. (8): accumulate the aligned spectra
+    const bool RI = p.ri_Fs != nullptr;               // the frame's spectrum is kept: Eq. (9) update, or Eq. (8) accumulation
+    float2 *const Fs = RI ? p.ri_Fs + (size_t)cid * H * (W / 2) : nullptr;  // this cluster's copy
+    float4 *const Fab = RI ? p.ri_Fab + (size_t)cid * H : nullptr;
     uint64_t rt_seq = 0;    // sequence number of the command being served
     uint32_t cph = 0;       // phase parity of the command barrier
     auto emit = [&](int f, float dyv, float dxv, float pkv, int wyv, int wxv) {
@@ -668,17 +671,30 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             const int ps = idx / NC, q = rank * NC + idx % NC;
             if (q == 0) continue;
             const size_t gi = (size_t)ps * (W / 2) + q;
-            const float2 Fv = __ldcg(&p.ri_Fs[gi]), Gv = __ldcg(&p.Gt[gi]);
-            const float2 Fp = cmul(Fv, cmul(wyt[ps], wxt[q]));
-            __stcg(const_cast<float2 *>(&p.Gt[gi]), make_float2(fmaf(b1f, Gv.x, scf * Fp.x), fmaf(b1f, Gv.y, -scf * Fp.y)));
+            const float2 Fp = cmul(__ldcg(&Fs[gi]), cmul(wyt[ps], wxt[q]));
+            if (ACC) {  // Eq. (8): this cluster's running sum of the aligned spectra
+                float2 *a = p.acc_G + (size_t)cid * H * (W / 2) + gi;
+                const float2 av = __ldcg(a);
+                __stcg(a, make_float2(av.x + Fp.x, av.y + Fp.y));
+            } else {
+                const float2 Gv = __ldcg(&p.Gt[gi]);
+                __stcg(const_cast<float2 *>(&p.Gt[gi]), make_float2(fmaf(b1f, Gv.x, scf * Fp.x), fmaf(b1f, Gv.y, -scf * Fp.y)));
+            }
         }
         if (rank == 0) {
             for (int ps = tid; ps < H; ps += NT) {
                 const int fy = (int)p.col_freq[ps];
-                const float4 Fv = __ldcg(&p.ri_Fab[ps]), Gv = __ldcg(&p.ab[ps]);
+                const float4 Fv = __ldcg(&Fab[ps]);
                 const float2 wy = wyt[ps];
                 const float2 Fa = cmul(make_float2(Fv.x, Fv.y), wy);
                 const float2 Fb = cmul(make_float2(Fv.z, Fv.w), make_float2(wy.x * (float)cnx, wy.y * (float)cnx));
+                if (ACC) {
+                    float4 *a = p.acc_ab + (size_t)cid * H + ps;
+                    const float4 av = __ldcg(a);
+                    __stcg(a, make_float4(av.x + Fa.x, av.y + Fa.y, av.z + Fb.x, av.w + Fb.y));
+                    continue;
+                }
+                const float4 Gv = __ldcg(&p.ab[ps]);
                 float4 o;
                 o.x = fy == 0 ? 0.f : fmaf(b1f, Gv.x, scf * Fa.x);  // the DC bin of the reference stays zero (R10)
                 o.y = fy == 0 ? 0.f : fmaf(b1f, Gv.y, -scf * Fa.y);
@@ -688,7 +704,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
             if (tid == 0) {
                 const double mean_i = ((double)*f00 + c0d * H * W) / ((double)H * (double)W);
-                __stcg(p.ri_emean, b1 * __ldcg(p.ri_emean) + a0 * mean_i);
+                if (ACC) __stcg(p.acc_mean + cid, __ldcg(p.acc_mean + cid) + mean_i);
+                else __stcg(p.ri_emean, b1 * __ldcg(p.ri_emean) + a0 * mean_i);
             }
         }
         __threadfence();
@@ -834,7 +851,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 #pragma unroll
                     for (int k = 0; k < RL; ++k) {
                         const size_t gi = (size_t)(g * RL + k) * (W / 2) + q;
-                        if (RI) __stcg(&p.ri_Fs[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
+                        if (RI) __stcg(&Fs[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
                         w[k] = cmul(v[brev(k, bits)], __ldcg(&p.Gt[gi]));  // through L2: the RI update rewrites Gt
                     }
                     dft_reg<RL, true>(w);
@@ -857,7 +874,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         const float4 g = __ldcg(&p.ab[s]);  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
-                        if (RI) __stcg(&p.ri_Fab[s], make_float4(fa.x, fa.y, fb.x, fb.y));
+                        if (RI) __stcg(&Fab[s], make_float4(fa.x, fa.y, fb.x, fb.y));
                         const float2 pa = cmul(fa, make_float2(g.x, g.y)), pb = cmul(fb, make_float2(g.z, g.w));
                         o[e] = make_float2(pa.x - pb.y, pa.y + pb.x);
                         if (s == 0) *f00 = z.x;  // sum of (I - c0): DC add-back for `peak`
@@ -960,7 +977,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
         if (u == 1) {
             if (rank == 0 && tid == 0) {
-                const double Em = RI ? __ldcg(p.ri_emean) : p.Emean;
+                const double Em = p.ri_emean ? __ldcg(p.ri_emean) : p.Emean;
                 emit(f, (float)wy, (float)wx, (float)(p.peak_sign * (cc_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
             }
             if (RI) {
@@ -1334,7 +1351,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
         stamp(7, f);
         if (rank == 0 && tid == 0) {
-            const double Em = RI ? __ldcg(p.ri_emean) : p.Emean;
+            const double Em = p.ri_emean ? __ldcg(p.ri_emean) : p.Emean;
             emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
                  (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
         }
