@@ -614,8 +614,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     const bool RT = p.rt_cmd != nullptr;
     const bool ACC = p.acc_G != nullptr;              // offline iteration, Eq. (8): accumulate the aligned spectra
     const bool RI = p.ri_Fs != nullptr;               // the frame's spectrum is kept: Eq. (9) update, or Eq. (8) accumulation
-    float2 *const Fs = RI ? p.ri_Fs + (size_t)cid * H * (W / 2) : nullptr;  // this cluster's copy
-    float4 *const Fab = RI ? p.ri_Fab + (size_t)cid * H : nullptr;
+    // this cluster's copy of the frame spectrum (computed at the use sites: no registers held through the GEMM phases)
+    auto Fs_of = [&]() { return p.ri_Fs + (size_t)cid * H * (W / 2); };
+    auto Fab_of = [&]() { return p.ri_Fab + (size_t)cid * H; };
     uint64_t rt_seq = 0;    // sequence number of the command being served
     uint32_t cph = 0;       // phase parity of the command barrier
     auto emit = [&](int f, float dyv, float dxv, float pkv, int wyv, int wxv) {
@@ -671,7 +672,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             const int ps = idx / NC, q = rank * NC + idx % NC;
             if (q == 0) continue;
             const size_t gi = (size_t)ps * (W / 2) + q;
-            const float2 Fp = cmul(__ldcg(&Fs[gi]), cmul(wyt[ps], wxt[q]));
+            const float2 Fp = cmul(__ldcg(&Fs_of()[gi]), cmul(wyt[ps], wxt[q]));
             if (ACC) {  // Eq. (8): this cluster's running sum of the aligned spectra
                 float2 *a = p.acc_G + (size_t)cid * H * (W / 2) + gi;
                 const float2 av = __ldcg(a);
@@ -684,7 +685,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if (rank == 0) {
             for (int ps = tid; ps < H; ps += NT) {
                 const int fy = (int)p.col_freq[ps];
-                const float4 Fv = __ldcg(&Fab[ps]);
+                const float4 Fv = __ldcg(&Fab_of()[ps]);
                 const float2 wy = wyt[ps];
                 const float2 Fa = cmul(make_float2(Fv.x, Fv.y), wy);
                 const float2 Fb = cmul(make_float2(Fv.z, Fv.w), make_float2(wy.x * (float)cnx, wy.y * (float)cnx));
@@ -851,7 +852,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 #pragma unroll
                     for (int k = 0; k < RL; ++k) {
                         const size_t gi = (size_t)(g * RL + k) * (W / 2) + q;
-                        if (RI) __stcg(&Fs[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
+                        if (RI) __stcg(&Fs_of()[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
                         w[k] = cmul(v[brev(k, bits)], __ldcg(&p.Gt[gi]));  // through L2: the RI update rewrites Gt
                     }
                     dft_reg<RL, true>(w);
@@ -874,7 +875,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         const float4 g = __ldcg(&p.ab[s]);  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
-                        if (RI) __stcg(&Fab[s], make_float4(fa.x, fa.y, fb.x, fb.y));
+                        if (RI) __stcg(&Fab_of()[s], make_float4(fa.x, fa.y, fb.x, fb.y));
                         const float2 pa = cmul(fa, make_float2(g.x, g.y)), pb = cmul(fb, make_float2(g.z, g.w));
                         o[e] = make_float2(pa.x - pb.y, pa.y + pb.x);
                         if (s == 0) *f00 = z.x;  // sum of (I - c0): DC add-back for `peak`
