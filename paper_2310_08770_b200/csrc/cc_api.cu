@@ -606,7 +606,8 @@ extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
     float *ddx = plan->dres, *ddy = plan->dres + plan->res_cap, *dpk = plan->dres + 2 * (size_t)plan->res_cap;
     int nchunks = (batch + chunk - 1) / chunk;
     for (int ci = 0; ci < nchunks; ++ci) {
-        const int b = ci & 1, f0 = ci * chunk, n = std::min(chunk, batch - f0);
+        // with the running reference image (Eq. (9)) the chunks must run in order: one stream, one staging buffer
+        const int b = plan->ri_a0 > 0.0 ? 0 : (ci & 1), f0 = ci * chunk, n = std::min(chunk, batch - f0);
         cudaStream_t s = plan->hs[b];
         CK(cudaMemcpyAsync(plan->dframes[b], (const unsigned char *)frames + (size_t)f0 * fbytes, (size_t)n * fbytes,
                            cudaMemcpyHostToDevice, s));

@@ -62,6 +62,10 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.cc_plan_create_weighted(ctypes.byref(h), 64, 64, 1, 10, rp, 1, ctypes.c_float(-2.0)) == 1  # epsilon < 0
     assert lib.cc_rt_submit(None, None) == 1 and lib.cc_rt_wait(None, None, None, None) == 1
     assert lib.cc_rt_close(None) == 0
+    assert lib.cc_plan_enable_reference_update(None, 0.1) == 1
+    assert lib.cc_plan_get_reference_spectrum(None, None) == 1
+    assert lib.cc_track_accumulate(None, None, 4, None, None, None, None) == 1
+    assert lib.cc_plan_update_reference_from_accumulator(None, None) == 1
     assert lib.cc_drift_correct(None, None, -1, 0.1, 0.0, None, None, None, None) == 1
     assert lib.cc_drift_correct(None, None, 4, 0.1, 0.0, None, None, None, None) == 1
     assert lib.cc_track_latency_probe(None, None, 1, None, None, None, None, None) == 1

@@ -536,3 +536,24 @@ def test_offline_iterative_reference_matches_oracle(gpu, oracle_mod, ci, n, u, p
     scale = np.max(np.abs(G[1:, 1:]))
     assert np.max(np.abs(Gd - _half(G))[:, 1:]) < 1e-4 * scale + 3e-2 * scale * np.sum(step > TOL_PX) / (u * n)
     assert abs(Gd[0, 0] / G[0, 0] - 1) < 1e-6
+
+
+def test_host_path_with_running_reference(gpu):
+    """cc_track_host keeps the frame order when the reference is updated after every frame (chunks on one stream)."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr = wl.frames(cfg, np.arange(200))
+    ref = wl.reference(cfg)
+    res = []
+    for host in (False, True):
+        plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, ref)
+        plan.enable_reference_update(0.05)
+        if host:
+            dx, dy, pk = plan.track_host(fr)
+        else:
+            dx, dy, pk = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr))]
+        res.append((dx, dy, pk, plan.reference_spectrum()))
+        plan.close()
+    for a, b in zip(res[0], res[1]):
+        assert np.array_equal(a, b)
