@@ -565,7 +565,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     // double[9][NC].  Result: out[a*3+b] valid in all threads of all CTAs.  Summation order is fixed.
     auto xeval9 = [&](auto getR, auto phase, const double *nyq_c, double *terms, double *out) {
         static_assert((24 * NC) % 32 == 0, "whole warps per (a, ql) group sweep");
-        for (int t = tid; t < 24 * NC; t += NT) {  // warp-uniform trip count
+        constexpr int XIT = (24 * NC + NT - 1) / NT;
+#pragma unroll
+        for (int it = 0; it < XIT; ++it) {  // unrolled: the table loads of all trips go out together
+            const int t = tid + it * NT;
+            if (t >= 24 * NC) break;       // warp-uniform (24 NC and NT are multiples of 32)
             const int o = t >> 3, sub = t & 7;
             const int a = o / NC, ql = o % NC;
             const int q = rank * NC + ql;
@@ -1280,10 +1284,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
                 // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j'):
                 // rows ms-1..ms+1 of the plan's fp64 table Dpol[M][H] (zero weights outside the grid)
-                for (int e = tid; e < 3 * H; e += NT) {
-                    const int a = e / H, j = e % H;
-                    const int mm = ms - 1 + a;
-                    dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
+#pragma unroll
+                for (int it = 0; it < (3 * H + NT - 1) / NT; ++it) {  // unrolled: all loads of a thread go out together
+                    const int e = tid + it * NT;
+                    if (e < 3 * H) {
+                        const int a = e / H, j = e % H;
+                        const int mm = ms - 1 + a;
+                        dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
+                    }
                 }
                 __syncthreads();
                 for (int e = tid; e < NSL * NC; e += NT) {
