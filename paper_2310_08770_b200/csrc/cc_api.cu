@@ -766,6 +766,9 @@ extern "C" cc_status cc_rt_wait(cc_rt *rt, float *dx, float *dy, float *peak)
     double t0 = mono_us();
     for (;;) {
         if (__atomic_load_n((uint32_t *)&rt->res[3], __ATOMIC_ACQUIRE) == (uint32_t)rt->seq) break;
+#if defined(__x86_64__) || defined(__i386__)
+        __builtin_ia32_pause();  // spin-wait hint: the result arrives by a PCIe write into this cache line
+#endif
         if (mono_us() - t0 > 2.0e5) {  // 200 ms without an answer
             // the kernel may have hit its idle timeout just as the frame was submitted: restart once
             if (!*rt->alive && restarts == 0) {
