@@ -557,3 +557,25 @@ def test_host_path_with_running_reference(gpu):
         plan.close()
     for a, b in zip(res[0], res[1]):
         assert np.array_equal(a, b)
+
+
+def test_concurrent_streams_on_one_plan(gpu):
+    """include/cc.h: a plan without scratch (scratch_bytes == 0) may be used by cc_track on several streams at once."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(3)
+    fr = wl.frames(cfg, np.arange(600))
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, cfg.upsample, wl.reference(cfg))
+    assert plan.info()["scratch_bytes"] == 0
+    d = plan.device_frames(fr)
+    ref_out = [t.clone() for t in plan.track(d)]
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        a = plan.track(d[:300], stream=s1)
+        b = plan.track(d[300:], stream=s2)
+    s1.synchronize()
+    s2.synchronize()
+    for k in range(3):
+        assert torch.equal(torch.cat([a[k], b[k]]), ref_out[k])
+    plan.close()
