@@ -30,8 +30,8 @@ CCV(f512x256_u16,  512,  256, 4, uint16_t, 256, 10, 4,  5, 5, false, 12,  4, 16,
 CCV(f128x1024_u16, 128, 1024, 8, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
 CCV(f1024x128_u16, 1024, 128, 4, uint16_t, 256,  5, 4,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
 // 512x512 single-frame (latency) variant: one frame over a 16-CTA cluster (non-portable cluster size)
-CCV(f512_u16_c16,  512,  512, 16, uint16_t, 256,  4, 4,  1, 5, false, 32, 16,  8,  4,  3,  2,  1)
-CCV(f512_u8_c16,   512,  512, 16, uint8_t,  256,  4, 4,  1, 5, false, 32, 16,  8,  4,  3,  2,  1)
+CCV(f512_u16_c16,  512,  512, 16, uint16_t, 256,  8, 4,  1, 5, false, 32, 16,  8,  4,  3,  2,  2)
+CCV(f512_u8_c16,   512,  512, 16, uint8_t,  256,  8, 4,  1, 5, false, 32, 16,  8,  4,  3,  2,  2)
 // 256x256 single-frame (latency) variants: one frame over an 8-CTA cluster
 CCV(f256_u16_c8,   256,  256, 8, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
 CCV(f256_u8_c8,    256,  256, 8, uint8_t,  256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
