@@ -91,6 +91,21 @@ __device__ __forceinline__ uint64_t globaltimer_ns()
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
+// packed FP32 pairs (Blackwell FFMA2: two fused multiply-adds per instruction, each IEEE-rounded like fmaf)
+__device__ __forceinline__ unsigned long long pack2(float x, float y)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+    return r;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float &x, float &y) { asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
 // ------------------------------------------------------------------ small complex helpers
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a*conj(b)
@@ -1026,10 +1041,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     const int gc0 = ch * MC1 + tm1 * TM1;
                     const bool isV = gc0 >= DSBp;
                     float acc[TM1][TN1];
+                    unsigned long long acc2[TM1][TN1 / 2];  // the k-loop accumulates column pairs with FFMA2
 #pragma unroll
                     for (int i = 0; i < TM1; ++i)
 #pragma unroll
-                        for (int j = 0; j < TN1; ++j) acc[i][j] = 0.f;
+                        for (int j = 0; j < TN1 / 2; ++j) acc2[i][j] = 0ull;
                     for (int kt = 0; kt < p.KT1; ++kt) {
                         const float *At = ring_acquire();
 #pragma unroll
@@ -1058,13 +1074,22 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                 const float4 t = *reinterpret_cast<const float4 *>(brow + v * Cn1 * 4);
                                 b[4 * v] = t.x, b[4 * v + 1] = t.y, b[4 * v + 2] = t.z, b[4 * v + 3] = t.w;
                             }
+                            unsigned long long b2[TN1 / 2];
 #pragma unroll
-                            for (int i = 0; i < TM1; ++i)
+                            for (int j = 0; j < TN1 / 2; ++j) b2[j] = pack2(b[2 * j], b[2 * j + 1]);
 #pragma unroll
-                                for (int j = 0; j < TN1; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+                            for (int i = 0; i < TM1; ++i) {
+                                const unsigned long long aa = pack2(a[i], a[i]);
+#pragma unroll
+                                for (int j = 0; j < TN1 / 2; ++j) acc2[i][j] = fma2(aa, b2[j], acc2[i][j]);
+                            }
                         }
                         ring_release();
                     }
+#pragma unroll
+                    for (int i = 0; i < TM1; ++i)
+#pragma unroll
+                        for (int j = 0; j < TN1 / 2; ++j) unpack2(acc2[i][j], acc[i][2 * j], acc[i][2 * j + 1]);
                     if constexpr (KS1 > 1) {  // sum the k-slices into slice 0
                         const int t1 = tm1 * Cn1 + tn1;
                         if (ks1 > 0) {
