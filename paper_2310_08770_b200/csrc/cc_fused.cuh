@@ -1172,10 +1172,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     for (int i = 0; i < TM2; ++i) Arow[i] = Tb + (size_t)min(rbase + i, 2 * DS - 1) * LDT;
                     for (int nc2 = 0; nc2 < p.nnc2; ++nc2) {
                         float aE[TM2][TN2], aO[TM2][TN2];
+                        unsigned long long aE2[TM2][2], aO2[TM2][2];  // columns 0..3 as pairs (FFMA2); column 4 scalar
 #pragma unroll
-                        for (int i = 0; i < TM2; ++i)
-#pragma unroll
-                            for (int j = 0; j < TN2; ++j) aE[i][j] = 0.f, aO[i][j] = 0.f;
+                        for (int i = 0; i < TM2; ++i) {
+                            aE2[i][0] = aE2[i][1] = aO2[i][0] = aO2[i][1] = 0ull;
+                            if constexpr (TN2 > 4) aE[i][4] = 0.f, aO[i][4] = 0.f;
+                        }
                         constexpr int KT2 = W / (4 * G2);
                         for (int kt = 0; kt < KT2; ++kt) {
                             const float *Bt = ring_acquire();
@@ -1195,18 +1197,27 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                     float b[TN2];
                                     b[0] = b4.x, b[1] = b4.y, b[2] = b4.z, b[3] = b4.w;
                                     if constexpr (C::X2 == 1) b[4] = kk == 0 ? x4.x : kk == 1 ? x4.y : kk == 2 ? x4.z : x4.w;
+                                    const unsigned long long b01 = pack2(b[0], b[1]), b23 = pack2(b[2], b[3]);
 #pragma unroll
                                     for (int i = 0; i < TM2; ++i) {
                                         const float av = kk == 0 ? a4[i].x : kk == 1 ? a4[i].y : kk == 2 ? a4[i].z : a4[i].w;
-#pragma unroll
-                                        for (int j = 0; j < TN2; ++j) {
-                                            if ((kk & 1) == 0) aE[i][j] = fmaf(av, b[j], aE[i][j]);
-                                            else aO[i][j] = fmaf(av, b[j], aO[i][j]);
+                                        const unsigned long long aa = pack2(av, av);
+                                        if ((kk & 1) == 0) {
+                                            aE2[i][0] = fma2(aa, b01, aE2[i][0]), aE2[i][1] = fma2(aa, b23, aE2[i][1]);
+                                            if constexpr (TN2 > 4) aE[i][4] = fmaf(av, b[4], aE[i][4]);
+                                        } else {
+                                            aO2[i][0] = fma2(aa, b01, aO2[i][0]), aO2[i][1] = fma2(aa, b23, aO2[i][1]);
+                                            if constexpr (TN2 > 4) aO[i][4] = fmaf(av, b[4], aO[i][4]);
                                         }
                                     }
                                 }
                             }
                             ring_release();
+                        }
+#pragma unroll
+                        for (int i = 0; i < TM2; ++i) {
+                            unpack2(aE2[i][0], aE[i][0], aE[i][1]), unpack2(aE2[i][1], aE[i][2], aE[i][3]);
+                            unpack2(aO2[i][0], aO[i][0], aO[i][1]), unpack2(aO2[i][1], aO[i][2], aO[i][3]);
                         }
                         if constexpr (KS2 > 1) {  // sum the k-slices into slice 0
                             const int t2 = tm2 * Cn2 + tn2;
