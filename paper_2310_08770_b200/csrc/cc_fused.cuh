@@ -106,6 +106,24 @@ __device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigne
     return d;
 }
 
+// complex add / subtract as one packed instruction each (IEEE per lane, same results as two scalar adds)
+__device__ __forceinline__ float2 cadd2(float2 a, float2 b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pack2(a.x, a.y)), "l"(pack2(b.x, b.y)));
+    float2 r;
+    unpack2(d, r.x, r.y);
+    return r;
+}
+__device__ __forceinline__ float2 csub2(float2 a, float2 b)
+{
+    unsigned long long d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pack2(a.x, a.y)), "l"(pack2(b.x, b.y)));
+    float2 r;
+    unpack2(d, r.x, r.y);
+    return r;
+}
+
 // ------------------------------------------------------------------ small complex helpers
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a*conj(b)
@@ -154,8 +172,8 @@ __device__ __forceinline__ void dft_reg(float2 (&v)[R])
             if ((i & span) == 0) {
                 const int j = i | span;
                 const float2 a = v[i], b = v[j];
-                v[i] = make_float2(a.x + b.x, a.y + b.y);
-                const float2 d = make_float2(a.x - b.x, a.y - b.y);
+                v[i] = cadd2(a, b);
+                const float2 d = csub2(a, b);
                 const int t16 = (i & (span - 1)) * (8 / span);  // twiddle angle in units of 2 pi / 16
                 if (t16 == 0) {
                     v[j] = d;
