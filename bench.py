@@ -405,7 +405,7 @@ def main():
     t_hbm = (frames[0].nbytes + 12) / (hbm_gbs * 1e9)
     roofline = {
         "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": 1.317e9, "traffic_source": "ncu --set full capture profiles/r1g_summary.md: dram read 1.3130 GB + write 3.9 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
+        "traffic": 1.318e9, "traffic_source": "ncu --set full capture profiles/r1h_summary.md: dram read 1.3134 GB + write 4.2 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
         "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
         "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,
