@@ -270,10 +270,10 @@ cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info);
 cc_status cc_fp32_peak_probe(double *tflops, void *stream);
 
 /*
- * cc_fp32_tile_probe -- second measurement aid: an 8x8 register-tile FFMA loop with all three operands in
- * registers (the instruction mix of a register-tiled FP32 GEMM inner loop, no memory traffic).  The rate it
- * reaches is the practical ceiling of the upsampled-DFT GEMM loops; cc_fp32_peak_probe's loop (constant
- * operands) reaches the nominal lane rate.
+ * cc_fp32_tile_probe -- second measurement aid: an 8x8 register-tile loop of scalar FFMA with all three operands
+ * in registers (the instruction mix of a classic register-tiled FP32 GEMM inner loop, no memory traffic).  It stays
+ * well below the lane rate that cc_fp32_peak_probe's constant-operand loop reaches; the library's own GEMM loops
+ * therefore use the packed fma.rn.f32x2 form.
  *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
  */
 cc_status cc_fp32_tile_probe(double *tflops, void *stream);
