@@ -18,8 +18,8 @@ CCV(f128_u8_c8,    128,  128, 8, uint8_t,  256,  2, 4,  1, 4, false, 68, 32,  8,
 CCV(f128_u16_c8,   128,  128, 8, uint16_t, 256,  2, 4,  1, 4, false, 68, 32,  8,  8,  8,  6,  4)
 CCV(f256_u16,      256,  256, 2, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
 CCV(f256_u8,       256,  256, 2, uint8_t,  256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1)
-CCV(f512_u16,      512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false, 16, 16,  8,  4,  3,  2,  1)
-CCV(f512_u8,       512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false, 16, 16,  8,  4,  3,  2,  1)
+CCV(f512_u16,      512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false, 16,  8,  8,  4,  3,  2,  1)
+CCV(f512_u8,       512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false, 16,  8,  8,  4,  3,  2,  1)
 CCV(f1024_u16,    1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1)
 CCV(f1024_u8,     1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1)
 // non-square camera formats of the paper's Table I; H = rows, W = columns
