@@ -35,3 +35,11 @@ CCV(f512_u8_c16,   512,  512, 16, uint8_t,  256,  8, 4,  1, 5, false, 32, 16,  8
 // 256x256 single-frame (latency) variants: one frame over an 8-CTA cluster
 CCV(f256_u16_c8,   256,  256, 8, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
 CCV(f256_u8_c8,    256,  256, 8, uint8_t,  256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+// non-square single-frame (latency) variants: one frame over an 8- or 16-CTA cluster (the paper's Table I is measured one
+// image per call)
+CCV(f128x256_u16_c8,   128,  256,  8, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+CCV(f256x128_u16_c8,   256,  128,  8, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+CCV(f256x512_u16_c16,  256,  512, 16, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+CCV(f512x256_u16_c16,  512,  256, 16, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+CCV(f128x1024_u16_c16, 128, 1024, 16, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
+CCV(f1024x128_u16_c8,  1024, 128,  8, uint16_t, 256,  5, 4,  5, 5, false, 16, 16,  4,  4,  3,  2,  1)

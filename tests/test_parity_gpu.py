@@ -424,6 +424,32 @@ def test_single_frame_variants_match_oracle(gpu, oracle_mod, ci, n):
     assert np.max(np.abs(s[:, 2] / o.peak - 1)) <= TOL_PEAK
 
 
+@pytest.mark.parametrize("H,W,u", [(128, 256, 64), (256, 128, 128), (256, 512, 64), (512, 256, 64), (128, 1024, 64),
+                                   (1024, 128, 64), (128, 256, 1024)])
+def test_non_square_single_frame_variants(gpu, oracle_mod, H, W, u):
+    """The paper measures Table I one image per call.  Batch-1 calls on the non-square formats
+    select their cluster (latency) variants: same grid points as the batched variant and as the oracle (CC-SN)."""
+    rng = np.random.default_rng(H * 3 + W + u)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+    spot = lambda sy, sx: 900.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 4.0 ** 2)) + 15.0
+    ref = spot(0.0, 0.0).astype(np.float32)
+    n = 6 if u <= 128 else 3
+    sh = rng.uniform(-9, 9, size=(n, 2))
+    fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 4095).astype(np.uint16)
+    plan = gpu.Plan(H, W, fr.dtype, u, ref, method="sn", epsilon=200.0)
+    info = plan.info()
+    assert info["lat_cluster_size"] > info["cluster_size"]
+    d = plan.device_frames(fr)
+    big = np.concatenate([fr] * (info["lat_max_clusters"] // n + 2))           # more frames than the latency variant takes
+    bx, by, _ = [t.cpu().numpy()[:n] for t in plan.track(plan.device_frames(big))]
+    s = np.array([[t.item() for t in plan.track(d[i], 1)] for i in range(n)], dtype=np.float32)
+    plan.close()
+    o = oracle_mod.track(fr, ref, u, method="sn", epsilon=200.0)
+    assert np.array_equal(s[:, 0], bx) and np.array_equal(s[:, 1], by)
+    assert np.max(np.abs(s[:, 0] - o.dx)) <= TOL_PX and np.max(np.abs(s[:, 1] - o.dy)) <= TOL_PX
+    assert np.max(np.abs(s[:, 2] / o.peak - 1)) <= TOL_PEAK
+
+
 # ---------------------------------------------------------------- running reference image (PAPER.md:L102-108, Eq. (9))
 def _half(G):
     return G[:, : G.shape[1] // 2 + 1]
