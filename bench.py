@@ -211,7 +211,7 @@ def run_table1(args):
     on synthetic 12-bit spot frames: images/s of sequential single-frame calls (the paper's mode) and of one batched
     call.  Context for BASELINE.md section 1, not a target."""
     import torch
-    from paper_2310_08770_b200 import Plan
+    from paper_2310_08770_b200 import Plan, RtSession
     rng = np.random.default_rng(7)
     for (H, W) in ((128, 256), (256, 256), (256, 512), (512, 512), (128, 1024)):
         y, x = np.mgrid[0:H, 0:W].astype(np.float64)
@@ -234,9 +234,18 @@ def run_table1(args):
             batched = nb / (a.elapsed_time(b) * 1e-3)
             plan.latency_probe(d, 20)
             lat = plan.latency_probe(d, 100)[3]
+            torch.cuda.current_stream().synchronize()
+            rt = RtSession(plan, 1000)           # the resident session kernel: no launch + synchronise per image
+            try:
+                rt.latency_probe(d.data_ptr(), 20)
+                lat_rt = rt.latency_probe(d.data_ptr(), 100)[3]
+            finally:
+                rt.close()
             print(json.dumps({"rows_x_cols": "%dx%d" % (H, W), "u": u, "method": "CC-SN",
                               "images_per_s_single_frame_calls": 1e6 / float(np.median(lat)),
                               "single_frame_latency_us_median": float(np.median(lat)),
+                              "images_per_s_rt_session": 1e6 / float(np.median(lat_rt)),
+                              "rt_session_latency_us_median": float(np.median(lat_rt)),
                               "images_per_s_batched": batched, "batch": nb}), flush=True)
             plan.close()
 
@@ -405,7 +414,7 @@ def main():
     t_hbm = (frames[0].nbytes + 12) / (hbm_gbs * 1e9)
     roofline = {
         "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": 1.318e9, "traffic_source": "ncu --set full capture profiles/r1h_summary.md: dram read 1.3134 GB + write 4.2 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
+        "traffic": 1.318e9, "traffic_source": "ncu --set full capture profiles/r1j_summary.md: dram read 1.3128 GB + write 4.7 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
         "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
         "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,

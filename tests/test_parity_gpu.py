@@ -443,8 +443,16 @@ def test_non_square_single_frame_variants(gpu, oracle_mod, H, W, u):
     big = np.concatenate([fr] * (info["lat_max_clusters"] // n + 2))           # more frames than the latency variant takes
     bx, by, _ = [t.cpu().numpy()[:n] for t in plan.track(plan.device_frames(big))]
     s = np.array([[t.item() for t in plan.track(d[i], 1)] for i in range(n)], dtype=np.float32)
+    import torch
+    torch.cuda.current_stream().synchronize()
+    rt = gpu.RtSession(plan, idle_timeout_ms=2000)                             # the session serves the cluster variant
+    try:
+        got = np.array([rt.track(d.data_ptr() + i * fr[0].nbytes) for i in range(n)], dtype=np.float32)
+    finally:
+        rt.close()
     plan.close()
     o = oracle_mod.track(fr, ref, u, method="sn", epsilon=200.0)
+    assert np.array_equal(got, s)
     assert np.array_equal(s[:, 0], bx) and np.array_equal(s[:, 1], by)
     assert np.max(np.abs(s[:, 0] - o.dx)) <= TOL_PX and np.max(np.abs(s[:, 1] - o.dy)) <= TOL_PX
     assert np.max(np.abs(s[:, 2] / o.peak - 1)) <= TOL_PEAK
