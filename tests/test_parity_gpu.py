@@ -485,7 +485,23 @@ def test_reference_spectrum_accessor_and_aligned_copies(gpu, oracle_mod):
     plan.close()
 
 
-@pytest.mark.parametrize("ci,n,a0", [(2, 300, 0.02), (1, 120, 0.1), (3, 40, 0.05)])
+class _Fmt:
+    """A Table-I camera format as a stand-in for a workloads config: 12-bit spot on a random walk."""
+    def __init__(self, H, W, u):
+        self.H, self.W, self.upsample = H, W, u
+
+    def make(self, n):
+        H, W = self.H, self.W
+        rng = np.random.default_rng(H + 5 * W)
+        y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+        spot = lambda sy, sx: 900.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 4.0 ** 2)) + 15.0
+        sh = np.cumsum(rng.normal(0.0, 0.3, size=(n, 2)), axis=0)
+        fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 4095).astype(np.uint16)
+        return fr, spot(0.0, 0.0).astype(np.float32)
+
+
+@pytest.mark.parametrize("ci,n,a0", [(2, 300, 0.02), (1, 120, 0.1), (3, 40, 0.05), (_Fmt(256, 128, 64), 60, 0.05),
+                                     (_Fmt(128, 1024, 32), 24, 0.05)], ids=["cfg2", "cfg1", "cfg3", "256x128", "128x1024"])
 def test_running_reference_matches_oracle(gpu, oracle_mod, ci, n, a0):
     """Closed loop of Eq. (9): the device rewrites its fp32 reference spectrum after every frame, the oracle its
     float64 one.  Integer peaks must agree on every frame; the sub-pixel grid point on nearly all of them and never
@@ -493,9 +509,13 @@ def test_running_reference_matches_oracle(gpu, oracle_mod, ci, n, a0):
     differ in the 7th digit); the spectra must still agree to 1e-4 of their scale after n frames."""
     import torch
     from paper_2310_08770_b200 import workloads as wl
-    cfg = wl.config(ci)
-    fr = wl.frames(cfg, np.arange(n))
-    ref = wl.reference(cfg)
+    if isinstance(ci, _Fmt):                                       # non-square formats: the cluster (latency) variants
+        cfg = ci
+        fr, ref = cfg.make(n)
+    else:
+        cfg = wl.config(ci)
+        fr = wl.frames(cfg, np.arange(n))
+        ref = wl.reference(cfg)
     u = cfg.upsample
     o, G = oracle_mod.track_rt(fr, ref, u, a0)
     plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, u, ref)
