@@ -404,7 +404,7 @@ def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
 
 @pytest.mark.parametrize("ci,n", [(3, 24), (4, 12)])
 def test_single_frame_variants_match_oracle(gpu, oracle_mod, ci, n):
-    """Sequential batch-1 calls select the small-batch cluster variants (8 CTAs at 256x256, 16 CTAs at 512x512);
+    """Sequential batch-1 calls select the small-batch cluster variants (16 CTAs at 256x256 and 512x512);
     they return the oracle's grid points and the same displacements as the batched variant."""
     from paper_2310_08770_b200 import workloads as wl
     cfg = wl.config(ci)
