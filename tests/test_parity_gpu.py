@@ -554,6 +554,25 @@ def test_running_reference_matches_oracle(gpu, oracle_mod, ci, n, a0):
     assert np.array_equal(got[:, 0], dx[m // 2:m]) and np.array_equal(got[:, 1], dy[m // 2:m])
 
 
+@pytest.mark.parametrize("H,W", [(256, 256), (128, 256), (1024, 128)])
+@pytest.mark.parametrize("u", [1, 5, 13, 20])
+def test_cluster_variants_with_fewer_offsets_than_ctas(gpu, oracle_mod, H, W, u):
+    """Small upsampling factors on the 16-CTA single-frame variants: floor(M/2)+1 offsets per axis <= 16 CTAs, so some
+    CTAs own no offset (u = 1: M = 2; u = 20: exactly one each).  Batch-1 calls against the oracle and the batched variant."""
+    fr, ref = _Fmt(H, W, u).make(4)
+    plan = gpu.Plan(H, W, fr.dtype, u, ref)
+    info = plan.info()
+    assert info["lat_cluster_size"] == 16
+    bx, by, _ = [t.cpu().numpy()[:4] for t in plan.track(plan.device_frames(np.concatenate([fr] * 6)))]
+    d = plan.device_frames(fr)
+    s = np.array([[t.item() for t in plan.track(d[i], 1)] for i in range(4)], dtype=np.float32)
+    plan.close()
+    o = oracle_mod.track(fr, ref, u)
+    assert np.array_equal(s[:, 0], bx) and np.array_equal(s[:, 1], by)
+    assert np.max(np.abs(s[:, 0] - o.dx)) <= TOL_PX and np.max(np.abs(s[:, 1] - o.dy)) <= TOL_PX
+    assert np.max(np.abs(s[:, 2] / o.peak - 1)) <= TOL_PEAK
+
+
 @pytest.mark.parametrize("ci,n,u,passes", [(1, 300, 20, 3), (3, 90, 100, 2)])
 def test_offline_iterative_reference_matches_oracle(gpu, oracle_mod, ci, n, u, passes):
     """Offline analysis, Eq. (8), starting from E_0 = I_0: every pass tracks all frames in parallel
