@@ -43,3 +43,6 @@ CCV(f128x1024_u16_c16, 128, 1024, 16, uint16_t, 256,  5, 4,  5, 5, false, 32, 16
 CCV(f128x256_u16_c16,  128,  256, 16, uint16_t, 256,  5, 4,  5, 5, false, 32, 16,  4,  4,  3,  2,  1)
 CCV(f256x128_u16_c16,  256,  128, 16, uint16_t, 256,  5, 4,  5, 5, false,  8, 16,  4,  4,  3,  2,  1)
 CCV(f1024x128_u16_c16, 1024, 128, 16, uint16_t, 256,  5, 4,  5, 5, false,  8, 16,  4,  4,  3,  2,  1)
+// 1024x1024 single-frame (latency) variant: one frame over a 16-CTA cluster
+CCV(f1024_u16_c16, 1024, 1024, 16, uint16_t, 256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1)
+CCV(f1024_u8_c16,  1024, 1024, 16, uint8_t,  256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1)

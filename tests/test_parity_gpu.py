@@ -402,9 +402,9 @@ def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
     _compare(o, dx, dy, pk, iy, ix, "%dx%d u=%d CC-SN" % (H, W, u))
 
 
-@pytest.mark.parametrize("ci,n", [(3, 24), (4, 12)])
+@pytest.mark.parametrize("ci,n", [(3, 24), (4, 12), (5, 4)])
 def test_single_frame_variants_match_oracle(gpu, oracle_mod, ci, n):
-    """Sequential batch-1 calls select the small-batch cluster variants (16 CTAs at 256x256 and 512x512);
+    """Sequential batch-1 calls select the small-batch cluster variants (16 CTAs at 256x256, 512x512 and 1024x1024);
     they return the oracle's grid points and the same displacements as the batched variant."""
     from paper_2310_08770_b200 import workloads as wl
     cfg = wl.config(ci)
