@@ -27,10 +27,13 @@
  *   - `peak` is the (upsampled) correlation sum at the maximum, in
  *     pixel-value^2 units (sum_r I(r+d) E(r)).
  *
- * Threading: a plan is immutable after creation.  cc_track() on one plan may
- * be enqueued on several streams concurrently only when cc_plan_info()
- * reports scratch_bytes == 0; otherwise serialise the calls.  cc_track_host()
- * uses plan-owned staging buffers and must be serialised per plan.
+ * Threading: a plan is immutable after creation (unless the reference update
+ * of Eq. (9) is switched on, see cc_plan_enable_reference_update).  cc_track()
+ * on one plan may be enqueued on several streams concurrently only when
+ * cc_plan_info() reports scratch_bytes == 0; otherwise serialise the calls.
+ * cc_track_host() uses plan-owned staging buffers and must be serialised per
+ * plan.  A real-time session (cc_rt_*) owns its scratch and may run beside
+ * cc_track on the same plan.  Measurement aids: include/cc_bench.h.
  */
 #ifndef CC_H
 #define CC_H
@@ -118,6 +121,8 @@ cc_status cc_track(const cc_plan *plan, const void *frames, int batch,
  * cc_track_debug -- cc_track that additionally returns the wrapped integer
  * peak of step a5 (PAPER.md:L90 sentence 1).
  *   iy, ix   DEVICE pointers, batch int32 each, or NULL
+ * (The optional per-phase timing argument of the interface sketch in SURVEY.md 8(b), `phase_ns`, lives in
+ * cc_track_profile below, as SM-clock cycles per phase.)
  */
 cc_status cc_track_debug(const cc_plan *plan, const void *frames, int batch,
                          float *dx, float *dy, float *peak, int *iy, int *ix, void *stream);
@@ -137,30 +142,24 @@ cc_status cc_track_profile(const cc_plan *plan, const void *frames, int batch,
                            unsigned long long *phase_cycles, void *stream);
 
 /*
+ * cc_plan_set_host_chunk -- frames per host->device chunk of cc_track_host (0: the default, about 64 MB of
+ * frames and at least one wave of clusters).  Chunks alternate between two plan-owned streams so that the copy
+ * of one overlaps the kernel of the other.
+ */
+cc_status cc_plan_set_host_chunk(cc_plan *plan, int frames_per_chunk);
+
+/*
  * cc_track_host -- the same path for HOST buffers (pageable or pinned): frames
  * are copied host->device in chunks overlapped with compute, results are
  * copied back, and the call returns after everything has completed.
  *   frames            HOST pointer, batch*H*W pixels
  *   dx, dy, peak      HOST pointers, batch float32 each (peak may be NULL)
- * Uses plan-owned streams and staging buffers (grown on first use).
+ * Uses plan-owned streams and staging buffers (grown on first use; shapes whose spectrum block lives in global
+ * scratch get a second scratch for the second stream).  On an error both streams are drained before the call
+ * returns: nothing is in flight on the caller's buffers afterwards.
  */
 cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
                         float *dx, float *dy, float *peak);
-
-/*
- * cc_track_latency_probe -- measurement aid for the real-time (batch-1)
- * mode of the paper (one displacement per camera frame):
- * n sequential calls of cc_track(batch = 1) on consecutive frames, each
- * followed by cudaStreamSynchronize, with the host monotonic clock read
- * around every call + synchronise pair.
- *   frames   DEVICE pointer, n frames (as for cc_track)
- *   dx,dy    DEVICE pointers, n float32 each (call i writes element i)
- *   peak     DEVICE pointer, n float32, or NULL
- *   lat_us   HOST pointer, receives n latencies in microseconds
- * Synchronises the stream.
- */
-cc_status cc_track_latency_probe(const cc_plan *plan, const void *frames, int n,
-                                 float *dx, float *dy, float *peak, double *lat_us, void *stream);
 
 /*
  * Real-time session -- the paper's real-time mode (PAPER.md:L102-104, L216:
@@ -194,16 +193,6 @@ cc_status cc_rt_submit(cc_rt *rt, const void *frame);
 cc_status cc_rt_wait(cc_rt *rt, float *dx, float *dy, float *peak);
 cc_status cc_rt_track(cc_rt *rt, const void *frame, float *dx, float *dy, float *peak);
 cc_status cc_rt_close(cc_rt *rt);
-
-/*
- * cc_rt_latency_probe -- measurement aid: n sequential cc_rt_track calls on
- * consecutive frames with the host monotonic clock around each call.
- *   frames   n frames, DEVICE or pinned mapped HOST pointer
- *   dx,dy,peak  HOST pointers, n float32 each (peak may be NULL)
- *   lat_us   HOST pointer, n latencies in microseconds
- */
-cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, float *dy, float *peak,
-                              double *lat_us);
 
 /*
  * cc_plan_enable_reference_update -- the paper's real-time analysis (Eq. (9)): after every
@@ -261,22 +250,6 @@ cc_status cc_plan_destroy(cc_plan *plan);
 
 /* Fills *info; returns CC_ERR_INVALID_ARG on NULL. */
 cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info);
-
-/*
- * cc_fp32_peak_probe -- measurement aid for bench.py's roofline: runs a
- * dependent-free FFMA loop on every SM and returns the achieved FP32 rate.
- *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
- */
-cc_status cc_fp32_peak_probe(double *tflops, void *stream);
-
-/*
- * cc_fp32_tile_probe -- second measurement aid: an 8x8 register-tile loop of scalar FFMA with all three operands
- * in registers (the instruction mix of a classic register-tiled FP32 GEMM inner loop, no memory traffic).  It stays
- * well below the lane rate that cc_fp32_peak_probe's constant-operand loop reaches; the library's own GEMM loops
- * therefore use the packed fma.rn.f32x2 form.
- *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
- */
-cc_status cc_fp32_tile_probe(double *tflops, void *stream);
 
 const char *cc_status_string(cc_status s);
 const char *cc_last_error(void); /* thread-local detail of the last failure */

@@ -1,0 +1,58 @@
+/*
+ * cc_bench.h -- measurement aids of libcc_b200.so (same library as include/cc.h, separate header: none of these
+ * is part of the tracking interface).  Used by bench.py and the GPU tests.
+ */
+#ifndef CC_BENCH_H
+#define CC_BENCH_H
+
+#include "cc.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/*
+ * cc_track_latency_probe -- measurement aid for the real-time (batch-1)
+ * mode of the paper (one displacement per camera frame):
+ * n sequential calls of cc_track(batch = 1) on consecutive frames, each
+ * followed by cudaStreamSynchronize, with the host monotonic clock read
+ * around every call + synchronise pair.
+ *   frames   DEVICE pointer, n frames (as for cc_track)
+ *   dx,dy    DEVICE pointers, n float32 each (call i writes element i)
+ *   peak     DEVICE pointer, n float32, or NULL
+ *   lat_us   HOST pointer, receives n latencies in microseconds
+ * Synchronises the stream.
+ */
+cc_status cc_track_latency_probe(const cc_plan *plan, const void *frames, int n,
+                                 float *dx, float *dy, float *peak, double *lat_us, void *stream);
+
+/*
+ * cc_rt_latency_probe -- measurement aid: n sequential cc_rt_track calls on
+ * consecutive frames with the host monotonic clock around each call.
+ *   frames   n frames, DEVICE or pinned mapped HOST pointer
+ *   dx,dy,peak  HOST pointers, n float32 each (peak may be NULL)
+ *   lat_us   HOST pointer, n latencies in microseconds
+ */
+cc_status cc_rt_latency_probe(cc_rt *rt, const void *frames, int n, float *dx, float *dy, float *peak,
+                              double *lat_us);
+
+/*
+ * cc_fp32_peak_probe -- measurement aid for bench.py's roofline: runs a
+ * dependent-free FFMA loop on every SM and returns the achieved FP32 rate.
+ *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
+ */
+cc_status cc_fp32_peak_probe(double *tflops, void *stream);
+
+/*
+ * cc_fp32_tile_probe -- second measurement aid: an 8x8 register-tile loop of scalar FFMA with all three operands
+ * in registers (the instruction mix of a classic register-tiled FP32 GEMM inner loop, no memory traffic).  It stays
+ * well below the lane rate that cc_fp32_peak_probe's constant-operand loop reaches; the library's own GEMM loops
+ * therefore use the packed fma.rn.f32x2 form.
+ *   tflops   HOST pointer, receives TFLOP/s (2 flop per FFMA)
+ */
+cc_status cc_fp32_tile_probe(double *tflops, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CC_BENCH_H */

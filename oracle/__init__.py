@@ -80,6 +80,14 @@ def _load():
                                      ctypes.POINTER(ctypes.c_float), ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
         lib.cco_iterate_reference.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                               ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.POINTER(_Result), dp, dp]
+        lib.cco_step_from_spectrum.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp,
+                                               ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
+        lib.cco_track_rt_sn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                        ctypes.POINTER(ctypes.c_float), ctypes.c_double, ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
+        lib.cco_iterate_reference_sn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                 ctypes.POINTER(ctypes.c_float), ctypes.c_double, ctypes.c_int, ctypes.POINTER(_Result), dp, dp]
+        lib.cco_step_from_spectrum_sn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp,
+                                                  ctypes.c_double, ctypes.c_double, ctypes.POINTER(_Result), dp, dp]
         lib.cco_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -251,9 +259,16 @@ _RES_DT = np.dtype([("dy", "f8"), ("dx", "f8"), ("peak", "f8"), ("wy", "i4"), ("
                     ("cc_top1", "f8"), ("cc_top2", "f8"), ("up_top1", "f8"), ("up_top2", "f8")], align=True)
 
 
-def track_rt(frames, reference, u: int, a0: float):
+def _status(rc, what):
+    if rc == -3:
+        raise ValueError("oracle %s: CC-SN needs E + epsilon > 0 in every pixel of the current reference" % what)
+    if rc:
+        raise RuntimeError("oracle %s failed: %d" % (what, rc))
+
+
+def track_rt(frames, reference, u: int, a0: float, method: str = "u", epsilon: float = 0.0):
     """PAPER.md:L102-108, Eq. (9): sequential tracking with the running reference image.  Returns
-    (TrackResult, G) with G the complex spectrum (H, W) of the last reference image."""
+    (TrackResult, G) with G the complex spectrum (H, W) of the last reference image.  method "sn": CC-SN (R19)."""
     frames = np.ascontiguousarray(frames)
     if frames.ndim == 2:
         frames = frames[None]
@@ -262,29 +277,61 @@ def track_rt(frames, reference, u: int, a0: float):
     ref = np.ascontiguousarray(reference, dtype=np.float32)
     out = (_Result * max(B, 1))()
     gr, gi = np.empty((H, W)), np.empty((H, W))
-    rc = _load().cco_track_rt(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
-                              ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(a0), out, _d(gr), _d(gi))
-    if rc:
-        raise RuntimeError("oracle cco_track_rt failed: %d" % rc)
+    if method == "sn":
+        rc = _load().cco_track_rt_sn(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                     ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(epsilon), float(a0), out, _d(gr), _d(gi))
+    else:
+        rc = _load().cco_track_rt(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                  ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(a0), out, _d(gr), _d(gi))
+    _status(rc, "cco_track_rt")
     arr = np.frombuffer(out, dtype=_RES_DT)[:B]
     res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
                                                 "up_top1", "up_top2")))
     return res, gr + 1j * gi
 
 
-def iterate_reference(frames, reference, u: int, n_iter: int):
-    """PAPER.md:L94-100, Eq. (8): n_iter passes of the offline analysis.  Returns (TrackResult of the last pass, G)."""
+def iterate_reference(frames, reference, u: int, n_iter: int, method: str = "u", epsilon: float = 0.0):
+    """PAPER.md:L94-100, Eq. (8): n_iter passes of the offline analysis.  Returns (TrackResult of the last pass, G).
+    method "sn": CC-SN (R19)."""
     frames = np.ascontiguousarray(frames)
     dt = {np.dtype(np.uint8): 0, np.dtype(np.uint16): 1}[frames.dtype]
     B, H, W = frames.shape
     ref = np.ascontiguousarray(reference, dtype=np.float32)
     out = (_Result * B)()
     gr, gi = np.empty((H, W)), np.empty((H, W))
-    rc = _load().cco_iterate_reference(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
-                                       ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), int(n_iter), out, _d(gr), _d(gi))
-    if rc:
-        raise RuntimeError("oracle cco_iterate_reference failed: %d" % rc)
+    if method == "sn":
+        rc = _load().cco_iterate_reference_sn(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                              ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), float(epsilon), int(n_iter), out,
+                                              _d(gr), _d(gi))
+    else:
+        rc = _load().cco_iterate_reference(frames.ctypes.data_as(ctypes.c_void_p), dt, B, H, W, int(u),
+                                           ref.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), int(n_iter), out, _d(gr), _d(gi))
+    _status(rc, "cco_iterate_reference")
     arr = np.frombuffer(out, dtype=_RES_DT)[:B]
     res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
                                                 "up_top1", "up_top2")))
     return res, gr + 1j * gi
+
+
+def step_from_spectrum(frame, G, u: int, a0: float, method: str = "u", epsilon: float = 0.0):
+    """PAPER.md:L106, Eq. (9), ONE step from a given reference spectrum G (complex (H, W), full spectrum): returns
+    (TrackResult of the frame against G, Gn = a0 F[frame aligned] + (1 - a0) G).  a0 = 1: the aligned spectrum (a
+    summand of Eq. (8)).  method "sn": the frame is measured by Eq. (7) with the weight 1/(E + epsilon), E = F^-1[G]."""
+    frame = np.ascontiguousarray(frame)
+    dt = {np.dtype(np.uint8): 0, np.dtype(np.uint16): 1}[frame.dtype]
+    H, W = frame.shape
+    G = np.asarray(G, dtype=np.complex128)
+    gr, gi = _f64(G.real), _f64(G.imag)
+    nr, ni = np.empty((H, W)), np.empty((H, W))
+    out = (_Result * 1)()
+    if method == "sn":
+        rc = _load().cco_step_from_spectrum_sn(frame.ctypes.data_as(ctypes.c_void_p), dt, H, W, int(u), _d(gr), _d(gi),
+                                               float(epsilon), float(a0), out, _d(nr), _d(ni))
+    else:
+        rc = _load().cco_step_from_spectrum(frame.ctypes.data_as(ctypes.c_void_p), dt, H, W, int(u), _d(gr), _d(gi), float(a0), out,
+                                            _d(nr), _d(ni))
+    _status(rc, "cco_step_from_spectrum")
+    arr = np.frombuffer(out, dtype=_RES_DT)[:1]
+    res = TrackResult(*(arr[k].copy() for k in ("dy", "dx", "peak", "wy", "wx", "m", "n", "cc_top1", "cc_top2",
+                                                "up_top1", "up_top2")))
+    return res, nr + 1j * ni

@@ -482,14 +482,112 @@ int cco_drift_correct(const float *dx, const float *dy, int n, double a0, double
     return 0;
 }
 
+/* ---- shared steps of the analyses with a moving reference image (Secs. III.A, III.B) ----
+ *
+ * measure_against_spectrum: steps O1-O7 for ONE frame against a reference given by its spectrum G = F[E]
+ * (the paper holds the RI in Fourier space, Eqs. (8), (9)).  I: the frame's pixels as
+ * doubles.  F (out): F[I].  work: 4*H*W doubles. */
+static int measure_against_spectrum(const double *I, const double *G_re, const double *G_im, int H, int W, int u,
+                                    double *F_re, double *F_im, double *work, cco_result *out)
+{
+    const size_t n = (size_t)H * W;
+    double *P_re = work, *P_im = work + n, *cc = work + 2 * n, *cc_im = work + 3 * n;
+    int rc = cco_dft2_real(I, H, W, F_re, F_im);                     /* O2 */
+    conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);              /* O3 */
+    if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);             /* O4 */
+    cco_result r;
+    memset(&r, 0, sizeof r);
+    long idx;                                                         /* O5 */
+    top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
+    int y0 = (int)(idx / W), x0 = (int)(idx % W);
+    r.wy = (2 * y0 >= H) ? y0 - H : y0;
+    r.wx = (2 * x0 >= W) ? x0 - W : x0;
+    if (u == 1) {
+        r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
+        r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
+    } else {
+        int M = cco_grid_size(u), c = M / 2;                          /* O6 */
+        if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL, &r.m, &r.n, &r.up_top1, &r.up_top2);
+        r.dy = (double)r.wy + (double)(r.m - c) / (double)u;          /* O7 */
+        r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
+        r.peak = r.up_top1;
+    }
+    *out = r;
+    return rc;
+}
+
+/* align_spectrum: the spectrum of "I(r - r0)", the new image translated by its detected displacement so that it
+ * lines up with the RI (Eq. (1); used in Eqs. (8), (9)).  With this build's sign (frame(r) ~
+ * reference(r - d), R1) the aligned image is J(r) = I(r + d):
+ *     F[J](k) = F[I](k) exp(+2 pi i (fy dy / H + fx dx / W)),   fy, fx the signed frequencies;
+ * d is fractional, and on the Nyquist bins (even H, W) the real minimal-bandwidth interpolant multiplies by
+ * cos(pi d) instead (R18). */
+static void align_spectrum(const double *F_re, const double *F_im, int H, int W, double dy, double dx,
+                           double *A_re, double *A_im)
+{
+    for (int ky = 0; ky < H; ++ky) {
+        double wyr, wyi;
+        if (H % 2 == 0 && 2 * ky == H) { wyr = cos(M_PI * dy); wyi = 0.0; }
+        else {
+            double fy = (2 * ky < H) ? ky : (double)ky - H;
+            wyr = cos(2.0 * M_PI * fy * dy / H); wyi = sin(2.0 * M_PI * fy * dy / H);
+        }
+        for (int kx = 0; kx < W; ++kx) {
+            double wxr, wxi;
+            if (W % 2 == 0 && 2 * kx == W) { wxr = cos(M_PI * dx); wxi = 0.0; }
+            else {
+                double fx = (2 * kx < W) ? kx : (double)kx - W;
+                wxr = cos(2.0 * M_PI * fx * dx / W); wxi = sin(2.0 * M_PI * fx * dx / W);
+            }
+            const double wr = wyr * wxr - wyi * wxi, wi = wyr * wxi + wyi * wxr;
+            const size_t k = (size_t)ky * W + kx;
+            A_re[k] = F_re[k] * wr - F_im[k] * wi;
+            A_im[k] = F_re[k] * wi + F_im[k] * wr;
+        }
+    }
+}
+
+static void pixels_to_double(const void *frames, int dtype, size_t n, int b, double *I)
+{
+    if (dtype == 0) {
+        const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
+        for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+    } else {
+        const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
+        for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
+    }
+}
+
+/* One step of Eq. (9) from a GIVEN reference spectrum: the frame is measured against G (O1-O7),
+ * then Gn = a0 F[I aligned] + (1 - a0) G.  a0 = 1 returns the aligned spectrum itself -- one summand of Eq. (8)
+ * (PAPER.md:L98); a0 = 0 leaves G unchanged.  CC-U.  Gn may be NULL. */
+int cco_step_from_spectrum(const void *frame, int dtype, int H, int W, int u, const double *G_re, const double *G_im,
+                           double a0, cco_result *out, double *Gn_re, double *Gn_im)
+{
+    if (!frame || !G_re || !G_im || !out || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) || !(a0 >= 0.0 && a0 <= 1.0))
+        return -2;
+    const size_t n = (size_t)H * W;
+    double *buf = (double *)malloc(sizeof(double) * n * 9);
+    if (!buf) return -1;
+    double *I = buf, *F_re = buf + n, *F_im = buf + 2 * n, *A_re = buf + 3 * n, *A_im = buf + 4 * n, *work = buf + 5 * n;
+    pixels_to_double(frame, dtype, n, 0, I);
+    int rc = measure_against_spectrum(I, G_re, G_im, H, W, u, F_re, F_im, work, out);
+    if (!rc && Gn_re && Gn_im) {
+        align_spectrum(F_re, F_im, H, W, out->dy, out->dx, A_re, A_im);
+        const double b1 = 1.0 - a0;
+        for (size_t k = 0; k < n; ++k) {
+            Gn_re[k] = a0 * A_re[k] + b1 * G_re[k];
+            Gn_im[k] = a0 * A_im[k] + b1 * G_im[k];
+        }
+    }
+    free(buf);
+    return rc ? -1 : 0;
+}
+
 /* Real-time analysis with a running reference image, Eq. (9):
- *     F[E_i] = a0 F[I_i(r - r0)] + b1 F[E_{i-1}],   b1 = 1 - a0,
- * "I(r - r0)" being the new image translated by its detected displacement so that it lines up with the RI
- * (Eq. (1)).  With this build's sign (frame(r) ~ reference(r - d), R1) the aligned
- * image is J(r) = I(r + d), i.e. F[J](k) = F[I](k) exp(+2 pi i (fy dy / H + fx dx / W)) with signed
- * frequencies; d is fractional, and on the Nyquist bins (even H, W) the real minimal-bandwidth interpolant
- * multiplies by cos(pi d) instead (R18).  Frames are processed strictly in order: frame i is
- * measured against E_{i-1} (the RI given by the caller is E_{-1}), then E_i is formed.  CC-U only.
+ *     F[E_i] = a0 F[I_i(r - r0)] + b1 F[E_{i-1}],   b1 = 1 - a0
+ * (alignment: align_spectrum above).  Frames are processed strictly in order: frame i is measured against
+ * E_{i-1} (the RI given by the caller is E_{-1}), then E_i is formed.  CC-U only.
  * G_re/G_im (H*W each, may be NULL) receive the spectrum of the last RI. */
 int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
                  const float *reference, double a0, cco_result *out, double *G_out_re, double *G_out_im)
@@ -499,62 +597,19 @@ int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
         return -2;
     const size_t n = (size_t)H * W;
     const double b1 = 1.0 - a0;
-    double *buf = (double *)malloc(sizeof(double) * n * 10);
+    double *buf = (double *)malloc(sizeof(double) * n * 12);
     if (!buf) return -1;
     double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
-           *P_re = buf + 6 * n, *P_im = buf + 7 * n, *cc = buf + 8 * n, *cc_im = buf + 9 * n;
+           *A_re = buf + 6 * n, *A_im = buf + 7 * n, *work = buf + 8 * n;
     for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
     int rc = cco_dft2_real(E, H, W, G_re, G_im);
     for (int b = 0; b < batch && !rc; ++b) {
-        if (dtype == 0) {
-            const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
-            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
-        } else {
-            const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
-            for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
-        }
-        rc = cco_dft2_real(I, H, W, F_re, F_im);
-        conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);
-        if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);
-        cco_result r;
-        memset(&r, 0, sizeof r);
-        long idx;
-        top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
-        int y0 = (int)(idx / W), x0 = (int)(idx % W);
-        r.wy = (2 * y0 >= H) ? y0 - H : y0;
-        r.wx = (2 * x0 >= W) ? x0 - W : x0;
-        if (u == 1) {
-            r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
-            r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
-        } else {
-            int M = cco_grid_size(u), c = M / 2;
-            if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL, &r.m, &r.n, &r.up_top1, &r.up_top2);
-            r.dy = (double)r.wy + (double)(r.m - c) / (double)u;
-            r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
-            r.peak = r.up_top1;
-        }
-        out[b] = r;
-        /* Eq. (9): G <- a0 F[I(r + d)] + b1 G */
-        for (int ky = 0; ky < H; ++ky) {
-            double wyr, wyi;
-            if (H % 2 == 0 && 2 * ky == H) { wyr = cos(M_PI * r.dy); wyi = 0.0; }
-            else {
-                double fy = (2 * ky < H) ? ky : (double)ky - H;
-                wyr = cos(2.0 * M_PI * fy * r.dy / H); wyi = sin(2.0 * M_PI * fy * r.dy / H);
-            }
-            for (int kx = 0; kx < W; ++kx) {
-                double wxr, wxi;
-                if (W % 2 == 0 && 2 * kx == W) { wxr = cos(M_PI * r.dx); wxi = 0.0; }
-                else {
-                    double fx = (2 * kx < W) ? kx : (double)kx - W;
-                    wxr = cos(2.0 * M_PI * fx * r.dx / W); wxi = sin(2.0 * M_PI * fx * r.dx / W);
-                }
-                const double wr = wyr * wxr - wyi * wxi, wi = wyr * wxi + wyi * wxr;
-                const size_t k = (size_t)ky * W + kx;
-                const double sr = F_re[k] * wr - F_im[k] * wi, si = F_re[k] * wi + F_im[k] * wr;
-                G_re[k] = a0 * sr + b1 * G_re[k];
-                G_im[k] = a0 * si + b1 * G_im[k];
-            }
+        pixels_to_double(frames, dtype, n, b, I);
+        rc = measure_against_spectrum(I, G_re, G_im, H, W, u, F_re, F_im, work, &out[b]);
+        align_spectrum(F_re, F_im, H, W, out[b].dy, out[b].dx, A_re, A_im);
+        for (size_t k = 0; k < n; ++k) {                 /* Eq. (9) */
+            G_re[k] = a0 * A_re[k] + b1 * G_re[k];
+            G_im[k] = a0 * A_im[k] + b1 * G_im[k];
         }
     }
     if (!rc && G_out_re && G_out_im) {
@@ -567,76 +622,31 @@ int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
 
 /* Offline analysis, Eq. (8): for each complete pass through the images,
  *     F[E_n] = (1/N) sum_i F[I_i(r - r0_i)],
- * every displacement r0_i of the pass being measured against the constant RI E_{n-1}; the aligned image is
- * I_i(r + d_i) as in cco_track_rt (R18).  n_iter passes are made, starting from the caller's reference
- * (the paper starts from E_0 = I_0: pass the first frame).  `out` receives the displacements measured in the LAST
- * pass (against E_{n_iter-1}), G_out the spectrum of E_{n_iter}.  CC-U.  Sequential. */
+ * every displacement r0_i of the pass being measured against the constant RI E_{n-1} (alignment: align_spectrum
+ * above).  n_iter passes are made, starting from the caller's reference (the paper starts from E_0 = I_0: pass the
+ * first frame).  `out` receives the displacements measured in the LAST pass (against E_{n_iter-1}), G_out the
+ * spectrum of E_{n_iter}.  CC-U.  Sequential. */
 int cco_iterate_reference(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
                           int n_iter, cco_result *out, double *G_out_re, double *G_out_im)
 {
     if (!frames || !reference || !out || batch <= 0 || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) || n_iter < 1)
         return -2;
     const size_t n = (size_t)H * W;
-    double *buf = (double *)malloc(sizeof(double) * n * 12);
+    double *buf = (double *)malloc(sizeof(double) * n * 14);
     if (!buf) return -1;
     double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
-           *P_re = buf + 6 * n, *P_im = buf + 7 * n, *cc = buf + 8 * n, *cc_im = buf + 9 * n, *A_re = buf + 10 * n,
-           *A_im = buf + 11 * n;
+           *A_re = buf + 6 * n, *A_im = buf + 7 * n, *S_re = buf + 8 * n, *S_im = buf + 9 * n, *work = buf + 10 * n;
     for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
     int rc = cco_dft2_real(E, H, W, G_re, G_im);
     for (int it = 0; it < n_iter && !rc; ++it) {
-        for (size_t i = 0; i < n; ++i) A_re[i] = A_im[i] = 0.0;
+        for (size_t i = 0; i < n; ++i) S_re[i] = S_im[i] = 0.0;
         for (int b = 0; b < batch && !rc; ++b) {
-            if (dtype == 0) {
-                const unsigned char *p = (const unsigned char *)frames + (size_t)b * n;
-                for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
-            } else {
-                const unsigned short *p = (const unsigned short *)frames + (size_t)b * n;
-                for (size_t i = 0; i < n; ++i) I[i] = (double)p[i];
-            }
-            rc = cco_dft2_real(I, H, W, F_re, F_im);
-            conj_product(F_re, F_im, G_re, G_im, n, P_re, P_im);
-            if (!rc) rc = cco_idft2(P_re, P_im, H, W, cc, cc_im);
-            cco_result r;
-            memset(&r, 0, sizeof r);
-            long idx;
-            top_two(cc, (long)n, &idx, &r.cc_top1, &r.cc_top2);
-            int y0 = (int)(idx / W), x0 = (int)(idx % W);
-            r.wy = (2 * y0 >= H) ? y0 - H : y0;
-            r.wx = (2 * x0 >= W) ? x0 - W : x0;
-            if (u == 1) {
-                r.dy = r.wy; r.dx = r.wx; r.peak = r.cc_top1;
-                r.up_top1 = r.cc_top1; r.up_top2 = r.cc_top2;
-            } else {
-                int M = cco_grid_size(u), c = M / 2;
-                if (!rc) rc = cco_upsampled(P_re, P_im, H, W, u, y0, x0, NULL, &r.m, &r.n, &r.up_top1, &r.up_top2);
-                r.dy = (double)r.wy + (double)(r.m - c) / (double)u;
-                r.dx = (double)r.wx + (double)(r.n - c) / (double)u;
-                r.peak = r.up_top1;
-            }
-            out[b] = r;
-            for (int ky = 0; ky < H; ++ky) {          /* A += F[I_b(r + d_b)] */
-                double wyr, wyi;
-                if (H % 2 == 0 && 2 * ky == H) { wyr = cos(M_PI * r.dy); wyi = 0.0; }
-                else {
-                    double fy = (2 * ky < H) ? ky : (double)ky - H;
-                    wyr = cos(2.0 * M_PI * fy * r.dy / H); wyi = sin(2.0 * M_PI * fy * r.dy / H);
-                }
-                for (int kx = 0; kx < W; ++kx) {
-                    double wxr, wxi;
-                    if (W % 2 == 0 && 2 * kx == W) { wxr = cos(M_PI * r.dx); wxi = 0.0; }
-                    else {
-                        double fx = (2 * kx < W) ? kx : (double)kx - W;
-                        wxr = cos(2.0 * M_PI * fx * r.dx / W); wxi = sin(2.0 * M_PI * fx * r.dx / W);
-                    }
-                    const double wr = wyr * wxr - wyi * wxi, wi = wyr * wxi + wyi * wxr;
-                    const size_t k = (size_t)ky * W + kx;
-                    A_re[k] += F_re[k] * wr - F_im[k] * wi;
-                    A_im[k] += F_re[k] * wi + F_im[k] * wr;
-                }
-            }
+            pixels_to_double(frames, dtype, n, b, I);
+            rc = measure_against_spectrum(I, G_re, G_im, H, W, u, F_re, F_im, work, &out[b]);
+            align_spectrum(F_re, F_im, H, W, out[b].dy, out[b].dx, A_re, A_im);
+            for (size_t k = 0; k < n; ++k) { S_re[k] += A_re[k]; S_im[k] += A_im[k]; }
         }
-        for (size_t i = 0; i < n; ++i) { G_re[i] = A_re[i] / batch; G_im[i] = A_im[i] / batch; }   /* Eq. (8) */
+        for (size_t i = 0; i < n; ++i) { G_re[i] = S_re[i] / batch; G_im[i] = S_im[i] / batch; }   /* Eq. (8) */
     }
     if (!rc && G_out_re && G_out_im) {
         memcpy(G_out_re, G_re, sizeof(double) * n);
@@ -644,4 +654,139 @@ int cco_iterate_reference(const void *frames, int dtype, int batch, int H, int W
     }
     free(buf);
     return rc ? -1 : 0;
+}
+
+/* ---- CC-SN with a moving reference image (R19) -------------------------------------------------------
+ * the discussion of Secs. III.A/III.B "can be easily adapted for the CC-SN method by replacing
+ * I_i -> I_i'^2 and E_n -> 1/E_n".  Substituted literally into Eqs. (8)/(9) this would average I'^2 into "1/E",
+ * which is neither the reciprocal of an image average nor dimensionally consistent with Eq. (7).  Reading taken:
+ * the replacement applies to the CORRELATION (Eq. (7) instead of Eq. (4)), while the RI keeps the meaning Eq. (5)
+ * gives it -- the estimate of the average image ("see Sec. III for how this [the offset] affects the RI",
+ * the RI is built from the offset images I' = I + eps).  So the state is F[E'], updated by Eqs. (8)/(9)
+ * from the ALIGNED OFFSET IMAGES I_i', and every frame is measured by Eq. (7) with the weight 1/E' of the current
+ * state.  Because the alignment leaves the DC bin untouched and a0 + b1 = 1 (and a mean has weights summing to 1),
+ * E'_i = E_i + eps exactly, E_i being the same filter on the raw images: the state is held as G = F[E] and
+ * the offset is added when the weight is formed. */
+
+/* Gw = F[-1/(E + eps)] from the state G = F[E]  (E = Re F^-1[G]); fails (-3) unless E + eps > 0 everywhere.
+ * work: 3*H*W doubles. */
+static int sn_weight_spectrum(const double *G_re, const double *G_im, int H, int W, double eps,
+                              double *Gw_re, double *Gw_im, double *work)
+{
+    const size_t n = (size_t)H * W;
+    double *e_re = work, *e_im = work + n, *w = work + 2 * n;
+    if (cco_idft2(G_re, G_im, H, W, e_re, e_im)) return -1;
+    for (size_t i = 0; i < n; ++i) {
+        const double ep = e_re[i] + eps;
+        if (!(ep > 0.0)) return -3;
+        w[i] = -1.0 / ep;                                   /* -(1/E'), Eq. (7); minimum of S = maximum of -S (R15) */
+    }
+    return cco_dft2_real(w, H, W, Gw_re, Gw_im);
+}
+
+/* One frame by Eq. (7) against the state G = F[E]; F (out) = F[I] of the RAW frame (what Eqs. (8)/(9) align).
+ * work: 9*H*W doubles. */
+static int measure_sn_against_state(const double *I, const double *G_re, const double *G_im, int H, int W, int u, double eps,
+                                    double *F_re, double *F_im, double *work, cco_result *out)
+{
+    const size_t n = (size_t)H * W;
+    double *Gw_re = work, *Gw_im = work + n, *I2 = work + 2 * n, *F2_re = work + 3 * n, *F2_im = work + 4 * n, *w2 = work + 5 * n;
+    int rc = sn_weight_spectrum(G_re, G_im, H, W, eps, Gw_re, Gw_im, w2);
+    if (rc) return rc;
+    for (size_t i = 0; i < n; ++i) I2[i] = (I[i] + eps) * (I[i] + eps);        /* I'^2, Eq. (7) */
+    rc = measure_against_spectrum(I2, Gw_re, Gw_im, H, W, u, F2_re, F2_im, w2, out);
+    out->peak = -out->peak;                                  /* report S, as cco_track_sn does */
+    out->cc_top1 = -out->cc_top1; out->cc_top2 = -out->cc_top2;
+    out->up_top1 = -out->up_top1; out->up_top2 = -out->up_top2;
+    if (!rc) rc = cco_dft2_real(I, H, W, F_re, F_im);
+    return rc;
+}
+
+int cco_step_from_spectrum_sn(const void *frame, int dtype, int H, int W, int u, const double *G_re, const double *G_im,
+                              double eps, double a0, cco_result *out, double *Gn_re, double *Gn_im)
+{
+    if (!frame || !G_re || !G_im || !out || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) || !(a0 >= 0.0 && a0 <= 1.0) ||
+        !(eps >= 0.0))
+        return -2;
+    const size_t n = (size_t)H * W;
+    double *buf = (double *)malloc(sizeof(double) * n * 14);
+    if (!buf) return -1;
+    double *I = buf, *F_re = buf + n, *F_im = buf + 2 * n, *A_re = buf + 3 * n, *A_im = buf + 4 * n, *work = buf + 5 * n;
+    pixels_to_double(frame, dtype, n, 0, I);
+    int rc = measure_sn_against_state(I, G_re, G_im, H, W, u, eps, F_re, F_im, work, out);
+    if (!rc && Gn_re && Gn_im) {
+        align_spectrum(F_re, F_im, H, W, out->dy, out->dx, A_re, A_im);
+        const double b1 = 1.0 - a0;
+        for (size_t k = 0; k < n; ++k) {
+            Gn_re[k] = a0 * A_re[k] + b1 * G_re[k];
+            Gn_im[k] = a0 * A_im[k] + b1 * G_im[k];
+        }
+    }
+    free(buf);
+    return rc == -3 ? -3 : (rc ? -1 : 0);
+}
+
+int cco_track_rt_sn(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference, double eps,
+                    double a0, cco_result *out, double *G_out_re, double *G_out_im)
+{
+    if (!frames || !reference || !out || batch < 0 || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) ||
+        !(a0 >= 0.0 && a0 <= 1.0) || !(eps >= 0.0))
+        return -2;
+    const size_t n = (size_t)H * W;
+    const double b1 = 1.0 - a0;
+    double *buf = (double *)malloc(sizeof(double) * n * 17);
+    if (!buf) return -1;
+    double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
+           *A_re = buf + 6 * n, *A_im = buf + 7 * n, *work = buf + 8 * n;
+    for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    int rc = cco_dft2_real(E, H, W, G_re, G_im);
+    for (int b = 0; b < batch && !rc; ++b) {
+        pixels_to_double(frames, dtype, n, b, I);
+        rc = measure_sn_against_state(I, G_re, G_im, H, W, u, eps, F_re, F_im, work, &out[b]);
+        if (rc) break;
+        align_spectrum(F_re, F_im, H, W, out[b].dy, out[b].dx, A_re, A_im);
+        for (size_t k = 0; k < n; ++k) {                 /* Eq. (9) on the raw images; E' = E + eps (see above) */
+            G_re[k] = a0 * A_re[k] + b1 * G_re[k];
+            G_im[k] = a0 * A_im[k] + b1 * G_im[k];
+        }
+    }
+    if (!rc && G_out_re && G_out_im) {
+        memcpy(G_out_re, G_re, sizeof(double) * n);
+        memcpy(G_out_im, G_im, sizeof(double) * n);
+    }
+    free(buf);
+    return rc == -3 ? -3 : (rc ? -1 : 0);
+}
+
+int cco_iterate_reference_sn(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
+                             double eps, int n_iter, cco_result *out, double *G_out_re, double *G_out_im)
+{
+    if (!frames || !reference || !out || batch <= 0 || H <= 0 || W <= 0 || u < 1 || (dtype != 0 && dtype != 1) || n_iter < 1 ||
+        !(eps >= 0.0))
+        return -2;
+    const size_t n = (size_t)H * W;
+    double *buf = (double *)malloc(sizeof(double) * n * 19);
+    if (!buf) return -1;
+    double *E = buf, *G_re = buf + n, *G_im = buf + 2 * n, *I = buf + 3 * n, *F_re = buf + 4 * n, *F_im = buf + 5 * n,
+           *A_re = buf + 6 * n, *A_im = buf + 7 * n, *S_re = buf + 8 * n, *S_im = buf + 9 * n, *work = buf + 10 * n;
+    for (size_t i = 0; i < n; ++i) E[i] = (double)reference[i];
+    int rc = cco_dft2_real(E, H, W, G_re, G_im);
+    for (int it = 0; it < n_iter && !rc; ++it) {
+        for (size_t i = 0; i < n; ++i) S_re[i] = S_im[i] = 0.0;
+        for (int b = 0; b < batch && !rc; ++b) {
+            pixels_to_double(frames, dtype, n, b, I);
+            rc = measure_sn_against_state(I, G_re, G_im, H, W, u, eps, F_re, F_im, work, &out[b]);
+            if (rc) break;
+            align_spectrum(F_re, F_im, H, W, out[b].dy, out[b].dx, A_re, A_im);
+            for (size_t k = 0; k < n; ++k) { S_re[k] += A_re[k]; S_im[k] += A_im[k]; }
+        }
+        if (rc) break;
+        for (size_t i = 0; i < n; ++i) { G_re[i] = S_re[i] / batch; G_im[i] = S_im[i] / batch; }   /* Eq. (8) */
+    }
+    if (!rc && G_out_re && G_out_im) {
+        memcpy(G_out_re, G_re, sizeof(double) * n);
+        memcpy(G_out_im, G_im, sizeof(double) * n);
+    }
+    free(buf);
+    return rc == -3 ? -3 : (rc ? -1 : 0);
 }

@@ -21,7 +21,8 @@
  *   trigonometric interpolant).
  *
  * Parity pins: every function below is pinned by tests/test_oracle_pins.py
- * (P1-P10); nothing here is "parity unpinned".
+ * (P0-P11, SN1-5, D1-3, RI1-3, IT1-3, ST1, SR1-6); nothing here is
+ * "parity unpinned".
  */
 #ifndef CC_ORACLE_H
 #define CC_ORACLE_H
@@ -125,6 +126,29 @@ int cco_track_rt(const void *frames, int dtype, int batch, int H, int W, int u,
  * F[I_i(r + d_i)] (alignment as in cco_track_rt).  out: displacements of the last pass; G_out: spectrum of E_{n_iter}. */
 int cco_iterate_reference(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
                           int n_iter, cco_result *out, double *G_out_re, double *G_out_im);
+
+/* One step of Eq. (9) from a GIVEN reference spectrum G = F[E] (H*W complex, full spectrum): O1-O7 of `frame`
+ * against G, then Gn = a0 F[frame aligned] + (1 - a0) G.  a0 = 1: Gn is the aligned spectrum itself, one summand of
+ * Eq. (8).  Lets a test drive the oracle from the state another implementation holds (input only).  CC-U.
+ * Shares its two steps (measure against a spectrum; align by the Fourier shift theorem) with cco_track_rt and
+ * cco_iterate_reference, so the pins of either function pin all three. */
+int cco_step_from_spectrum(const void *frame, int dtype, int H, int W, int u, const double *G_re, const double *G_im,
+                           double a0, cco_result *out, double *Gn_re, double *Gn_im);
+
+/* CC-SN with a moving reference image (PAPER.md:L92 applied to Eqs. (8), (9); R19): the state is the
+ * spectrum G = F[E] of the average RAW image; every frame is measured by Eq. (7) with the weight 1/(E + eps) formed
+ * from the current state (E = Re F^-1[G]; returns -3 unless E + eps > 0 everywhere), then the state is updated with
+ * the frame aligned by its displacement, exactly as in the CC-U functions (E' = E + eps holds identically).
+ * Results report S (the minimised sum) like cco_track_sn.
+ *   cco_track_rt_sn            Eq. (9), frames in order (as cco_track_rt)
+ *   cco_iterate_reference_sn   Eq. (8), n_iter passes (as cco_iterate_reference)
+ *   cco_step_from_spectrum_sn  one step from a given state (as cco_step_from_spectrum) */
+int cco_track_rt_sn(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference, double eps,
+                    double a0, cco_result *out, double *G_out_re, double *G_out_im);
+int cco_iterate_reference_sn(const void *frames, int dtype, int batch, int H, int W, int u, const float *reference,
+                             double eps, int n_iter, cco_result *out, double *G_out_re, double *G_out_im);
+int cco_step_from_spectrum_sn(const void *frame, int dtype, int H, int W, int u, const double *G_re, const double *G_im,
+                              double eps, double a0, cco_result *out, double *Gn_re, double *Gn_im);
 
 int cco_num_threads(void);
 

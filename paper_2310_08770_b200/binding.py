@@ -19,7 +19,8 @@ CC_U8, CC_U16 = 0, 1
 _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
-EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host", "cc_plan_destroy",
+EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host",
+           "cc_plan_set_host_chunk", "cc_plan_destroy",
            "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_track_accumulate",
            "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
@@ -64,6 +65,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_track_profile.restype = ci
         lib.cc_track_host.argtypes = [vp, vp, ci, vp, vp, vp]
         lib.cc_track_host.restype = ci
+        lib.cc_plan_set_host_chunk.argtypes = [vp, ci]
+        lib.cc_plan_set_host_chunk.restype = ci
         lib.cc_track_latency_probe.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp]
         lib.cc_track_latency_probe.restype = ci
         lib.cc_rt_open.argtypes = [vp, ci, ctypes.POINTER(vp)]
@@ -250,6 +253,10 @@ class Plan:
                                                      pk.data_ptr(), lat.ctypes.data_as(ctypes.c_void_p),
                                                      torch.cuda.current_stream(dev).cuda_stream))
         return dx, dy, pk, lat
+
+    def set_host_chunk(self, frames_per_chunk: int):
+        """cc_plan_set_host_chunk: frames per host->device chunk of track_host (0: default)."""
+        _check(load_library().cc_plan_set_host_chunk(self._h, int(frames_per_chunk)))
 
     def track_host(self, frames_np, dx=None, dy=None, peak=None):
         """cc_track_host: host numpy frames in, host numpy results out (H2D/D2H inside)."""

@@ -33,7 +33,11 @@ def variants():
 
 
 def _newest_src():
-    return max(os.path.getmtime(os.path.join(CSRC, f)) for f in os.listdir(CSRC))
+    """Newest of the sources, the public headers (enums and struct layouts the binding mirrors) and this file (FLAGS)."""
+    inc = os.path.join(os.path.dirname(HERE), "include")
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.abspath(__file__)]
+    files += [os.path.join(inc, f) for f in os.listdir(inc) if f.endswith(".h")]
+    return max(os.path.getmtime(f) for f in files)
 
 
 def _run(cmd, log):

@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "../../include/cc.h"
+#include "../../include/cc_bench.h"
 #include "cc_common.h"
 
 // ------------------------------------------------------------------ variants
@@ -60,6 +61,7 @@ struct VarPlan {
     uint32_t sched_head[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     float *nyqc = nullptr;      // device: cos(pi e / u)
     float2 *Sg = nullptr;       // global spectrum scratch (s_global variants)
+    float2 *Sg_alt = nullptr;   // second copy, used by cc_track_host's second stream (allocated on first use)
     size_t sg_bytes = 0;
     bool ready = false;
 };
@@ -98,6 +100,7 @@ struct cc_plan {
     void *dframes[2] = {nullptr, nullptr};
     float *dres = nullptr;  // [3][cap]
     int chunk_cap = 0, res_cap = 0;
+    int host_chunk = 0;     // frames per cc_track_host chunk (0: about 64 MB of frames)
 };
 
 // ------------------------------------------------------------------ host fp64 FFT (plan time only)
@@ -334,7 +337,8 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
     cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab), cudaFree(plan->ri_emean), cudaFree(plan->col_freq);
     cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
-    for (VarPlan *vp : {&plan->thr, &plan->lat}) cudaFree(vp->Sg), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
+    for (VarPlan *vp : {&plan->thr, &plan->lat})
+        cudaFree(vp->Sg), cudaFree(vp->Sg_alt), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
         if (plan->hev[i]) cudaEventDestroy(plan->hev[i]);
@@ -536,7 +540,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
 }
 
 static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
-                            int *iy, int *ix, unsigned long long *phase_clk, void *stream)
+                            int *iy, int *ix, unsigned long long *phase_clk, void *stream, int sg_slot = 0)
 {
     if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track: bad plan or batch");
     if (batch == 0) return CC_OK;
@@ -549,6 +553,7 @@ static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, 
     CcParams p{};
     fill_params(plan, *vp, p);
     p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix, p.phase_clk = phase_clk;
+    if (sg_slot == 1 && vp->Sg_alt) p.Sg = vp->Sg_alt;  // cc_track_host's second stream: its own spectrum scratch
     const int ncl = ri ? 1 : std::min(batch, vp->max_clusters);
     cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
@@ -574,14 +579,22 @@ extern "C" cc_status cc_track(const cc_plan *plan, const void *frames, int batch
     return track_impl(plan, frames, batch, dx, dy, peak, nullptr, nullptr, nullptr, stream);
 }
 
+extern "C" cc_status cc_plan_set_host_chunk(cc_plan *plan, int frames_per_chunk)
+{
+    if (!plan || frames_per_chunk < 0) return fail(CC_ERR_INVALID_ARG, "cc_plan_set_host_chunk: bad plan or chunk");
+    plan->host_chunk = frames_per_chunk;
+    return CC_OK;
+}
+
 extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak)
 {
     if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_host: bad plan or batch");
     if (batch == 0) return CC_OK;
     if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track_host: null pointer");
     const size_t fbytes = (size_t)plan->H * plan->W * (plan->dtype == CC_U8 ? 1 : 2);
-    // chunk: about 64 MB of frames, at least one wave of clusters
-    int chunk = (int)std::max<size_t>((size_t)plan->thr.max_clusters, (size_t)(64u << 20) / fbytes);
+    // chunk: about 64 MB of frames, at least one wave of clusters (or what cc_plan_set_host_chunk asked for)
+    int chunk = plan->host_chunk > 0 ? plan->host_chunk
+                                     : (int)std::max<size_t>((size_t)plan->thr.max_clusters, (size_t)(64u << 20) / fbytes);
     chunk = std::min(chunk, batch);
     if (!plan->hs[0]) {
         for (int i = 0; i < 2; ++i) {
@@ -593,6 +606,7 @@ extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
         for (int i = 0; i < 2; ++i) {
             cudaFree(plan->dframes[i]);
             plan->dframes[i] = nullptr;
+            plan->chunk_cap = 0;
             CK(cudaMalloc(&plan->dframes[i], (size_t)chunk * fbytes));
         }
         plan->chunk_cap = chunk;
@@ -600,25 +614,37 @@ extern "C" cc_status cc_track_host(cc_plan *plan, const void *frames, int batch,
     if (batch > plan->res_cap) {
         cudaFree(plan->dres);
         plan->dres = nullptr;
+        plan->res_cap = 0;
         CK(cudaMalloc((void **)&plan->dres, (size_t)3 * batch * sizeof(float)));
         plan->res_cap = batch;
     }
+    // variants that keep the spectrum block in plan-owned global scratch (1024 x 1024): the kernels of the two streams
+    // overlap, so the second stream gets a scratch of its own
+    for (VarPlan *vp : {&plan->thr, &plan->lat})
+        if (vp->ready && vp->v.s_global && !vp->Sg_alt) CK(cudaMalloc((void **)&vp->Sg_alt, vp->sg_bytes));
     float *ddx = plan->dres, *ddy = plan->dres + plan->res_cap, *dpk = plan->dres + 2 * (size_t)plan->res_cap;
-    int nchunks = (batch + chunk - 1) / chunk;
-    for (int ci = 0; ci < nchunks; ++ci) {
+    const int nchunks = (batch + chunk - 1) / chunk;
+    cc_status st = CC_OK;
+    cudaError_t ce = cudaSuccess;
+    for (int ci = 0; ci < nchunks && st == CC_OK && ce == cudaSuccess; ++ci) {
         // with the running reference image (Eq. (9)) the chunks must run in order: one stream, one staging buffer
         const int b = plan->ri_a0 > 0.0 ? 0 : (ci & 1), f0 = ci * chunk, n = std::min(chunk, batch - f0);
         cudaStream_t s = plan->hs[b];
-        CK(cudaMemcpyAsync(plan->dframes[b], (const unsigned char *)frames + (size_t)f0 * fbytes, (size_t)n * fbytes,
-                           cudaMemcpyHostToDevice, s));
-        cc_status st = cc_track(plan, plan->dframes[b], n, ddx + f0, ddy + f0, dpk + f0, (void *)s);
-        if (st != CC_OK) return st;
-        CK(cudaMemcpyAsync(dx + f0, ddx + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
-        CK(cudaMemcpyAsync(dy + f0, ddy + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
-        if (peak) CK(cudaMemcpyAsync(peak + f0, dpk + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s));
+        ce = cudaMemcpyAsync(plan->dframes[b], (const unsigned char *)frames + (size_t)f0 * fbytes, (size_t)n * fbytes,
+                             cudaMemcpyHostToDevice, s);
+        if (ce != cudaSuccess) break;
+        st = track_impl(plan, plan->dframes[b], n, ddx + f0, ddy + f0, dpk + f0, nullptr, nullptr, nullptr, (void *)s, b);
+        if (st != CC_OK) break;
+        ce = cudaMemcpyAsync(dx + f0, ddx + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(dy + f0, ddy + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess && peak) ce = cudaMemcpyAsync(peak + f0, dpk + f0, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, s);
     }
-    CK(cudaStreamSynchronize(plan->hs[0]));
-    CK(cudaStreamSynchronize(plan->hs[1]));
+    // drain both streams on every path: no copy into or out of the caller's buffers is in flight after the return
+    const cudaError_t s0 = cudaStreamSynchronize(plan->hs[0]), s1 = cudaStreamSynchronize(plan->hs[1]);
+    if (st != CC_OK) return st;
+    if (ce != cudaSuccess) return fail_cuda(ce, "cc_track_host: copy");
+    if (s0 != cudaSuccess) return fail_cuda(s0, "cc_track_host: stream 0");
+    if (s1 != cudaSuccess) return fail_cuda(s1, "cc_track_host: stream 1");
     return CC_OK;
 }
 
@@ -659,6 +685,7 @@ struct cc_rt {
     const void *pending = nullptr;             // frame of that submission (for a restart)
     bool in_flight = false;
     unsigned long long timeout_ns = 0;
+    float2 *Sg = nullptr;                      // the session's own spectrum scratch (s_global variants)
 };
 
 static double mono_us()
@@ -684,6 +711,7 @@ static cc_status rt_launch(cc_rt *rt)
     p.rt_res = (float *)((char *)rt->dbox + 64);
     p.rt_alive = (int *)((char *)rt->dbox + 128);
     p.rt_timeout_ns = rt->timeout_ns;
+    if (rt->Sg) p.Sg = rt->Sg;  // not the plan's: cc_track(batch 1) on the same plan may run beside the session
     cudaError_t e = rt->vp->v.launch(p, 1, rt->vp->smem_bytes, rt->stream);
     if (e != cudaSuccess) {
         *rt->alive = 0;
@@ -704,6 +732,7 @@ extern "C" cc_status cc_rt_close(cc_rt *rt)
         cudaStreamDestroy(rt->stream);
     }
     if (rt->hbox) cudaFreeHost(rt->hbox);
+    cudaFree(rt->Sg);
     delete rt;
     return CC_OK;
 }
@@ -722,9 +751,13 @@ extern "C" cc_status cc_rt_open(cc_plan *plan, int idle_timeout_ms, cc_rt **out)
         e = cudaHostGetDevicePointer(&rt->dbox, rt->hbox, 0);
     }
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&rt->stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess && rt->vp->v.s_global)
+        e = cudaMalloc((void **)&rt->Sg, (size_t)rt->vp->v.CS * ((size_t)plan->H * (plan->W / 2 / rt->vp->v.CS)) * sizeof(float2));
     if (e != cudaSuccess) {
         cc_status s = fail_cuda(e, "cc_rt_open");
         if (rt->hbox) cudaFreeHost(rt->hbox);
+        if (rt->stream) cudaStreamDestroy(rt->stream);
+        cudaFree(rt->Sg);
         delete rt;
         return s;
     }
@@ -1045,7 +1078,22 @@ extern "C" cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info)
     return CC_OK;
 }
 
-// ------------------------------------------------------------------ FP32 peak probe
+// ------------------------------------------------------------------ FP32 peak probes (include/cc_bench.h)
+namespace {
+struct DevBuf {  // freed on every return path
+    void *p = nullptr;
+    ~DevBuf() { cudaFree(p); }
+};
+struct EvPair {
+    cudaEvent_t a = nullptr, b = nullptr;
+    ~EvPair()
+    {
+        if (a) cudaEventDestroy(a);
+        if (b) cudaEventDestroy(b);
+    }
+};
+}  // namespace
+
 __global__ void __launch_bounds__(1024, 1) cc_ffma_probe_kernel(float *out, int iters)
 {
     float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f,
@@ -1070,11 +1118,13 @@ extern "C" cc_status cc_fp32_peak_probe(double *tflops, void *stream)
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int blocks = sms * 2, threads = 1024, iters = 4096;
-    float *out = nullptr;
-    CK(cudaMalloc((void **)&out, (size_t)blocks * threads * sizeof(float)));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
+    DevBuf ob;
+    EvPair ev;
+    CK(cudaMalloc(&ob.p, (size_t)blocks * threads * sizeof(float)));
+    float *out = (float *)ob.p;
+    CK(cudaEventCreate(&ev.a));
+    CK(cudaEventCreate(&ev.b));
+    const cudaEvent_t e0 = ev.a, e1 = ev.b;
     cudaStream_t s = (cudaStream_t)stream;
     cc_ffma_probe_kernel<<<blocks, threads, 0, s>>>(out, 64);
     float best = 1e30f;
@@ -1087,7 +1137,6 @@ extern "C" cc_status cc_fp32_peak_probe(double *tflops, void *stream)
         CK(cudaEventElapsedTime(&ms, e0, e1));
         best = std::min(best, ms);
     }
-    cudaEventDestroy(e0), cudaEventDestroy(e1), cudaFree(out);
     const double flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)blocks * (double)threads;
     *tflops = flops / ((double)best * 1e-3) / 1e12;
     return CC_OK;
@@ -1126,13 +1175,15 @@ extern "C" cc_status cc_fp32_tile_probe(double *tflops, void *stream)
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int blocks = sms, threads = 256, iters = 20000;  // 8 warps per SM, as the fused kernel runs
-    float *out = nullptr, *in = nullptr;
-    CK(cudaMalloc((void **)&out, (size_t)blocks * threads * sizeof(float)));
-    CK(cudaMalloc((void **)&in, 4096));
+    DevBuf ob, ib;
+    EvPair ev;
+    CK(cudaMalloc(&ob.p, (size_t)blocks * threads * sizeof(float)));
+    CK(cudaMalloc(&ib.p, 4096));
+    float *out = (float *)ob.p, *in = (float *)ib.p;
     CK(cudaMemset(in, 0, 4096));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
+    CK(cudaEventCreate(&ev.a));
+    CK(cudaEventCreate(&ev.b));
+    const cudaEvent_t e0 = ev.a, e1 = ev.b;
     cudaStream_t s = (cudaStream_t)stream;
     cc_ffma_tile_probe_kernel<<<blocks, threads, 0, s>>>(out, in, 64);
     float best = 1e30f;
@@ -1145,7 +1196,6 @@ extern "C" cc_status cc_fp32_tile_probe(double *tflops, void *stream)
         CK(cudaEventElapsedTime(&ms, e0, e1));
         best = std::min(best, ms);
     }
-    cudaEventDestroy(e0), cudaEventDestroy(e1), cudaFree(out), cudaFree(in);
     *tflops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads / ((double)best * 1e-3) / 1e12;
     return CC_OK;
 }

@@ -19,9 +19,14 @@ def lib():
 
 
 def _declared_functions():
-    txt = open(os.path.join(ROOT, "include", "cc.h")).read()
-    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(cc_[a-z0-9_]+)\s*\(", txt)))
+    """Every function declared by include/*.h (cc.h: the tracking interface; cc_bench.h: measurement aids)."""
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for f in sorted(os.listdir(inc)):
+        if f.endswith(".h"):
+            txt = re.sub(r"/\*.*?\*/", "", open(os.path.join(inc, f)).read(), flags=re.S)
+            names |= set(re.findall(r"\b(cc_[a-z0-9_]+)\s*\(", txt))
+    return sorted(names)
 
 
 def test_header_symbols_exported(lib):
@@ -69,6 +74,7 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.cc_drift_correct(None, None, -1, 0.1, 0.0, None, None, None, None) == 1
     assert lib.cc_drift_correct(None, None, 4, 0.1, 0.0, None, None, None, None) == 1
     assert lib.cc_track_latency_probe(None, None, 1, None, None, None, None, None) == 1
+    assert lib.cc_plan_set_host_chunk(None, 4) == 1
 
 
 def test_no_device_is_a_loud_error(lib):

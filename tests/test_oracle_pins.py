@@ -584,3 +584,165 @@ def test_it2_iterations_sharpen_the_reference(oracle_mod):
     # the averaged RI sits at frame 0's position: compare its spectrum modulus with the clean template's
     noisy = np.abs(np.fft.fft2(fr[0].astype(np.float64)))
     assert np.sum((np.abs(G3) - np.abs(np.fft.fft2(clean))) ** 2) < 0.2 * np.sum((noisy - np.abs(np.fft.fft2(clean))) ** 2)
+
+
+def test_it3_fractional_alignment_through_the_iteration(oracle_mod):
+    """The IT analogue of RI2: frames that are phase-ramp shifts (on the 1/u grid, even H and W) of a band-limited
+    image are shifted back onto it by Eq. (8)'s alignment, so after one pass G equals fft2(ref) up to the +-0.5
+    rounding of the integer pixels.  Fractional phases and the Nyquist cos(pi d) branch are decisive here: a wrong
+    alignment sign doubles the shift instead of removing it (error ~ |G|, five orders above the bound)."""
+    rng = _rng(63)
+    H, W, u = 16, 24, 8
+    B0 = np.fft.fft2(rng.standard_normal((H, W)))
+    B0[H // 2, :] = 0
+    B0[:, W // 2] = 0
+    base = np.real(np.fft.ifft2(B0))
+    fy, fx = np.fft.fftfreq(H)[:, None], np.fft.fftfreq(W)[None, :]
+    ref = np.round(base * (2000.0 / np.abs(base).max())) + 3000.0
+    shifts = [(0.375, -0.25), (-1.5, 2.125), (0.0, 0.0), (2.625, 0.5), (-0.125, -3.75)]
+    fr = np.stack([np.round(np.real(np.fft.ifft2(np.fft.fft2(ref) * np.exp(-2j * np.pi * (fy * dy + fx * dx)))))
+                   for dy, dx in shifts]).astype(np.uint16)
+    res, G = oracle_mod.iterate_reference(fr, ref.astype(np.float32), u, 1)
+    assert np.allclose(res.dy, [s[0] for s in shifts]) and np.allclose(res.dx, [s[1] for s in shifts])
+    Gr = np.fft.fft2(ref)
+    err = np.max(np.abs(G - Gr))
+    assert err < 5 * np.sqrt(H * W / 12.0) and err < 1e-2 * np.median(np.abs(Gr))
+    # the mean of Eq. (8) is a plain mean: the result does not depend on the order of the frames
+    res_p, G_p = oracle_mod.iterate_reference(fr[::-1].copy(), ref.astype(np.float32), u, 1)
+    assert np.max(np.abs(G_p - G)) < 1e-9 * np.abs(G[0, 0]) and np.allclose(res_p.dy[::-1], res.dy)
+
+
+def test_st1_step_from_a_given_spectrum(oracle_mod):
+    """cco_step_from_spectrum (the entry the GPU open-loop tests drive): from G = fft2(ref) (library FFT) it returns
+    cco_track's displacement; with a0 = 1 the returned spectrum is that of the frame rolled back by its integer shift
+    (np.roll, no Fourier arithmetic); with a0 in between, the blend of Eq. (9); a0 = 0 leaves G untouched."""
+    rng = _rng(64)
+    H, W = 12, 16
+    ref = rng.integers(0, 300, size=(H, W)).astype(np.float32)
+    G0 = np.fft.fft2(ref.astype(np.float64))
+    for (a, b) in [(2, -3), (0, 0), (-5, 7)]:
+        frame = np.roll(ref, (a, b), axis=(0, 1)).astype(np.uint16)
+        t = oracle_mod.track(frame[None], ref, 4)
+        for a0 in (1.0, 0.25, 0.0):
+            r, Gn = oracle_mod.step_from_spectrum(frame, G0, 4, a0)
+            assert (r.dy[0], r.dx[0]) == (t.dy[0], t.dx[0]) == (float(a), float(b))
+            back = np.fft.fft2(np.roll(frame.astype(np.float64), (-a, -b), axis=(0, 1)))
+            assert np.max(np.abs(Gn - (a0 * back + (1 - a0) * G0))) < 1e-9 * np.abs(G0[0, 0])
+    # a noisy frame against a spectrum that is NOT that of an integer image: same result as the piecewise pipeline
+    frame = rng.poisson(ref.astype(np.float64) + 5).astype(np.uint16)
+    Gq = G0 * (1.0 + 0.01 * rng.standard_normal(G0.shape))
+    Gq = np.fft.fft2(np.real(np.fft.ifft2(Gq)))                          # spectrum of a real image
+    r, _ = oracle_mod.step_from_spectrum(frame, Gq, 4, 0.5)
+    t = _track_f(oracle_mod, frame.astype(np.float64), np.real(np.fft.ifft2(Gq)), 4)
+    assert (r.dy[0], r.dx[0]) == (t["dy"], t["dx"]) and abs(r.peak[0] - t["peak"]) <= 1e-9 * abs(t["peak"])
+
+
+# ---------------------------------------------------------------- CC-SN with a moving reference image (DESIGN.md R19)
+# SR1  a0 = 0 is cco_track_sn with the fixed reference
+# SR2  exact translations of the RI leave it unchanged; d = shift; S_min = sum(E + eps) (Cauchy-Schwarz, as SN1)
+# SR3  eps -> infinity reproduces the CC-U loop of Eq. (9) (PAPER.md:L161)
+# SR4  zero-displacement frames: the state is the low-pass filter of Eq. (9) written out (as RI3)
+# SR5  frame i is weighted by 1/(E_{i-1} + eps) with E_{i-1} the UPDATED image average: brute-force Eq. (7)
+# SR6  Eq. (8): after one pass the state is the plain mean of the rolled-back frames, and the second pass weights
+#      with 1/(that mean + eps): brute-force Eq. (7)
+def test_sr1_a0_zero_is_the_fixed_reference(oracle_mod):
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr, ref = wl.frames(cfg, np.arange(6)), wl.reference(cfg)
+    a = oracle_mod.track(fr, ref, 20, method="sn", epsilon=50.0)
+    b, G = oracle_mod.track_rt(fr, ref, 20, 0.0, method="sn", epsilon=50.0)
+    assert np.array_equal(a.dx, b.dx) and np.array_equal(a.dy, b.dy) and np.allclose(a.peak, b.peak, rtol=1e-10)
+    assert np.allclose(G, np.fft.fft2(ref.astype(np.float64)), rtol=1e-10, atol=1e-6)
+
+
+def test_sr2_aligned_copies_leave_the_reference_unchanged(oracle_mod):
+    rng = _rng(71)
+    H, W, eps = 16, 24, 12.5
+    ref = rng.integers(3, 200, size=(H, W)).astype(np.float32)
+    shifts = [(3, -5), (0, 7), (-6, 0), (8, 12), (1, 1)]
+    fr = np.stack([np.roll(ref, s, axis=(0, 1)) for s in shifts]).astype(np.uint16)
+    G0 = np.fft.fft2(ref.astype(np.float64))
+    for a0 in (0.3, 1.0):
+        res, G = oracle_mod.track_rt(fr, ref, 4, a0, method="sn", epsilon=eps)
+        assert np.max(np.abs(G - G0)) < 1e-9 * np.max(np.abs(G0))
+        for k, (a, b) in enumerate(shifts):
+            assert (res.dy[k], res.dx[k]) == (a - H if 2 * a >= H else a, b - W if 2 * b >= W else b)
+        assert np.allclose(res.peak, np.sum(ref.astype(np.float64) + eps), rtol=1e-10)
+    res, G = oracle_mod.iterate_reference(fr, ref, 4, 2, method="sn", epsilon=eps)
+    assert np.max(np.abs(G - G0)) < 1e-9 * np.max(np.abs(G0)) and np.allclose(res.peak, np.sum(ref.astype(np.float64) + eps), rtol=1e-10)
+
+
+def test_sr3_large_offset_reproduces_the_ccu_loop(oracle_mod):
+    """PAPER.md:L161 for the closed loop: with eps = 1e7 the weights are flat, the displacements are those of the CC-U
+    loop (at most one grid step away, mostly identical) and so is the running reference."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(1)
+    fr, ref = wl.frames(cfg, np.arange(16)), wl.reference(cfg)
+    ru, Gu = oracle_mod.track_rt(fr, ref, 20, 0.2)
+    rs, Gs = oracle_mod.track_rt(fr, ref, 20, 0.2, method="sn", epsilon=1e7)
+    d = np.hypot(rs.dx - ru.dx, rs.dy - ru.dy)
+    assert d.max() <= 0.05 * np.sqrt(2) + 1e-12 and np.mean(d == 0) >= 0.75
+    scale = np.max(np.abs(Gu[1:, 1:]))
+    assert np.max(np.abs(Gs - Gu)) < 2e-2 * scale
+    near, _ = oracle_mod.track_rt(fr, ref, 20, 0.2, method="sn", epsilon=1.0)
+    assert np.hypot(near.dx - ru.dx, near.dy - ru.dy).mean() > d.mean()       # a small offset is a different estimator
+
+
+def test_sr4_filter_weights_closed_form(oracle_mod):
+    rng = _rng(72)
+    H = W = 16
+    y, x = np.mgrid[0:H, 0:W]
+    ref = (500.0 * np.exp(-((y - 8) ** 2 + (x - 8) ** 2) / 8.0) + 20.0).astype(np.float32)
+    fr = np.clip(np.round(ref[None] + rng.normal(0, 1.0, size=(5, H, W))), 0, 65535).astype(np.uint16)
+    a0 = 0.25
+    res, G = oracle_mod.track_rt(fr, ref, 2, a0, method="sn", epsilon=30.0)
+    assert np.all(res.dx == 0) and np.all(res.dy == 0)
+    expect = (1 - a0) ** 5 * np.fft.fft2(ref.astype(np.float64))
+    for k in range(5):
+        expect = expect + a0 * (1 - a0) ** (4 - k) * np.fft.fft2(fr[k].astype(np.float64))
+    assert np.max(np.abs(G - expect)) < 1e-9 * np.max(np.abs(expect))
+
+
+def test_sr5_weight_follows_the_updated_reference(oracle_mod):
+    """Frame 0 sits on the RI (d_0 = 0), so E_0 = a0 I_0 + b1 E_{-1} pixel by pixel (no Fourier arithmetic); frame 1
+    must then be measured with the weight 1/(E_0 + eps): integer minimiser, minimum and runner-up of the literal
+    double loop of Eq. (7).  Fails for a stale weight 1/(E_{-1} + eps) and for the literal substitution of L92."""
+    rng = _rng(73)
+    H, W, eps, a0 = 10, 12, 6.0, 0.6
+    y, x = np.mgrid[0:H, 0:W]
+    ref = (150.0 * np.exp(-((y - 5) ** 2 + (x - 6) ** 2) / 5.0) + 8.0).astype(np.float32)
+    f0 = rng.poisson(ref.astype(np.float64)).astype(np.uint16)
+    f1 = rng.poisson(np.roll(ref.astype(np.float64), (2, -3), axis=(0, 1))).astype(np.uint16)
+    res, G = oracle_mod.track_rt(np.stack([f0, f1]), ref, 1, a0, method="sn", epsilon=eps)
+    assert (res.dy[0], res.dx[0]) == (0.0, 0.0)
+    E0 = a0 * f0.astype(np.float64) + (1 - a0) * ref.astype(np.float64)
+    S = _sn_direct(f1.astype(np.float64), E0, eps)
+    y0, x0 = divmod(int(np.argmin(S)), W)
+    assert (res.wy[1] % H, res.wx[1] % W) == (y0, x0) == (2, W - 3)
+    assert abs(res.peak[1] / S.min() - 1) < 1e-11 and abs(res.cc_top2[1] / np.partition(S.ravel(), 1)[1] - 1) < 1e-11
+    stale = _sn_direct(f1.astype(np.float64), ref.astype(np.float64), eps)
+    assert abs(res.peak[1] / stale.min() - 1) > 1e-4                          # the pin can tell the two apart
+    # one step from a given state gives the same answer (cco_step_from_spectrum_sn)
+    r1, _ = oracle_mod.step_from_spectrum(f1, np.fft.fft2(E0), 1, a0, method="sn", epsilon=eps)
+    assert (r1.dy[0], r1.dx[0]) == (res.dy[1], res.dx[1]) and abs(r1.peak[0] / res.peak[1] - 1) < 1e-11
+    with pytest.raises(ValueError):                                           # E + eps must stay positive
+        oracle_mod.step_from_spectrum(f1, np.fft.fft2(E0 - 200.0), 1, a0, method="sn", epsilon=eps)
+
+
+def test_sr6_offline_passes(oracle_mod):
+    rng = _rng(74)
+    H, W, N, eps = 12, 12, 10, 9.0
+    y, x = np.mgrid[0:H, 0:W]
+    base = 400.0 * np.exp(-((y - 6) ** 2 + (x - 6) ** 2) / 6.0) + 30.0
+    shifts = rng.integers(-3, 4, size=(N, 2))
+    shifts[0] = 0
+    fr = np.stack([np.roll(rng.poisson(base), tuple(s), axis=(0, 1)) for s in shifts]).astype(np.uint16)
+    res, G = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 1, 1, method="sn", epsilon=eps)
+    assert np.array_equal(res.wy, shifts[:, 0]) and np.array_equal(res.wx, shifts[:, 1])
+    mean = np.mean([np.roll(f.astype(np.float64), tuple(-s), axis=(0, 1)) for f, s in zip(fr, shifts)], axis=0)
+    assert np.max(np.abs(G - np.fft.fft2(mean))) < 1e-9 * np.abs(G[0, 0])
+    res2, G2 = oracle_mod.iterate_reference(fr, fr[0].astype(np.float32), 1, 2, method="sn", epsilon=eps)
+    for k in range(N):
+        S = _sn_direct(fr[k].astype(np.float64), mean, eps)
+        assert abs(res2.peak[k] / S.min() - 1) < 1e-11
+    assert np.max(np.abs(G2 - G)) < 1e-9 * np.abs(G[0, 0])

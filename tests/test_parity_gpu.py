@@ -62,15 +62,14 @@ def _compare(o, dx, dy, pk, iy, ix, label, near_tie=0.0, u=None):
     assert rel <= TOL_PEAK, "%s: peak relative error %.2e" % (label, rel)
 
 
-# (config, number of parity-subset frames the oracle is run on)
-SUBSETS = [(1, 1000), (2, 1000), (3, 400), (4, 64), (5, 24)]
-
-
-@pytest.mark.parametrize("ci,n", SUBSETS)
-def test_config_parity_subset(gpu, oracle_mod, ci, n):
+@pytest.mark.parametrize("ci", [1, 2, 3, 4, 5])
+def test_config_parity_subset(gpu, oracle_mod, ci):
+    """The parity subsets of SURVEY.md 8(c) as workloads.CONFIGS encodes them: cfg 1 all 1000 frames, cfg 2 every
+    10th of 10,000 (1000), cfg 3 every 10th (1000), cfg 4 every 10th (200), cfg 5 every 8th, first 64."""
     from paper_2310_08770_b200 import workloads as wl
     cfg = wl.config(ci)
-    idx = wl.oracle_subset(cfg)[:n]
+    idx = wl.oracle_subset(cfg)
+    assert len(idx) == cfg.oracle_count
     fr = wl.frames(cfg, idx)
     ref = wl.reference(cfg)
     o = oracle_mod.track(fr, ref, cfg.upsample)
@@ -402,7 +401,7 @@ def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
     _compare(o, dx, dy, pk, iy, ix, "%dx%d u=%d CC-SN" % (H, W, u))
 
 
-@pytest.mark.parametrize("ci,n", [(3, 24), (4, 12), (5, 4)])
+@pytest.mark.parametrize("ci,n", [(3, 24), (4, 12), (5, 16)])
 def test_single_frame_variants_match_oracle(gpu, oracle_mod, ci, n):
     """Sequential batch-1 calls select the small-batch cluster variants (16 CTAs at 256x256, 512x512 and 1024x1024);
     they return the oracle's grid points and the same displacements as the batched variant."""
@@ -463,6 +462,37 @@ def _half(G):
     return G[:, : G.shape[1] // 2 + 1]
 
 
+def _full(Gh, W):
+    """(H, W/2 + 1) half-spectrum of a real image -> full (H, W) spectrum, G[ky][W - kx] = conj(G[-ky][kx])."""
+    H = Gh.shape[0]
+    G = np.empty((H, W), np.complex128)
+    G[:, : W // 2 + 1] = Gh
+    neg = (-np.arange(H)) % H
+    G[:, W // 2 + 1:] = np.conj(Gh[neg][:, W // 2 - 1:0:-1])
+    return G
+
+
+# Closed loop (the result of frame i feeds the reference of frame i+1; device state fp32, oracle state float64): the
+# two references differ in the 7th digit, so a frame whose two best grid points the ORACLE itself separates by less
+# than CLOSED_LOOP_MARGIN (relative) may resolve to the neighbouring point.  Every differing frame must be such a
+# near-tie, one grid step away; their number is printed and bounded by what was measured (DESIGN.md section 3).
+CLOSED_LOOP_MARGIN = 2e-5
+CLOSED_LOOP_MIN_SAME = 0.98
+
+
+def _closed_loop_compare(o, dx, dy, u, label):
+    step = np.maximum(np.abs(dx - o.dx), np.abs(dy - o.dy))
+    diff = np.nonzero(step > TOL_PX)[0]
+    marg = np.abs(o.up_top1 - o.up_top2) / np.maximum(np.abs(o.up_top1), 1e-300)
+    print("%s: %d of %d frames on the neighbouring grid point; oracle top-1/top-2 margins there: %s"
+          % (label, len(diff), len(dx), np.array2string(marg[diff], precision=2)))
+    for i in diff:
+        assert step[i] <= 1.0 / u + 1e-5, "%s frame %d: %.4f px from the oracle (more than one grid step)" % (label, i, step[i])
+        assert marg[i] < CLOSED_LOOP_MARGIN, "%s frame %d differs but is no near-tie: oracle margin %.2e" % (label, i, marg[i])
+    assert len(diff) <= (1.0 - CLOSED_LOOP_MIN_SAME) * len(dx), "%s: %d of %d frames differ" % (label, len(diff), len(dx))
+    return len(diff)
+
+
 def test_reference_spectrum_accessor_and_aligned_copies(gpu, oracle_mod):
     """cc_plan_get_reference_spectrum returns F[E]; frames that are exact circular shifts of the RI are shifted
     back onto it by Eq. (9), so the running reference does not move (pin RI2 of the oracle, here on the device)."""
@@ -504,9 +534,10 @@ class _Fmt:
                                      (_Fmt(128, 1024, 32), 24, 0.05)], ids=["cfg2", "cfg1", "cfg3", "256x128", "128x1024"])
 def test_running_reference_matches_oracle(gpu, oracle_mod, ci, n, a0):
     """Closed loop of Eq. (9): the device rewrites its fp32 reference spectrum after every frame, the oracle its
-    float64 one.  Integer peaks must agree on every frame; the sub-pixel grid point on nearly all of them and never
-    differ by more than one grid step (a rounding-level near-tie may resolve differently once the two references
-    differ in the 7th digit); the spectra must still agree to 1e-4 of their scale after n frames."""
+    float64 one.  Integer peaks must agree on every frame; the sub-pixel grid point too, except on frames that the
+    oracle's own top-1/top-2 margin proves to be near-ties (_closed_loop_compare); the spectra must still agree to
+    1e-5 of their scale after n frames.  The step itself is checked open loop, at the full bar, in
+    test_reference_update_step_open_loop."""
     import torch
     from paper_2310_08770_b200 import workloads as wl
     if isinstance(ci, _Fmt):                                       # non-square formats: the cluster (latency) variants
@@ -528,12 +559,11 @@ def test_running_reference_matches_oracle(gpu, oracle_mod, ci, n, a0):
     iy, ix = np.concatenate([iy1, iy2]), np.concatenate([ix1, ix2])
     Gd = plan.reference_spectrum()
     assert np.array_equal(iy, o.wy) and np.array_equal(ix, o.wx)
-    step = np.maximum(np.abs(dx - o.dx), np.abs(dy - o.dy))
-    assert step.max() <= 1.0 / u + 1e-5, step.max()
-    assert np.mean(step < TOL_PX) >= 0.97, np.mean(step < TOL_PX)
+    ndiff = _closed_loop_compare(o, dx, dy, u, "Eq. (9) closed loop %s" % getattr(cfg, "name", "%dx%d" % (cfg.H, cfg.W)))
     assert np.max(np.abs(pk / o.peak - 1)) < 1e-4
     scale = np.max(np.abs(G[1:, 1:]))
-    assert np.max(np.abs(Gd - _half(G))[:, 1:]) < 1e-4 * scale + 3e-2 * scale * a0 * np.sum(step > TOL_PX) / u
+    # a frame aligned one grid step off changes its summand by at most 2 pi (1/2) (1/u) = 3/u of its bins, weight a0
+    assert np.max(np.abs(Gd - _half(G))[:, 1:]) < 1e-5 * scale + 3e-2 * scale * a0 * ndiff / u
     # switching the update off freezes the reference
     plan.enable_reference_update(0.0)
     fx, fy, _ = [t.cpu().numpy() for t in plan.track(d[:4])]
@@ -577,8 +607,9 @@ def test_cluster_variants_with_fewer_offsets_than_ctas(gpu, oracle_mod, H, W, u)
 def test_offline_iterative_reference_matches_oracle(gpu, oracle_mod, ci, n, u, passes):
     """Offline analysis, Eq. (8), starting from E_0 = I_0: every pass tracks all frames in parallel
     (cc_track_accumulate, two chunks) and replaces the reference by the mean of the aligned frames.  Same closed-loop
-    criterion as the running reference: integer peaks exact, sub-pixel never more than a grid step away and identical on
-    >= 97 %, reference spectra equal to 1e-4 of their scale; the device result is deterministic."""
+    criterion as the running reference (_closed_loop_compare: every differing frame a proven near-tie), reference
+    spectra equal to 1e-5 of their scale; the device result is deterministic.  Each pass is checked open loop, at the
+    full bar, in test_offline_pass_open_loop."""
     import torch
     from paper_2310_08770_b200 import workloads as wl
     cfg = wl.config(ci)
@@ -602,12 +633,10 @@ def test_offline_iterative_reference_matches_oracle(gpu, oracle_mod, ci, n, u, p
         plan.close()
         outs.append((dx, dy, Gd))
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][2], outs[1][2])     # deterministic
-    step = np.maximum(np.abs(dx - o.dx), np.abs(dy - o.dy))
-    assert step.max() <= 1.0 / u + 1e-5, step.max()
-    assert np.mean(step < TOL_PX) >= 0.97, np.mean(step < TOL_PX)
+    ndiff = _closed_loop_compare(o, dx, dy, u, "Eq. (8) closed loop %s" % cfg.name)
     assert np.max(np.abs(pk / o.peak - 1)) < 1e-4
     scale = np.max(np.abs(G[1:, 1:]))
-    assert np.max(np.abs(Gd - _half(G))[:, 1:]) < 1e-4 * scale + 3e-2 * scale * np.sum(step > TOL_PX) / (u * n)
+    assert np.max(np.abs(Gd - _half(G))[:, 1:]) < 1e-5 * scale + 3e-2 * scale * ndiff / (u * n)
     assert abs(Gd[0, 0] / G[0, 0] - 1) < 1e-6
 
 
@@ -652,3 +681,102 @@ def test_concurrent_streams_on_one_plan(gpu):
     for k in range(3):
         assert torch.equal(torch.cat([a[k], b[k]]), ref_out[k])
     plan.close()
+
+
+# ---------------------------------------------------------------- open-loop steps of Eq. (9) / Eq. (8), full north_star bar
+@pytest.mark.parametrize("ci,n,a0", [(2, 60, 0.05), (1, 60, 0.1), (3, 16, 0.05)], ids=["cfg2", "cfg1", "cfg3"])
+def test_reference_update_step_open_loop(gpu, oracle_mod, ci, n, a0):
+    """ONE step of Eq. (9) at a time, device and oracle from the SAME state: before frame i the device's reference
+    spectrum is read (cc_plan_get_reference_spectrum) and handed to the oracle (cco_step_from_spectrum: input only);
+    d_i must be the oracle's grid point (2e-3 px, exact integer peak, peak to 1e-4) and the device's spectrum after the
+    step must equal a0 F[I_i aligned] + b1 G to 1e-6 of its scale."""
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    fr = wl.frames(cfg, np.arange(n))
+    u = cfg.upsample
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, u, wl.reference(cfg))
+    plan.enable_reference_update(a0)
+    d = plan.device_frames(fr)
+    worst = 0.0
+    for i in range(n):
+        G_before = _full(plan.reference_spectrum().astype(np.complex128), cfg.W)
+        dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(d[i], 1, debug=True)]
+        G_after = plan.reference_spectrum().astype(np.complex128)
+        o, Gn = oracle_mod.step_from_spectrum(fr[i], G_before, u, a0)
+        _compare(o, dx, dy, pk, iy, ix, "%s Eq. (9) step %d" % (cfg.name, i))
+        scale = np.max(np.abs(Gn[1:, 1:]))
+        err = np.max(np.abs(G_after - _half(Gn))[:, 1:]) / scale
+        worst = max(worst, err)
+        assert err < 1e-6, "frame %d: spectrum after the step off by %.2e of its scale" % (i, err)
+        assert abs(G_after[0, 0] / Gn[0, 0] - 1) < 1e-6
+    print("%s: Eq. (9) open-loop steps, worst spectrum error %.2e of scale" % (cfg.name, worst))
+    plan.close()
+
+
+@pytest.mark.parametrize("ci,n,u", [(1, 96, 20), (3, 24, 100)], ids=["cfg1", "cfg3"])
+def test_offline_pass_open_loop(gpu, oracle_mod, ci, n, u):
+    """ONE pass of Eq. (8) at a time from the SAME reference: every frame's displacement against the device's current
+    spectrum at the full bar, and the device's new reference equal to the plain mean of the oracle's aligned spectra
+    (cco_step_from_spectrum with a0 = 1) to 1e-6 of its scale.  Two passes, starting from E_0 = I_0."""
+    import torch
+    from paper_2310_08770_b200 import workloads as wl
+    cfg = wl.config(ci)
+    fr = wl.frames(cfg, np.arange(n))
+    plan = gpu.Plan(cfg.H, cfg.W, fr.dtype, u, fr[0].astype(np.float32))
+    d = plan.device_frames(fr)
+    for it in range(2):
+        G_before = _full(plan.reference_spectrum().astype(np.complex128), cfg.W)
+        k = n // 3
+        a = plan.track_accumulate(d[:k])
+        b = plan.track_accumulate(d[k:])
+        plan.update_reference_from_accumulator()
+        dx, dy, pk = [torch.cat([a[j], b[j]]).cpu().numpy() for j in range(3)]
+        G_after = plan.reference_spectrum().astype(np.complex128)
+        mean = np.zeros((cfg.H, cfg.W), np.complex128)
+        for i in range(n):
+            o, A = oracle_mod.step_from_spectrum(fr[i], G_before, u, 1.0)
+            assert abs(dx[i] - o.dx[0]) <= TOL_PX and abs(dy[i] - o.dy[0]) <= TOL_PX, (
+                "pass %d frame %d: gpu (%.4f, %.4f) oracle (%.4f, %.4f), oracle margin %.2e"
+                % (it, i, dy[i], dx[i], o.dy[0], o.dx[0], (o.up_top1[0] - o.up_top2[0]) / abs(o.up_top1[0])))
+            assert abs(pk[i] / o.peak[0] - 1) <= TOL_PEAK
+            mean += A / n
+        scale = np.max(np.abs(mean[1:, 1:]))
+        err = np.max(np.abs(G_after - _half(mean))[:, 1:]) / scale
+        print("%s pass %d: new reference off by %.2e of its scale" % (cfg.name, it, err))
+        assert err < 1e-6 and abs(G_after[0, 0] / mean[0, 0] - 1) < 1e-6
+    plan.close()
+
+
+# ---------------------------------------------------------------- cc_track_host with several chunks on two streams
+@pytest.mark.parametrize("H,W,dt,n,chunk,mode", [(64, 64, np.uint16, 500, 64, "plain"), (1024, 1024, np.uint16, 40, 12, "plain"),
+                                                 (1024, 1024, np.uint8, 9, 2, "plain"), (64, 64, np.uint16, 200, 32, "ri")],
+                         ids=["64x64-8chunks", "1024x1024-u16-4chunks-thr", "1024x1024-u8-5chunks", "64x64-ri-7chunks"])
+def test_host_path_multi_chunk(gpu, H, W, dt, n, chunk, mode):
+    """cc_track_host splits the batch into chunks that alternate between two streams (copy of one chunk under the
+    kernel of the other); shapes whose spectrum block lives in global scratch (1024 x 1024) run two kernels at once,
+    each on its own scratch.  With the Eq. (9) update the chunks stay in order on one stream.  Result == cc_track."""
+    import torch
+    rng = np.random.default_rng(H + n)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+    spot = lambda sy, sx: 180.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 3.0 ** 2)) + 8.0
+    ref = spot(0.0, 0.0).astype(np.float32)
+    sh = rng.uniform(-6, 6, size=(n, 2))
+    fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 255).astype(dt)
+    res = []
+    for host in (False, True):
+        plan = gpu.Plan(H, W, fr.dtype, 20, ref)
+        if mode == "ri":
+            plan.enable_reference_update(0.05)
+        if host:
+            plan.set_host_chunk(chunk)
+            out = plan.track_host(fr)
+            out2 = plan.track_host(fr) if mode != "ri" else out          # staging buffers and scratch are reused
+            assert all(np.array_equal(a, b) for a, b in zip(out, out2))
+        else:
+            out = [t.cpu().numpy() for t in plan.track(plan.device_frames(fr))]
+        torch.cuda.synchronize()
+        res.append(out)
+        plan.close()
+    for a, b in zip(res[0], res[1]):
+        assert np.array_equal(a, b)
+    assert np.median(np.hypot(res[1][0] - sh[:, 1], res[1][1] - sh[:, 0])) < 0.2
