@@ -198,18 +198,27 @@ cc_status cc_rt_close(cc_rt *rt);
  * cc_plan_enable_reference_update -- the paper's real-time analysis (Eq. (9)): after every
  * frame the plan's reference image is replaced by  F[E_i] = a0 F[I_i aligned] + (1 - a0) F[E_{i-1}],  the aligned
  * image being the frame translated by its detected displacement (Fourier shift theorem; cos(pi d) on the Nyquist
- * bins -- DESIGN.md R18).  a0 = 1 - exp(-T/tau) in (0, 1]; a0 == 0 switches the update off again.  CC-U plans only
- * (CC_ERR_UNSUPPORTED otherwise).  Frames are then processed strictly in order by ONE cluster (the largest-cluster
- * variant of the shape): frame i of a cc_track batch is measured against the reference left by frame i-1, and
- * consecutive cc_track / cc_rt_track calls continue the sequence.  cc_track thereby MODIFIES the plan: calls on
- * one plan must be serialised (same stream).  May synchronise the device.
+ * bins -- DESIGN.md R18).  a0 = 1 - exp(-T/tau) in (0, 1]; a0 == 0 switches the update off again.
+ * Frames are then processed strictly in order: frame i of a cc_track batch is measured against the reference left
+ * by frame i-1, and consecutive cc_track / cc_rt_track calls continue the sequence.  cc_track thereby MODIFIES the
+ * plan: calls on one plan must be serialised (same stream).  May synchronise the device.
+ *   CC-U plans   the update runs inside the fused kernel (one cluster, the largest-cluster variant of the shape).
+ *   CC-SN plans  (R19) the state is F[E] of the average RAW image, kept in float64; after
+ *                every frame separate kernels apply Eq. (9) to it and rebuild the weight spectrum F[-1/(E + eps)]
+ *                that the fused kernel correlates with (one launch of the fused kernel per frame).  cc_rt_* cannot
+ *                serve such a plan (CC_ERR_UNSUPPORTED).  If E + eps ever becomes <= 0 in some pixel, the next
+ *                cc_plan_get_reference_spectrum call reports CC_ERR_INVALID_ARG.
  *
- * cc_plan_get_reference_spectrum -- debugging / checkpoint aid: the spectrum F[E] the plan currently holds.
+ * cc_plan_get_reference_spectrum -- debugging / checkpoint aid: the spectrum F[E] of the plan's current reference
+ * image (for CC-SN plans: of E itself, not of the weight 1/(E + eps)).
  *   out   HOST pointer, H * (W/2 + 1) complex float32 (re, im interleaved), row ky, column kx = 0..W/2,
  *         natural frequency order, unnormalised (sum over pixels).  Synchronises the device.
+ * cc_plan_get_reference_spectrum_f64 -- the same as complex float64 (CC-SN plans hold their state in float64;
+ * CC-U plans return their float32 state widened).
  */
 cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0);
 cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *out);
+cc_status cc_plan_get_reference_spectrum_f64(const cc_plan *plan, double *out);
 
 /*
  * Offline analysis -- PAPER.md:L94-100, Eq. (8): the reference image of pass n is the mean of all images of the
@@ -217,8 +226,9 @@ cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *out);
  *     F[E_n] = (1/N) sum_i F[I_i aligned]        (alignment as in cc_plan_enable_reference_update).
  * cc_track_accumulate   cc_track over a batch (all clusters in parallel: "embarrassingly parallel", L100) that also
  *                       adds every frame's aligned spectrum to plan-owned per-cluster accumulators.  May be called
- *                       several times per pass (chunks of a data set).  CC-U plans without the Eq. (9) update.
- *                       Allocates on first use; arguments as cc_track.
+ *                       several times per pass (chunks of a data set).  Plans without the Eq. (9) update.  CC-SN
+ *                       plans (R19) sum the aligned RAW spectra in float64 with separate kernels after
+ *                       the tracking launch.  Allocates on first use; arguments as cc_track.
  * cc_plan_update_reference_from_accumulator
  *                       ends a pass: reduces the accumulators in a fixed order (deterministic), replaces the plan's
  *                       reference by the mean over all frames accumulated since the last call and clears them.

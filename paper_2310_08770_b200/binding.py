@@ -21,7 +21,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
 
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host",
            "cc_plan_set_host_chunk", "cc_plan_destroy",
-           "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_track_accumulate",
+           "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_plan_get_reference_spectrum_f64", "cc_track_accumulate",
            "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
@@ -86,6 +86,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_plan_enable_reference_update.restype = ci
         lib.cc_plan_get_reference_spectrum.argtypes = [vp, vp]
         lib.cc_plan_get_reference_spectrum.restype = ci
+        lib.cc_plan_get_reference_spectrum_f64.argtypes = [vp, vp]
+        lib.cc_plan_get_reference_spectrum_f64.restype = ci
         lib.cc_track_accumulate.argtypes = [vp, vp, ci, vp, vp, vp, vp]
         lib.cc_track_accumulate.restype = ci
         lib.cc_plan_update_reference_from_accumulator.argtypes = [vp, vp]
@@ -154,10 +156,12 @@ class Plan:
         """cc_plan_enable_reference_update: running reference image of PAPER.md Eq. (9); a0 = 0 switches it off."""
         _check(load_library().cc_plan_enable_reference_update(self._h, float(a0)))
 
-    def reference_spectrum(self) -> np.ndarray:
-        """cc_plan_get_reference_spectrum: complex64 (H, W/2 + 1), the spectrum F[E] the plan currently holds."""
-        out = np.empty((self.H, self.W // 2 + 1), np.complex64)
-        _check(load_library().cc_plan_get_reference_spectrum(self._h, out.ctypes.data_as(ctypes.c_void_p)))
+    def reference_spectrum(self, f64: bool = False) -> np.ndarray:
+        """cc_plan_get_reference_spectrum[_f64]: complex64 / complex128 (H, W/2 + 1), the spectrum F[E] of the plan's
+        current reference image."""
+        out = np.empty((self.H, self.W // 2 + 1), np.complex128 if f64 else np.complex64)
+        fn = load_library().cc_plan_get_reference_spectrum_f64 if f64 else load_library().cc_plan_get_reference_spectrum
+        _check(fn(self._h, out.ctypes.data_as(ctypes.c_void_p)))
         return out
 
     def track_accumulate(self, frames_dev, batch: int | None = None):

@@ -59,8 +59,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [NVCC] + FLAGS + ["-c", os.path.join(CSRC, "cc_variant.cu"), "-o", obj] + \
               ["-DCCV_%s=%s" % (k, v[k]) for k in _KEYS]
         jobs.append((cmd, obj))
-    api = os.path.join(OBJ, "cc_api.o")
-    jobs.append(([NVCC] + FLAGS + ["-c", os.path.join(CSRC, "cc_api.cu"), "-o", api], api))
+    for src in ("cc_api", "cc_refupdate"):
+        o = os.path.join(OBJ, src + ".o")
+        jobs.append(([NVCC] + FLAGS + ["-c", os.path.join(CSRC, src + ".cu"), "-o", o], o))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         outs = list(ex.map(lambda j: _run(j[0], j[1] + ".log"), jobs))
     if verbose:

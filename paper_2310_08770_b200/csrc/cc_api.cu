@@ -18,6 +18,7 @@
 #include "../../include/cc.h"
 #include "../../include/cc_bench.h"
 #include "cc_common.h"
+#include "cc_refupdate.h"
 
 // ------------------------------------------------------------------ variants
 #define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1) CcVariant cc_variant_##name();
@@ -91,6 +92,9 @@ struct cc_plan {
     double *acc_mean = nullptr;
     int acc_clusters = 0;
     long long acc_count = 0;      // frames accumulated since the last reference update
+    // CC-SN with a moving reference image (R19): fp64 state G = F[E], created on first use from the caller's image
+    CcSnState *sn_state = nullptr;
+    std::vector<float> sn_ref;    // the caller's reference image (CC-SN plans only)
     size_t table_bytes = 0;
     VarPlan thr, lat;  // throughput variant, small-batch (latency) variant
     bool has_lat = false;
@@ -337,6 +341,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
     cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab), cudaFree(plan->ri_emean), cudaFree(plan->col_freq);
     cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
+    cc_sn_state_destroy(plan->sn_state);
     for (VarPlan *vp : {&plan->thr, &plan->lat})
         cudaFree(vp->Sg), cudaFree(vp->Sg_alt), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc);
     for (int i = 0; i < 2; ++i) {
@@ -420,6 +425,7 @@ extern "C" cc_status cc_plan_create_weighted(cc_plan **out, int H, int W, cc_dty
             m2 += ep * ep;
         }
         pl->sn = 1, pl->sn_eps = (double)epsilon, pl->sn_c0 = nearbyint(m2 / (double)G.size());
+        pl->sn_ref = ref;
     } else {
         for (size_t i = 0; i < G.size(); ++i) G[i] = std::complex<double>((double)ref[i], 0.0);
     }
@@ -533,7 +539,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;
     p.c0 = pl->c0, p.u_bytes = vp.u_bytes, p.Emean = pl->Emean;
     p.ri_emean = pl->ri_emean;  // null while the reference mean is the host constant Emean
-    if (pl->ri_a0 > 0.0) {
+    if (pl->ri_a0 > 0.0 && !pl->sn) {  // CC-U: Eq. (9) inside the fused kernel; CC-SN: separate fp64 kernels (cc_refupdate.cu)
         p.ri_Fs = pl->ri_Fs, p.ri_Fab = pl->ri_Fab, p.col_freq = pl->col_freq, p.ri_a0 = pl->ri_a0;
     }
     p.sn = pl->sn, p.sn_eps = pl->sn_eps, p.sn_c0 = pl->sn_c0, p.peak_sign = pl->sn ? -1.0 : 1.0;
@@ -554,6 +560,22 @@ static cc_status track_impl(const cc_plan *plan, const void *frames, int batch, 
     fill_params(plan, *vp, p);
     p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak, p.iy = iy, p.ix = ix, p.phase_clk = phase_clk;
     if (sg_slot == 1 && vp->Sg_alt) p.Sg = vp->Sg_alt;  // cc_track_host's second stream: its own spectrum scratch
+    if (ri && plan->sn) {
+        // CC-SN with the running reference image (R19): one frame per launch against the current weight
+        // spectrum, then the fp64 update kernels rewrite it from the new state (Eq. (9) on the raw images)
+        const size_t fbytes = (size_t)plan->H * plan->W * (plan->dtype == CC_U8 ? 1 : 2);
+        const CcSnTables t{plan->Gt, plan->ab, plan->ri_emean, plan->col_freq};
+        for (int i = 0; i < batch; ++i) {
+            const void *fi = (const unsigned char *)frames + (size_t)i * fbytes;
+            p.frames = fi, p.batch = 1, p.dx = dx + i, p.dy = dy + i, p.peak = peak ? peak + i : nullptr;
+            p.iy = iy ? iy + i : nullptr, p.ix = ix ? ix + i : nullptr;
+            p.phase_clk = phase_clk ? phase_clk + (size_t)i * CC_NPHASE : nullptr;
+            cudaError_t e = vp->v.launch(p, 1, vp->smem_bytes, (cudaStream_t)stream);
+            if (e == cudaSuccess) e = cc_sn_update_eq9(plan->sn_state, fi, dy + i, dx + i, plan->ri_a0, t, (cudaStream_t)stream);
+            if (e != cudaSuccess) return fail_cuda(e, "CC-SN frame + reference update");
+        }
+        return CC_OK;
+    }
     const int ncl = ri ? 1 : std::min(batch, vp->max_clusters);
     cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
@@ -697,6 +719,9 @@ static double mono_us()
 
 static cc_status rt_launch(cc_rt *rt)
 {
+    if (rt->plan->sn && rt->plan->ri_a0 > 0.0)
+        return fail(CC_ERR_UNSUPPORTED, "a real-time session cannot serve a CC-SN plan with the Eq. (9) update: its reference is "
+                                        "rewritten by separate kernels between frames (use cc_track)");
     // a fresh kernel starts counting at sequence 0: rebase the mailbox
     CK(cudaStreamSynchronize(rt->stream));
     rt->seq = 0;
@@ -880,18 +905,63 @@ static cc_status ensure_spectrum_scratch(cc_plan *plan, int clusters)
     return CC_OK;
 }
 
+// CC-SN plans: the fp64 state G = F[E] (created from the caller's reference image on first use)
+static cc_status ensure_sn_state(cc_plan *plan)
+{
+    cc_status st = ensure_spectrum_scratch(plan, 0);
+    if (st != CC_OK || plan->sn_state) return st;
+    cudaError_t e = cc_sn_state_create(&plan->sn_state, plan->H, plan->W, plan->u, plan->dtype, plan->sn_eps, plan->sn_ref.data());
+    if (e != cudaSuccess)
+        return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "CC-SN reference state");
+    return CC_OK;
+}
+
 extern "C" cc_status cc_plan_enable_reference_update(cc_plan *plan, double a0)
 {
     if (!plan || !(a0 >= 0.0 && a0 <= 1.0)) return fail(CC_ERR_INVALID_ARG, "cc_plan_enable_reference_update: bad plan or a0");
-    if (plan->sn) return fail(CC_ERR_UNSUPPORTED, "the reference update of Eq. (9) is built for CC-U plans only");
     CK(cudaDeviceSynchronize());
     if (a0 == 0.0) {
         plan->ri_a0 = 0.0;
         return CC_OK;
     }
-    cc_status st = ensure_spectrum_scratch(plan, 1);
+    cc_status st = plan->sn ? ensure_sn_state(plan) : ensure_spectrum_scratch(plan, 1);
     if (st != CC_OK) return st;
     plan->ri_a0 = a0;
+    return CC_OK;
+}
+
+// the state of a CC-SN plan as a half spectrum (H x (W/2+1) complex128); creates the state on first use
+static cc_status sn_half_spectrum(cc_plan *plan, std::vector<double> &half)
+{
+    cc_status st = ensure_sn_state(plan);
+    if (st != CC_OK) return st;
+    const int H = plan->H, W = plan->W, Wh = W / 2;
+    std::vector<double> full((size_t)H * W * 2);
+    int flag = 0;
+    CK(cc_sn_read_state(plan->sn_state, full.data(), &flag));
+    if (flag) return fail(CC_ERR_INVALID_ARG, "CC-SN: reference + epsilon became non-positive in some pixel during the updates");
+    half.resize((size_t)H * (Wh + 1) * 2);
+    for (int ky = 0; ky < H; ++ky)
+        memcpy(&half[(size_t)ky * (Wh + 1) * 2], &full[(size_t)ky * W * 2], (size_t)(Wh + 1) * 2 * sizeof(double));
+    return CC_OK;
+}
+
+extern "C" cc_status cc_plan_get_reference_spectrum_f64(const cc_plan *plan, double *out)
+{
+    if (!plan || !out) return fail(CC_ERR_INVALID_ARG, "cc_plan_get_reference_spectrum_f64: null pointer");
+    const int H = plan->H, Wh = plan->W / 2;
+    const size_t n = (size_t)H * (Wh + 1);
+    if (plan->sn) {
+        std::vector<double> half;
+        cc_status st = sn_half_spectrum(const_cast<cc_plan *>(plan), half);
+        if (st != CC_OK) return st;
+        memcpy(out, half.data(), n * 2 * sizeof(double));
+        return CC_OK;
+    }
+    std::vector<float> f(n * 2);
+    cc_status st = cc_plan_get_reference_spectrum(plan, f.data());
+    if (st != CC_OK) return st;
+    for (size_t i = 0; i < n * 2; ++i) out[i] = (double)f[i];
     return CC_OK;
 }
 
@@ -899,6 +969,13 @@ extern "C" cc_status cc_plan_get_reference_spectrum(const cc_plan *plan, float *
 {
     if (!plan || !out) return fail(CC_ERR_INVALID_ARG, "cc_plan_get_reference_spectrum: null pointer");
     const int H = plan->H, W = plan->W, Wh = W / 2;
+    if (plan->sn) {  // CC-SN: the plan's tables hold the weight spectrum; F[E] is the fp64 state
+        std::vector<double> half;
+        cc_status st = sn_half_spectrum(const_cast<cc_plan *>(plan), half);
+        if (st != CC_OK) return st;
+        for (size_t i = 0; i < half.size(); ++i) out[i] = (float)half[i];
+        return CC_OK;
+    }
     CK(cudaDeviceSynchronize());
     std::vector<float2> Gt((size_t)H * Wh);
     std::vector<float4> ab(H);
@@ -927,11 +1004,22 @@ extern "C" cc_status cc_track_accumulate(cc_plan *plan, const void *frames, int 
                                          void *stream)
 {
     if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: bad plan or batch");
-    if (plan->sn) return fail(CC_ERR_UNSUPPORTED, "the offline iteration of Eq. (8) is built for CC-U plans only");
     if (plan->ri_a0 > 0.0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: switch the Eq. (9) update off first");
     if (batch == 0) return CC_OK;
     if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: null pointer");
     if (((uintptr_t)frames & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_track_accumulate: frames must be 16-byte aligned");
+    if (plan->sn) {
+        // CC-SN (R19): plain tracking of the batch against the current weight, then the aligned RAW spectra
+        // are summed in fp64 (frame order: deterministic)
+        cc_status st = ensure_sn_state(plan);  // first use: may synchronise
+        if (st == CC_OK) st = track_impl(plan, frames, batch, dx, dy, peak, nullptr, nullptr, nullptr, stream);
+        if (st != CC_OK) return st;
+        cudaError_t e = cc_sn_accumulate(plan->sn_state, frames, batch, dy, dx, (cudaStream_t)stream);
+        if (e != cudaSuccess)
+            return e == cudaErrorMemoryAllocation ? fail(CC_ERR_NOMEM, "device allocation failed") : fail_cuda(e, "CC-SN accumulation");
+        plan->acc_count += batch;
+        return CC_OK;
+    }
     const VarPlan *vp = &plan->thr;
     const int H = plan->H, W = plan->W, ncmax = vp->max_clusters;
     if (plan->acc_clusters < ncmax) {  // first use: may synchronise
@@ -997,6 +1085,13 @@ __global__ void cc_reduce_reference_kernel(float2 *acc_G, float4 *acc_ab, double
 extern "C" cc_status cc_plan_update_reference_from_accumulator(cc_plan *plan, void *stream)
 {
     if (!plan) return fail(CC_ERR_INVALID_ARG, "cc_plan_update_reference_from_accumulator: null plan");
+    if (plan->sn && plan->acc_count > 0 && plan->sn_state) {
+        const CcSnTables t{plan->Gt, plan->ab, plan->ri_emean, plan->col_freq};
+        cudaError_t e = cc_sn_finish_pass(plan->sn_state, plan->acc_count, t, (cudaStream_t)stream);
+        if (e != cudaSuccess) return fail_cuda(e, "CC-SN reference update");
+        plan->acc_count = 0;
+        return CC_OK;
+    }
     if (plan->acc_count <= 0 || !plan->acc_G) return fail(CC_ERR_INVALID_ARG, "nothing accumulated: call cc_track_accumulate first");
     const int H = plan->H, Wh = plan->W / 2;
     const double invN = 1.0 / (double)plan->acc_count, inv = invN / ((double)H * (double)plan->W);
