@@ -92,6 +92,7 @@ struct CcParams {
                                   //        sum/difference layout: j = 0, H/2: D_H(t-j); 0 < j < H/2: even part; H-j: odd part
     const double2 *Xpol;          // [M][W/2] (cos, sin)(2 pi q (n - c) / (u W))
     const double *nyq64;          // [M] cos(pi (n - c) / u)
+    const double2 *XpolR;         // latency variants with pol_smem: Xpol regrouped by cluster rank, [CS][M][NC], else null
 
     // real-time session (cc_rt_*): mapped host memory; null outside a session
     const volatile unsigned long long *rt_cmd;  // [0] sequence number of the newest command (~0: quit), [1] frame pointer | seq & 15
@@ -129,6 +130,8 @@ struct CcParams {
     double sn_eps, sn_c0;
     double peak_sign;
     int u_bytes;        // bytes of the raw/scratch/T union region
+    int pol_smem;       // latency variants: 1 = the fp64 polish tables (Dpol, this CTA's Xpol columns, nyq64) are copied
+                        // into shared memory once per launch (they fit), 0 = read from global memory
     double Emean;       // mean of the reference image (DC add-back for `peak`)
 };
 
@@ -141,6 +144,7 @@ struct CcVariant {
     int BK1, G2;                // stage-1 k-rows per tile; stage-2 groups of 4 k-rows per tile
     int s_global;  // 1: spectrum array lives in global memory (L2), 0: shared memory / DSMEM
     int NSTG;
+    int lat;       // 1: small-batch (latency) variant
     size_t (*fixed_smem)();                 // bytes that do not depend on M (S, tables, misc), before U/stg
     int (*raw_scratch_bytes)();             // raw ring + FFT scratch (lower bound of the U region)
     cudaError_t (*prepare)(int smem_bytes);  // sets func attributes

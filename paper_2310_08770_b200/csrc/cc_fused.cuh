@@ -211,6 +211,26 @@ __device__ __forceinline__ void fft_bfly(Addr addr, Twf twf)
         *addr(k) = o;
     }
 }
+// The same butterfly with separate load / store functors: ld(i) -> float2 input i, st(k, value) output k.
+template <int R, bool INV, bool TW, class Ld, class St, class Twf>
+__device__ __forceinline__ void fft_bfly_io(Ld ld, St st, Twf twf)
+{
+    float2 v[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) v[i] = ld(i);
+    if (INV && TW) {
+#pragma unroll
+        for (int i = 1; i < R; ++i) v[i] = cmulc(v[i], twf(i));
+    }
+    dft_reg<R, INV>(v);
+    constexpr int bits = ilog2c(R);
+#pragma unroll
+    for (int k = 0; k < R; ++k) {
+        float2 o = v[brev(k, bits)];
+        if (!INV && TW && k > 0) o = cmul(o, twf(k));
+        st(k, o);
+    }
+}
 // twiddles from the table tw[j] = (cos, -sin)(2 pi j / NTW)
 template <int R, bool INV, bool TW, int NTW, class Addr>
 __device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw)
@@ -219,6 +239,15 @@ __device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw
 }
 
 __device__ __forceinline__ int padi(int i) { return i + (i >> 4); }  // 1 float2 of padding per 16
+
+// Slot holding frequency k after the forward row FFT of length N (cc_common.h: k = k1 + r0 k2 + r0 r1 k3  <->
+// p = k1 N/r0 + k2 N/(r0 r1) + k3): powers of two throughout, so a few shifts instead of a table lookup.
+template <int N>
+__device__ __forceinline__ int row_slot_of(int k)
+{
+    constexpr int r0 = cc_radix_row(N, 0), r1 = cc_radix_row(N, 1);
+    return (k % r0) * (N / r0) + ((k / r0) % r1) * (N / (r0 * r1)) + k / (r0 * r1);
+}
 
 // Per-lane twiddles of the warp-level row FFT of length N: a lane handles the same butterflies of every row, so
 // its twiddles are loaded from the shared table once per phase and stay in registers (the inverse conjugates).
@@ -286,6 +315,41 @@ __device__ __forceinline__ void warp_fft(float2 *sc, const RowTw<N, NTW> &rt, in
     }
 }
 
+// Forward warp FFT whose first pass reads input x from in(x) (the decoded pixels: no staging store + reload).
+template <int N, int NTW, class In>
+__device__ __forceinline__ void warp_fft_fwd_from(float2 *sc, const RowTw<N, NTW> &rt, int gl, In in)
+{
+    using T = RowTw<N, NTW>;
+    constexpr int R0 = T::R0, R1 = T::R1, R2 = T::R2, LP = T::LP, ST = N / R0;
+#pragma unroll
+    for (int n = 0; n < T::NB0; ++n) {
+        const int g = gl + LP * n;
+        if (g < ST)
+            fft_bfly_io<R0, false, true>([&](int i) { return in(g + i * ST); }, [&](int k, float2 o) { sc[padi(g + k * ST)] = o; },
+                                         [&](int i) { return rt.t0[n * (R0 - 1) + i - 1]; });
+    }
+    __syncwarp();
+    if constexpr (R1 > 1) warp_fft_pass<N, N / R0, R1, false, T::S1, LP>(sc, rt.t1, gl);
+    if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, false, 1, LP>(sc, rt.t1, gl);
+}
+// Inverse warp FFT whose last pass hands output x to out(x, value) (streamed into the argmax: no store + reload).
+template <int N, int NTW, class Out>
+__device__ __forceinline__ void warp_fft_inv_to(float2 *sc, const RowTw<N, NTW> &rt, int gl, Out out)
+{
+    using T = RowTw<N, NTW>;
+    constexpr int R0 = T::R0, R1 = T::R1, R2 = T::R2, LP = T::LP, ST = N / R0;
+    if constexpr (R2 > 1) warp_fft_pass<N, N / (R0 * R1), R2, true, 1, LP>(sc, rt.t1, gl);
+    if constexpr (R1 > 1) warp_fft_pass<N, N / R0, R1, true, T::S1, LP>(sc, rt.t1, gl);
+#pragma unroll
+    for (int n = 0; n < T::NB0; ++n) {
+        const int g = gl + LP * n;
+        if (g < ST)
+            fft_bfly_io<R0, true, true>([&](int i) { return sc[padi(g + i * ST)]; }, [&](int k, float2 o) { out(g + k * ST, o); },
+                                        [&](int i) { return rt.t0[n * (R0 - 1) + i - 1]; });
+    }
+    __syncwarp();
+}
+
 // argmax record: larger value wins; equal values -> smaller index wins.
 struct Best {
     float v;
@@ -311,7 +375,7 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
           int R2_, int KS2_, int NSTG_, int PFD_, int KS1_>
 struct Cfg {
     static constexpr int NSTG = NSTG_;  // staging ring depth
-    static constexpr int NBARS = NSTG + 5;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1]
+    static constexpr int NBARS = NSTG + 7;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish tables [1]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -384,9 +448,41 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long long t_entry = clock64();
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (CS > 1) ? (int)cluster.block_rank() : 0;
     const int cid = blockIdx.x / CS, ncl = gridDim.x / CS;
+    constexpr int RG = C::RG, LP = C::LP;
+    const int gl = lane % LP, gp = lane / LP;  // lane within its row pair, row pair within the warp
+
+    // ---- loads whose latency the whole setup hides: the plan's twiddle tables (all variants) and, in the latency
+    // variants whose CTA slice is one raw chunk, the pixels of the first frame straight into registers (a plain
+    // coalesced load arrives in about a third of the time of a TMA copy + mbarrier round trip)
+    constexpr int NI_TW = (C::NTW + NT - 1) / NT, NI_W = (W + NT - 1) / NT;
+    float2 r_tw[NI_TW];
+    double2 r_64[C::LAT ? NI_W : 1];
+#pragma unroll
+    for (int e = 0; e < NI_TW; ++e)
+        if (tid + e * NT < C::NTW) r_tw[e] = __ldg(&p.tw[tid + e * NT]);
+    if constexpr (C::LAT) {
+#pragma unroll
+        for (int e = 0; e < NI_W; ++e)
+            if (tid + e * NT < W) r_64[e] = __ldg(&p.tw64[tid + e * NT]);
+    }
+    constexpr bool DIRECT = C::LAT && C::NCHK == 1 && (C::RCH / 2) <= C::NWARP * RG;
+    constexpr int NPX = W / LP;  // pixels per row per lane in the decode
+    PIX pxa[DIRECT ? NPX : 1], pxb[DIRECT ? NPX : 1];
+    bool direct_first = false;   // the first frame's pixels ride in registers instead of the raw ring
+    if constexpr (DIRECT) {
+        direct_first = !p.rt_cmd && cid < p.batch;
+        const int jp = warp * RG + gp;
+        if (direct_first && jp < C::RCH / 2) {
+            const PIX *fb = reinterpret_cast<const PIX *>(p.frames) + (size_t)cid * H * W + (size_t)rank * C::NR * W;
+            const PIX *ga = fb + (size_t)jp * W, *gb = fb + (size_t)(jp + C::RCH / 2) * W;
+#pragma unroll
+            for (int i = 0; i < NPX; ++i) pxa[i] = __ldg(ga + gl + i * LP), pxb[i] = __ldg(gb + gl + i * LP);
+        }
+    }
 
     // ---- shared memory carve-up
     float2 *const Ssm = reinterpret_cast<float2 *>(smem);
@@ -398,6 +494,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
     uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
+    uint64_t *const tbar = cbar + 1, *const pbar = tbar + 1;
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     float *const wv = reinterpret_cast<float *>(xchg + 2 * CS * XN);    // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
@@ -405,8 +502,6 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
     uint32_t *const relcnt = reinterpret_cast<uint32_t *>(cmdslot + 2);  // [NSTG] releases of each ring slot (mod NWARP)
 
-    constexpr int RG = C::RG, LP = C::LP;
-    const int gl = lane % LP, gp = lane / LP;  // lane within its row pair, row pair within the warp
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + (warp * RG + gp) * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
 
@@ -473,59 +568,72 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if (++r_idx == (uint32_t)p.ntiles_frame) r_idx = 0;
     };
 
-    // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts the first NSTG operand tiles and
-    // the first frame's raw rows in flight; the table copies of all threads overlap those copies; one cluster
-    // barrier ends the setup.
+    // ---- one-time setup.  Thread 0 initialises the mbarriers and at once puts in flight (TMA bulk copies) the plan
+    // tables (FFT twiddles, slot table; fp64 twiddles and -- where they fit -- the fp64 polish tables of the latency
+    // variants), the first NSTG operand tiles and the first frame's raw rows.  The cluster barrier that makes the
+    // mbarriers of all CTAs visible is split: arrive here, wait just before the first remote access (after the first
+    // raw chunk has landed), so neither the table latency nor the barrier latency is exposed.
+    const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
+    double2 *const t64s = reinterpret_cast<double2 *>(((uintptr_t)(relcnt + NSTG) + 15) & ~(uintptr_t)15);   // [W] (LAT)
+    // resident polish tables (p.pol_smem): Dpol [M][H], this CTA's columns of Xpol [M][NC], nyq64 [M rounded up to even]
+    double *const DpolS = reinterpret_cast<double *>(t64s + (C::LAT ? W : 0));
+    double2 *const XpolS = reinterpret_cast<double2 *>(DpolS + (size_t)p.M * H);
+    double *const nyqS = reinterpret_cast<double *>(XpolS + (size_t)p.M * NC);
+    const bool POLS = C::LAT && p.pol_smem != 0;
     if (tid == 0) {
         for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), relcnt[i] = 0u;
         mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
         mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1), mbar_init(cbar, 1);
+        mbar_init(tbar, 1), mbar_init(pbar, 1);
         fence_mbar_init();
-        if (total_tiles > 0) {  // fill the ring; the first schedule entries ride in the kernel parameters: no load latency
-            fence_proxy_async();
-#pragma unroll
-            for (int i = 0; i < NSTG; ++i)
-                if ((uint32_t)i < total_tiles) {
-                    mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
-                    bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)p.sched_head[i] * C::TILEF, (uint32_t)C::TILEF * 4u,
-                             &bfull[i]);
-                }
-        }
-        if (!p.rt_cmd && cid < p.batch) issue_raw_head(p.frames, cid);
+        if (!p.rt_cmd && cid < p.batch && !direct_first) issue_raw_head(p.frames, cid);
     }
-    const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
-    {   // table copies: all loads first (independent, non-coherent path), then the stores
-        constexpr int NI_TW = (NTW + NT - 1) / NT, NI_W = (W + NT - 1) / NT;
-        float2 r_tw[NI_TW];
-        uint16_t r_rs[NI_W];
-        double2 r_64[C::LAT ? NI_W : 1];
 #pragma unroll
-        for (int e = 0; e < NI_TW; ++e)
-            if (tid + e * NT < NTW) r_tw[e] = __ldg(&p.tw[tid + e * NT]);
+    for (int e = 0; e < NI_TW; ++e)
+        if (tid + e * NT < NTW) tw[tid + e * NT] = r_tw[e];
+    if constexpr (C::LAT) {
 #pragma unroll
         for (int e = 0; e < NI_W; ++e)
-            if (tid + e * NT < W) {
-                r_rs[e] = __ldg(&p.row_slot[tid + e * NT]);
-                if constexpr (C::LAT) r_64[e] = __ldg(&p.tw64[tid + e * NT]);
+            if (tid + e * NT < W) t64s[tid + e * NT] = r_64[e];
+    }
+    if constexpr (C::LAT) tw64 = t64s;
+    __syncthreads();  // the mbarrier inits are visible to every thread of the CTA
+    // the copies nobody waits for yet are issued by other warps, beside the first phase: the operand ring ...
+    if (tid == 32 && total_tiles > 0) {  // the first schedule entries ride in the kernel parameters: no load latency
+#pragma unroll
+        for (int i = 0; i < NSTG; ++i)
+            if ((uint32_t)i < total_tiles) {
+                mbar_expect_tx(&bfull[i], (uint32_t)C::TILEF * 4u);
+                bulk_g2s(stg + (size_t)i * C::TILEF, p.blob + (size_t)p.sched_head[i] * C::TILEF, (uint32_t)C::TILEF * 4u, &bfull[i]);
             }
-#pragma unroll
-        for (int e = 0; e < NI_TW; ++e)
-            if (tid + e * NT < NTW) tw[tid + e * NT] = r_tw[e];
-#pragma unroll
-        for (int e = 0; e < NI_W; ++e)
-            if (tid + e * NT < W) rslot[tid + e * NT] = r_rs[e];
-        if constexpr (C::LAT) {
-            double2 *t64 = reinterpret_cast<double2 *>(((uintptr_t)(relcnt + NSTG) + 15) & ~(uintptr_t)15);
-#pragma unroll
-            for (int e = 0; e < NI_W; ++e)
-                if (tid + e * NT < W) t64[tid + e * NT] = r_64[e];
-            tw64 = t64;
-        }
     }
+    // ... and the resident fp64 polish tables (Dpol, this CTA's slice of the rank-major copy of Xpol, nyq64)
+    if (tid == 64 && POLS) {
+        const uint32_t db = (uint32_t)p.M * H * 8u, xb = (uint32_t)p.M * NC * 16u, nb = (uint32_t)((p.M + 1) & ~1) * 8u;
+        mbar_expect_tx(pbar, db + xb + nb);
+        for (uint32_t o = 0; o < db; o += 32768u)
+            bulk_g2s(reinterpret_cast<unsigned char *>(DpolS) + o, reinterpret_cast<const unsigned char *>(p.Dpol) + o,
+                     db - o < 32768u ? db - o : 32768u, pbar);
+        bulk_g2s(XpolS, p.XpolR + (size_t)rank * p.M * NC, xb, pbar);
+        bulk_g2s(nyqS, p.nyq64, nb, pbar);
+    }
+    bool csync_pending = false;  // the cluster half of the setup barrier: arrive now, wait before the first remote access
+    if constexpr (CS > 1) {
+        asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+        csync_pending = true;
+    }
+    auto setup_cluster_wait = [&]() {
+        if constexpr (CS > 1) {
+            if (csync_pending) {
+                asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+                csync_pending = false;
+            }
+        }
+    };
+    bool pol_pending = POLS;
     uint32_t ph = 0;   // phase parity bits of the raw ring
     int xpar = 0;      // exchange buffer parity
     uint32_t xph = 0;  // phase parity bits of the two exchange barriers
-    csync();
 
     const int u = p.u, M = p.M, cM = p.c;
     const double c0d = p.sn ? p.sn_c0 : (double)p.c0;  // constant subtracted from every (transformed) pixel
@@ -638,7 +746,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         for (int k = 0; k < 9; ++k) out[k] = __shfl_sync(0xffffffffu, mine, k);
     };
 
-    long long tph = 0;
+    long long tph = t_entry;  // the first frame's phase 0 includes the kernel setup
     auto stamp = [&](int k, int f) {  // optional per-phase cycle counts (rank 0, thread 0)
         if (p.phase_clk && rank == 0 && tid == 0) {
             const long long now = clock64();
@@ -749,12 +857,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         __threadfence();
     };
 
+    constexpr int RLc = cc_radix_col(H, 2) > 1 ? cc_radix_col(H, 2) : cc_radix_col(H, 1);  // radix of the fused column pass
+    constexpr bool GPRE = C::LAT && NC * (H / RLc) <= NT;
+    float2 gpre[GPRE ? RLc : 1];
     for (int f = cid; RT || f < p.batch; f += ncl) {
         const void *frames = p.frames;
         if (RT) {
             // ---- real-time session (one displacement per camera frame, as it arrives): rank 0
             // polls the host's command word; (seq, frame pointer) go to every CTA of the cluster by st.async
             f = 0;
+            setup_cluster_wait();  // the peers' command barriers exist
             if constexpr (CS > 1) {
                 if (tid == 0) mbar_expect_tx(cbar, 16u);
             }
@@ -796,47 +908,76 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             frames = reinterpret_cast<const void *>(cmdslot[1]);
             if (tid == 0) issue_raw_head(frames, 0);
         }
-        if (p.phase_clk && rank == 0 && tid == 0) tph = clock64();
+        if (p.phase_clk && rank == 0 && tid == 0 && (RT || f != cid)) tph = clock64();  // first frame: phase 0 includes the setup
         // =============================================================== a1 + a2: ingest and row FFTs
         {
             const PIX *fbase = reinterpret_cast<const PIX *>(frames) + (size_t)f * H * W + (size_t)rank * NR * W;
             if (tid == 0 && !RT && f != cid) issue_raw_head(frames, f);  // the first frame's rows were requested during the setup
+            // latency variants: every thread owns at most one butterfly of the fused column pass; its RL values of
+            // conj(G)/(HW) are requested now (L2 latency hidden behind the ingest and the row FFTs)
+            if constexpr (GPRE) {
+                if (tid < NC * (H / RLc)) {
+                    const int ql = tid % NC, g = tid / NC, q = rank * NC + ql;
+                    if (q != 0) {
+#pragma unroll
+                        for (int k = 0; k < RLc; ++k) gpre[k] = __ldcg(&p.Gt[(size_t)(g * RLc + k) * (W / 2) + q]);
+                    }
+                }
+            }
             RowTw<W, NTW> rtw;
             rtw.load(tw, lane);
             const float c0f = (float)p.c0;
+            const bool from_regs = DIRECT && direct_first && f == cid;  // first frame of a latency variant
             for (int ck = 0; ck < C::NCHK; ++ck) {
                 const int rb = ck & 1;
-                bar_wait(rb);
+                if (!from_regs) bar_wait(rb);
+                setup_cluster_wait();  // first frame: every CTA of the cluster is set up (remote stores follow)
                 const PIX *rw = raw + (size_t)rb * C::RCH * W;
                 for (int jp0 = warp * RG; jp0 < C::RCH / 2; jp0 += NWARP * RG) {
                     const int jp = jp0 + gp;
                     const PIX *ra = rw + (size_t)jp * W;
                     const PIX *rbp = rw + (size_t)(jp + C::RCH / 2) * W;
-                    for (int x = gl; x < W; x += LP)
-                        if (p.sn) {  // CC-SN: I'^2 - c0 with I' = I + eps (Eq. (7)), one rounding
-                            const double ta = (double)ra[x] + p.sn_eps, tb = (double)rbp[x] + p.sn_eps;
-                            scr[padi(x)] = make_float2((float)fma(ta, ta, -p.sn_c0), (float)fma(tb, tb, -p.sn_c0));
+                    // decode fused into the first FFT pass: pixel x of the two rows is input x of the complex row FFT
+                    warp_fft_fwd_from<W, NTW>(scr, rtw, gl, [&](int x) {
+                        PIX va, vb;
+                        if constexpr (DIRECT) {
+                            const int i = (x - gl) / LP;  // compile-time after unrolling
+                            va = from_regs ? pxa[i] : ra[x], vb = from_regs ? pxb[i] : rbp[x];
                         } else {
-                            scr[padi(x)] = make_float2((float)ra[x] - c0f, (float)rbp[x] - c0f);
+                            va = ra[x], vb = rbp[x];
                         }
-                    __syncwarp();
-                    warp_fft<W, false, NTW>(scr, rtw, gl);
+                        if (p.sn) {  // CC-SN: I'^2 - c0 with I' = I + eps (Eq. (7)), one rounding
+                            const double ta = (double)va + p.sn_eps, tb = (double)vb + p.sn_eps;
+                            return make_float2((float)fma(ta, ta, -p.sn_c0), (float)fma(tb, tb, -p.sn_c0));
+                        }
+                        return make_float2((float)va - c0f, (float)vb - c0f);
+                    });
                     // untangle the two real rows and scatter to the column owners
                     const int ya = rank * NR + ck * C::RCH + jp, yb = ya + C::RCH / 2;
-                    for (int k = gl; k < W / 2; k += LP) {
-                        float2 A, B;
-                        if (k == 0) {
-                            const float2 z0 = scr[padi(rslot[0])], zn = scr[padi(rslot[W / 2])];
-                            A = make_float2(z0.x, zn.x);
-                            B = make_float2(z0.y, zn.y);
-                        } else {
-                            const float2 z1 = scr[padi(rslot[k])], z2 = scr[padi(rslot[W - k])];
-                            A = make_float2(0.5f * (z1.x + z2.x), 0.5f * (z1.y - z2.y));
-                            B = make_float2(0.5f * (z1.y + z2.y), -0.5f * (z1.x - z2.x));
+                    {
+                        constexpr int NK = (W / 2) / LP;  // spectrum columns per lane
+                        float2 z1[NK], z2[NK];
+#pragma unroll
+                        for (int i = 0; i < NK; ++i) {
+                            const int k = gl + i * LP;
+                            z1[i] = scr[padi(row_slot_of<W>(k))];
+                            z2[i] = scr[padi(row_slot_of<W>(k == 0 ? W / 2 : W - k))];
                         }
-                        float2 *Sd = Sof(k / NC);
-                        Sd[(size_t)ya * NC + (k % NC)] = A;
-                        Sd[(size_t)yb * NC + (k % NC)] = B;
+#pragma unroll
+                        for (int i = 0; i < NK; ++i) {
+                            const int k = gl + i * LP;
+                            float2 A, B;
+                            if (k == 0) {  // z1 = slot of frequency 0, z2 = slot of frequency W/2
+                                A = make_float2(z1[i].x, z2[i].x);
+                                B = make_float2(z1[i].y, z2[i].y);
+                            } else {
+                                A = make_float2(0.5f * (z1[i].x + z2[i].x), 0.5f * (z1[i].y - z2[i].y));
+                                B = make_float2(0.5f * (z1[i].y + z2[i].y), -0.5f * (z1[i].x - z2[i].x));
+                            }
+                            float2 *Sd = Sof(k / NC);
+                            Sd[(size_t)ya * NC + (k % NC)] = A;
+                            Sd[(size_t)yb * NC + (k % NC)] = B;
+                        }
                     }
                     __syncwarp();
                 }
@@ -876,6 +1017,16 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             for (int it = tid; it < NC * (H / RL); it += NT) {
                 const int ql = it % NC, g = it / NC;
                 const int q = rank * NC + ql;
+                // the butterfly's RL values of conj(G)/(HW) are requested first (through L2: the RI update rewrites Gt),
+                // so their latency runs under the shared-memory loads and the forward DFT
+                float2 gv[RL];
+                if constexpr (GPRE) {
+#pragma unroll
+                    for (int k = 0; k < RL; ++k) gv[k] = gpre[k];  // requested at the start of the frame
+                } else if (q != 0) {
+#pragma unroll
+                    for (int k = 0; k < RL; ++k) gv[k] = __ldcg(&p.Gt[(size_t)(g * RL + k) * (W / 2) + q]);
+                }
                 float2 v[RL];
 #pragma unroll
                 for (int i = 0; i < RL; ++i) v[i] = Sl[(size_t)(g * RL + i) * NC + ql];
@@ -890,7 +1041,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     for (int k = 0; k < RL; ++k) {
                         const size_t gi = (size_t)(g * RL + k) * (W / 2) + q;
                         if (RI) __stcg(&Fs_of()[gi], v[brev(k, bits)]);  // the frame's spectrum feeds the RI update
-                        w[k] = cmul(v[brev(k, bits)], __ldcg(&p.Gt[gi]));  // through L2: the RI update rewrites Gt
+                        w[k] = cmul(v[brev(k, bits)], gv[k]);
                     }
                     dft_reg<RL, true>(w);
 #pragma unroll
@@ -958,25 +1109,34 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             for (int jp0 = warp * RG; jp0 < NR / 2; jp0 += NWARP * RG) {
                 const int jp = jp0 + gp;
                 const int ya = rank * NR + jp, yb = ya + NR / 2;
-                for (int k = gl; k < W / 2; k += LP) {
-                    const float2 *Sd = Sof(k / NC);
-                    const float2 qa = Sd[(size_t)ya * NC + (k % NC)], qb = Sd[(size_t)yb * NC + (k % NC)];
-                    if (k == 0) {
-                        scr[padi(rslot[0])] = make_float2(qa.x, qb.x);
-                        scr[padi(rslot[W / 2])] = make_float2(qa.y, qb.y);
-                    } else {
-                        scr[padi(rslot[k])] = make_float2(qa.x - qb.y, qa.y + qb.x);
-                        scr[padi(rslot[W - k])] = make_float2(qa.x + qb.y, qb.x - qa.y);
+                {
+                    constexpr int NK = (W / 2) / LP;  // spectrum columns per lane
+                    float2 qa[NK], qb[NK];
+#pragma unroll
+                    for (int i = 0; i < NK; ++i) {  // all loads first: the (remote, for k / NC != rank) latencies overlap
+                        const int k = gl + i * LP;
+                        const float2 *Sd = Sof(k / NC);
+                        qa[i] = Sd[(size_t)ya * NC + (k % NC)];
+                        qb[i] = Sd[(size_t)yb * NC + (k % NC)];
+                    }
+#pragma unroll
+                    for (int i = 0; i < NK; ++i) {
+                        const int k = gl + i * LP;
+                        if (k == 0) {
+                            scr[padi(row_slot_of<W>(0))] = make_float2(qa[i].x, qb[i].x);
+                            scr[padi(row_slot_of<W>(W / 2))] = make_float2(qa[i].y, qb[i].y);
+                        } else {
+                            scr[padi(row_slot_of<W>(k))] = make_float2(qa[i].x - qb[i].y, qa[i].y + qb[i].x);
+                            scr[padi(row_slot_of<W>(W - k))] = make_float2(qa[i].x + qb[i].y, qb[i].x - qa[i].y);
+                        }
                     }
                 }
                 __syncwarp();
-                warp_fft<W, true, NTW>(scr, rtw, gl);
-                for (int x = gl; x < W; x += LP) {
-                    const float2 z = scr[padi(x)];
+                // the last inverse pass streams its outputs (two rows of the correlation) into the argmax
+                warp_fft_inv_to<W, NTW>(scr, rtw, gl, [&](int x, float2 z) {
                     if (better(z.x, ya * W + x, bst.v, bst.i)) bst.v = z.x, bst.i = ya * W + x;
                     if (better(z.y, yb * W + x, bst.v, bst.i)) bst.v = z.y, bst.i = yb * W + x;
-                }
-                __syncwarp();
+                });
             }
             const Best g = cluster_best(bst);
             y0 = g.i / W;
@@ -1334,27 +1494,38 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             double *dtab = reinterpret_cast<double *>(U);                      // [3][H]
             double2 *part = reinterpret_cast<double2 *>(dtab + 3 * H);         // [3][NSL][NC]
             double *terms = reinterpret_cast<double *>(part + 3 * NSL * NC);   // [9][NC]
+            if (pol_pending) {  // first frame: the resident polish tables (TMA copies issued during the setup) have landed
+                mbar_wait(pbar, 0u);
+                pol_pending = false;
+            }
             for (int iter = 0; iter < 8; ++iter) {
                 // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
                 // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j'):
-                // rows ms-1..ms+1 of the plan's fp64 table Dpol[M][H] (zero weights outside the grid)
+                // rows ms-1..ms+1 of the plan's fp64 table Dpol[M][H] (out-of-grid rows: their values are never used)
+                const double *dr0 = dtab, *dr1 = dtab + H, *dr2 = dtab + 2 * H;
+                if (POLS) {
+                    dr0 = DpolS + (size_t)min(max(ms - 1, 0), M - 1) * H;
+                    dr1 = DpolS + (size_t)min(max(ms, 0), M - 1) * H;
+                    dr2 = DpolS + (size_t)min(max(ms + 1, 0), M - 1) * H;
+                } else {
 #pragma unroll
-                for (int it = 0; it < (3 * H + NT - 1) / NT; ++it) {  // unrolled: all loads of a thread go out together
-                    const int e = tid + it * NT;
-                    if (e < 3 * H) {
-                        const int a = e / H, j = e % H;
-                        const int mm = ms - 1 + a;
-                        dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
+                    for (int it = 0; it < (3 * H + NT - 1) / NT; ++it) {  // unrolled: all loads of a thread go out together
+                        const int e = tid + it * NT;
+                        if (e < 3 * H) {
+                            const int a = e / H, j = e % H;
+                            const int mm = ms - 1 + a;
+                            dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
+                        }
                     }
+                    __syncthreads();
                 }
-                __syncthreads();
                 for (int e = tid; e < NSL * NC; e += NT) {
                     const int ql = e % NC, sl = e / NC;
                     double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
                     for (int j = sl; j < H; j += NSL) {
                         const float2 v = Sl[(size_t)((y0 + j) & (H - 1)) * NC + ql];
                         const double vx = (double)v.x, vy = (double)v.y;
-                        const double d0 = dtab[j], d1 = dtab[H + j], d2 = dtab[2 * H + j];
+                        const double d0 = dr0[j], d1 = dr1[j], d2 = dr2[j];
                         s0.x = fma(d0, vx, s0.x), s0.y = fma(d0, vy, s0.y);
                         s1.x = fma(d1, vx, s1.x), s1.y = fma(d1, vy, s1.y);
                         s2.x = fma(d2, vx, s2.x), s2.y = fma(d2, vy, s2.y);
@@ -1368,7 +1539,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 #pragma unroll
                 for (int b = 0; b < 3; ++b) {
                     const int nn = min(max(ns - 1 + b, 0), M - 1);  // out-of-grid neighbours are skipped below
-                    nyq[b] = sgx * __ldg(&p.nyq64[nn]);
+                    nyq[b] = sgx * (POLS ? nyqS[nn] : __ldg(&p.nyq64[nn]));
                 }
                 __syncthreads();
                 xeval9(
@@ -1389,7 +1560,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         // exp(2 pi i q (x0 u + n - c) / (u W)) = exp(2 pi i q x0 / W) * exp(2 pi i q (n - c) / (u W))
                         const int nn = min(max(ns - 1 + b, 0), M - 1);
                         const double2 w0 = tw64[(q * x0) & (W - 1)];
-                        const double2 w1 = __ldg(&p.Xpol[(size_t)nn * (W / 2) + q]);
+                        const double2 w1 = POLS ? XpolS[(size_t)nn * NC + (q - rank * NC)] : __ldg(&p.Xpol[(size_t)nn * (W / 2) + q]);
                         return make_double2(w0.x * w1.x - w0.y * w1.y, w0.x * w1.y + w0.y * w1.x);
                     },
                     nyq, terms, c9);
@@ -1486,6 +1657,7 @@ struct Launcher {
         v.KS1 = C::KS1;
         v.s_global = C::SG ? 1 : 0;
         v.NSTG = C::NSTG;
+        v.lat = C::LAT ? 1 : 0;
         v.fixed_smem = &fixed_smem;
         v.raw_scratch_bytes = &raw_scratch_bytes;
         v.prepare = &prepare;
