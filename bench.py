@@ -32,6 +32,10 @@ from paper_2310_08770_b200 import workloads as wl  # noqa: E402
 
 NOMINAL_SM_MHZ = 1965.0
 FP32_LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one 10,000-frame launch, from the committed capture
+TRAFFIC_BYTES_PER_10K_LAUNCH = 1.3173e9
+TRAFFIC_SOURCE = ("ncu --set full capture of one 10,000-frame launch, raw rows in profiles/r2a_cfg3_raw_metrics.csv "
+                  "(dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes 1.3108e9")
 
 
 def flops_per_frame(H, W, u):
@@ -241,7 +245,15 @@ def run_table1(args):
                 lat_rt = rt.latency_probe(d.data_ptr(), 100)[3]
             finally:
                 rt.close()
+            # the paper's real-time method like for like ("CC-SN algorithm implementations", with the
+            # reference image updated after every image, Eq. (9); R19): cc_track(batch 1) + synchronise per image
+            plan.enable_reference_update(0.02)
+            plan.latency_probe(d, 20)
+            lat_upd = plan.latency_probe(d, 100)[3]
+            plan.enable_reference_update(0.0)
             print(json.dumps({"rows_x_cols": "%dx%d" % (H, W), "u": u, "method": "CC-SN",
+                              "images_per_s_single_frame_calls_with_reference_update": 1e6 / float(np.median(lat_upd)),
+                              "single_frame_latency_us_median_with_reference_update": float(np.median(lat_upd)),
                               "images_per_s_single_frame_calls": 1e6 / float(np.median(lat)),
                               "single_frame_latency_us_median": float(np.median(lat)),
                               "images_per_s_rt_session": 1e6 / float(np.median(lat_rt)),
@@ -273,6 +285,49 @@ def run_table1(args):
                           "rt_session_latency_us_p99": float(np.percentile(lat_rt, 99)),
                           "median_error_px": float(np.median(np.hypot(dx - sh[:, 1], dy - sh[:, 0]))),
                           "paper": "470 Hz sustained, camera/USB3-limited, RTX 3080 Ti (PAPER.md:L210-216)"}), flush=True)
+
+
+def run_tc_probe():
+    """--tc-probe: the measured tensor-core experiment for the upsampled-DFT products (include/cc_bench.h,
+    cc_tc_gemm_probe): accuracy of 1 x TF32 / 3 x TF32 against float64 on stage-1 operands of cfg 3
+    (even Dirichlet weights x sums of rows of Q of a real frame) and the MMA rate with every SM busy."""
+    from paper_2310_08770_b200 import tc_gemm_probe
+    cfg = wl.config(3)
+    H, W, u = cfg.H, cfg.W, cfg.upsample
+    fr = wl.frames(cfg, [5])[0].astype(np.float64)
+    ref = wl.reference(cfg).astype(np.float64)
+    P = np.fft.fft2(fr - 50.0) * np.conj(np.fft.fft2(ref)) / (H * W)
+    P[0, 0] = 0
+    y0, _ = np.unravel_index(np.argmax(np.fft.ifft2(P).real), (H, W))
+    Q = np.fft.ifft(P, axis=0)[:, 1:65]                                   # the 64 columns of one CTA
+
+    def dirichlet(t):
+        x = np.pi * np.asarray(t, dtype=np.float64) / H
+        with np.errstate(divide="ignore", invalid="ignore"):
+            v = np.sin(np.pi * t) * np.cos(x) / (H * np.sin(x))
+        return np.where(np.abs(np.sin(x)) < 1e-15, 1.0, v)
+    K = 192
+    A, B = np.zeros((128, K)), np.zeros((K, 128))
+    for j in range(H // 2 + 1):
+        row = Q[(y0 + j) % H] if j in (0, H // 2) else Q[(y0 + j) % H] + Q[(y0 - j) % H]
+        B[j, 0::2], B[j, 1::2] = row.real, row.imag
+        dd = np.arange(76) / u
+        A[:76, j] = dirichlet(dd - j) if j in (0, H // 2) else 0.5 * (dirichlet(dd - j) + dirichlet(dd + j))
+    A32, B32 = A.astype(np.float32), B.astype(np.float32)
+    Dref = A32.astype(np.float64) @ B32.astype(np.float64)
+    scale = np.abs(Dref).max()
+    out = {"experiment": "tcgen05.mma kind::tf32, 128x128xK products per SM, accumulator in tensor memory", "K": K,
+           "fp32_host_sgemm_err": float(np.abs((A32 @ B32) - Dref).max() / scale)}
+    for passes in (1, 3):
+        D, sc, mc = tc_gemm_probe(A32, B32, passes=passes, iters=200)
+        out["tf32_x%d" % passes] = {"max_err_rel_to_result_scale": float(np.abs(D - Dref).max() / scale),
+                                    "staging_cycles_per_product": sc, "mma_cycles_per_product": mc}
+    r2 = tc_gemm_probe(A32, B32, passes=3, iters=100, repeat=2)[2]
+    r6 = tc_gemm_probe(A32, B32, passes=3, iters=100, repeat=6)[2]
+    per_mma = (r6 - r2) / (4 * 3 * (K // 8))
+    out["cycles_per_128x128x8_mma_all_sms_busy"] = per_mma
+    out["tf32_tflops_chip"] = 2.0 * 128 * 128 * 8 / per_mma * 148 * NOMINAL_SM_MHZ * 1e6 / 1e12
+    print(json.dumps(out))
 
 
 def run_reference(args, cfg):
@@ -321,12 +376,16 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--table", action="store_true", help="per-config numbers for BASELINE.md section 3 and exit")
     ap.add_argument("--table1", action="store_true", help="the paper's Table I settings (context numbers) and exit")
+    ap.add_argument("--tc-probe", action="store_true", help="tensor-core experiment for the upsampled-DFT products and exit")
     ap.add_argument("--phases", action="store_true", help="print the per-phase cycle breakdown of every config and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
     if args.phases:
         run_phases()
+        return
+    if args.tc_probe:
+        run_tc_probe()
         return
     if args.table:
         run_table(args)
@@ -365,6 +424,7 @@ def main():
         frames = np.concatenate([frames] * ((B + uniq - 1) // uniq))[:B]
     ref = wl.reference(cfg)
     t_gen = time.perf_counter() - t_gen
+    input_checksum = wl.checksum(frames)          # sum of all pixels + SHA-256 of frame 0 of the timed batch
     plan = Plan(cfg.H, cfg.W, frames.dtype, cfg.upsample, ref)
     info = plan.info()
     dfr = plan.device_frames(frames)
@@ -418,6 +478,8 @@ def main():
                "api": "cc_track_host (pinned host frames in, host dx/dy/peak out)"}
         same = bool(np.array_equal(hdx.numpy(), out[0].cpu().numpy()) and np.array_equal(hdy.numpy(), out[1].cpu().numpy()))
         e2e["matches_device_path"] = same
+        if not same:
+            raise SystemExit("bench.py: cc_track_host returned displacements that differ from cc_track on the same frames")
 
     if rank != 0:
         if world > 1:
@@ -439,7 +501,11 @@ def main():
     t_hbm = (frames[0].nbytes + 12) / (hbm_gbs * 1e9)
     roofline = {
         "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": 1.318e9, "traffic_source": "ncu --set full capture profiles/r1j_summary.md: dram read 1.3128 GB + write 4.7 MB per 10,000-frame launch", "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
+        "achieved_is": "ALGORITHMIC flop of SURVEY.md 8(d) (naive two-product upsampled DFT, 56.7 MFLOP per frame) / kernel time; "
+                       "the kernel's even/odd formulation executes 21.3 MFLOP per frame: see frac_executed",
+        "frac_executed": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12 / peak_tf,
+        "traffic": TRAFFIC_BYTES_PER_10K_LAUNCH * B / 10000.0, "traffic_source": TRAFFIC_SOURCE,
+        "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,
         "flop_per_frame": flop, "executed_flop_per_frame": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample),
         "executed_tflops": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); FFMA-loop probe measured %.1f TFLOP/s" % probe_tf,
@@ -524,7 +590,8 @@ def main():
                    "frames_per_step_per_gpu": B, "unique_frames": int(uniq), "parallelism": "replicas x%d" % world,
                    "l2": "inputs (%.2f GB per step) larger than L2" % (frames.nbytes / 1e9),
                    "cluster_size": info["cluster_size"], "clusters_resident": info["max_clusters"],
-                   "threads": info["threads"], "smem_bytes": info["smem_bytes"], "gen_s": round(t_gen, 1)},
+                   "threads": info["threads"], "smem_bytes": info["smem_bytes"], "gen_s": round(t_gen, 1),
+                   "input_checksum": input_checksum},
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu,
         "latency": latency, "wall_s_timed_region": wall,
     }

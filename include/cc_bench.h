@@ -52,6 +52,26 @@ cc_status cc_fp32_peak_probe(double *tflops, void *stream);
  */
 cc_status cc_fp32_tile_probe(double *tflops, void *stream);
 
+/*
+ * cc_tc_gemm_probe -- measured tensor-core experiment for step a6 (the upsampled DFT as matrix products,
+ * PAPER.md:L90; "the most computationally intensive component", L163).  Every SM computes the 128 x 128 x K product
+ * D = A B with tcgen05.mma kind::tf32 (accumulator in tensor memory): passes = 1 a single TF32 product, passes = 3
+ * the split A_hi B_hi + A_lo B_hi + A_hi B_lo that carries ~22 bits of each operand.  Not used by cc_track: the
+ * decision path stays FP32 + float64; this call provides the numbers behind that choice.
+ *   A        HOST pointer, 128 x K float32, row-major (the plan-constant operand, e.g. Dirichlet weights)
+ *   B        HOST pointer, K x 128 float32, row-major (the data operand, e.g. rows of Q)
+ *   K        multiple of 64
+ *   repeat   >= 1: every staged K tile is multiplied `repeat` times (D = repeat * A B): the slope of mma_cycles
+ *            against repeat is the issue-to-completion rate of the MMAs without the staging round trip
+ *   D        HOST pointer, receives 128 x 128 float32, row-major
+ *   stage_cycles, mma_cycles   HOST pointers (may be NULL): SM cycles per product spent staging the operands in
+ *            shared memory (load, hi/lo split, UMMA core-matrix layout) and from the first tcgen05.mma to the
+ *            completion of the last, averaged over `iters` repetitions with all SMs busy
+ * Synchronises the device.  CC_ERR_INVALID_ARG / CC_ERR_ARCH / CC_ERR_CUDA.
+ */
+cc_status cc_tc_gemm_probe(const float *A, const float *B, int K, int passes, int iters, int repeat, float *D,
+                           double *stage_cycles, double *mma_cycles);
+
 #ifdef __cplusplus
 }
 #endif

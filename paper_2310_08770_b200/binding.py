@@ -13,7 +13,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcc_b200.so")
+# CC_B200_LIB selects another build of the same library (the schedule-fuzzing build libcc_b200_fuzz.so of build.py --fuzz)
+LIB_PATH = os.environ.get("CC_B200_LIB") or os.path.join(_HERE, "libcc_b200.so")
 
 CC_U8, CC_U16 = 0, 1
 _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
@@ -22,7 +23,7 @@ _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_
 EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host",
            "cc_plan_set_host_chunk", "cc_plan_destroy",
            "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_plan_get_reference_spectrum_f64", "cc_track_accumulate",
-           "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_track_latency_probe",
+           "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_tc_gemm_probe", "cc_track_latency_probe",
            "cc_rt_open", "cc_rt_submit", "cc_rt_wait", "cc_rt_track", "cc_rt_close", "cc_rt_latency_probe", "cc_status_string", "cc_last_error"]
 
 
@@ -102,6 +103,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_drift_correct.restype = ci
         lib.cc_fp32_tile_probe.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         lib.cc_fp32_tile_probe.restype = ci
+        lib.cc_tc_gemm_probe.argtypes = [vp, vp, ci, ci, ci, ci, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        lib.cc_tc_gemm_probe.restype = ci
         lib.cc_status_string.argtypes = [ci]
         lib.cc_status_string.restype = ctypes.c_char_p
         lib.cc_last_error.restype = ctypes.c_char_p
@@ -339,3 +342,18 @@ def drift_correct(dx, dy, a0: float, max_step: float = 0.0, state=None, stream=N
     _check(load_library().cc_drift_correct(dx.data_ptr(), dy.data_ptr(), n, float(a0), float(max_step), state.data_ptr(),
                                            ox.data_ptr(), oy.data_ptr(), s))
     return ox, oy, state
+
+
+def tc_gemm_probe(A, B, passes: int = 3, iters: int = 50, repeat: int = 1):
+    """cc_tc_gemm_probe: D = A B (128 x K times K x 128) on the tensor cores (TF32, 1 or 3 passes).
+    Returns (D, stage_cycles, mma_cycles)."""
+    _torch()
+    A = np.ascontiguousarray(A, dtype=np.float32)
+    B = np.ascontiguousarray(B, dtype=np.float32)
+    assert A.shape[0] == 128 and B.shape[1] == 128 and A.shape[1] == B.shape[0]
+    D = np.empty((128, 128), np.float32)
+    sc, mc = ctypes.c_double(), ctypes.c_double()
+    vp = ctypes.c_void_p
+    _check(load_library().cc_tc_gemm_probe(A.ctypes.data_as(vp), B.ctypes.data_as(vp), A.shape[1], int(passes), int(iters), int(repeat),
+                                           D.ctypes.data_as(vp), ctypes.byref(sc), ctypes.byref(mc)))
+    return D, sc.value, mc.value

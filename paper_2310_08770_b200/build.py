@@ -49,19 +49,38 @@ def _run(cmd, log):
     return r.stdout
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, fuzz: bool = False) -> str:
+    """fuzz=True builds libcc_b200_fuzz.so: the same library with -DCC_FUZZ (random delays before every
+    synchronisation point; the race check of profiles/sanitizer_r2.md).  Load it with CC_B200_LIB=<path>."""
+    global OBJ, LIB
+    if fuzz:
+        return _build_fuzz(force, verbose)
+    return _build(force, verbose, [])
+
+
+def _build_fuzz(force, verbose):
+    global OBJ, LIB
+    obj0, lib0 = OBJ, LIB
+    OBJ, LIB = os.path.join(HERE, "build_fuzz"), os.path.join(HERE, "libcc_b200_fuzz.so")
+    try:
+        return _build(force, verbose, ["-DCC_FUZZ"])
+    finally:
+        OBJ, LIB = obj0, lib0
+
+
+def _build(force, verbose, extra):
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_src():
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     jobs = []
     for v in variants():
         obj = os.path.join(OBJ, "v_%s.o" % v["NAME"])
-        cmd = [NVCC] + FLAGS + ["-c", os.path.join(CSRC, "cc_variant.cu"), "-o", obj] + \
+        cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, "cc_variant.cu"), "-o", obj] + \
               ["-DCCV_%s=%s" % (k, v[k]) for k in _KEYS]
         jobs.append((cmd, obj))
-    for src in ("cc_api", "cc_refupdate"):
+    for src in ("cc_api", "cc_refupdate", "cc_tc_probe"):
         o = os.path.join(OBJ, src + ".o")
-        jobs.append(([NVCC] + FLAGS + ["-c", os.path.join(CSRC, src + ".cu"), "-o", o], o))
+        jobs.append(([NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src + ".cu"), "-o", o], o))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         outs = list(ex.map(lambda j: _run(j[0], j[1] + ".log"), jobs))
     if verbose:
@@ -77,4 +96,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True, fuzz="--fuzz" in sys.argv))

@@ -29,6 +29,26 @@ namespace cg = cooperative_groups;
 
 constexpr int XN = 10;    // doubles per cluster-exchange record
 
+// ------------------------------------------------------------------ schedule fuzzing (build.py --fuzz: -DCC_FUZZ)
+// compute-sanitizer is closed on the pool this was developed on, so the race check is done by perturbation: in the fuzz
+// build every synchronisation point (mbarrier waits, ring acquire / release, cluster exchanges, CTA / cluster barriers,
+// warp-level FFT passes) is preceded by a pseudo-random per-LANE delay of up to ~2 us.  A missing barrier or a slot
+// released too early then shows up as results that change from run to run or differ from the plain build
+// (paper_2310_08770_b200/selftest.py --compare-fuzz; profiles/sanitizer_r2.md).
+#ifdef CC_FUZZ
+__device__ __forceinline__ void cc_jitter()
+{
+    unsigned c = (unsigned)clock64();
+    unsigned h = (c ^ (threadIdx.x * 2654435761u) ^ (blockIdx.x * 40503u)) * 2246822519u;
+    h ^= h >> 15;
+    if ((h & 7u) == 0u) __nanosleep((h >> 8) & 2047u);
+}
+#define CC_JITTER() cc_jitter()
+#define __syncthreads() (cc_jitter(), __syncthreads())
+#else
+#define CC_JITTER() ((void)0)
+#endif
+
 // ------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *b, uint32_t cnt)
@@ -41,6 +61,7 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes)
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity)
 {
+    CC_JITTER();
     uint32_t ok;
     const uint32_t a = smem_u32(b);
     do {
@@ -286,6 +307,7 @@ template <int N, int L, int R, bool INV, int SETS, int LP>
 __device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int gl)
 {
     constexpr int ST = L / R, NB = (N / R + LP - 1) / LP;
+    CC_JITTER();
 #pragma unroll
     for (int n = 0; n < NB; ++n) {
         const int g = gl + LP * n;
@@ -513,6 +535,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         return Ssm;
     };
     auto csync = [&]() {
+        CC_JITTER();
         if constexpr (CS > 1) cluster.sync();
         else __syncthreads();
     };
@@ -552,6 +575,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         return stg + (size_t)c_slot * C::TILEF;
     };
     auto ring_release = [&]() {
+        CC_JITTER();
         __syncwarp();
         if (lane == 0) {
             __threadfence_block();  // this warp's reads of the slot are done before the count says so
@@ -647,6 +671,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if constexpr (CS > 1) mbar_expect_tx(&xbar[xpar], (uint32_t)(CS * bytes_per_rank));
     };
     auto xchg_send = [&](int k, uint64_t bits, int r) {  // my record word k -> rank r
+        CC_JITTER();
         if constexpr (CS > 1) {
             const uint32_t dst = mapa_u32(smem_u32(xchg + ((size_t)xpar * CS + rank) * XN + k), (uint32_t)r);
             st_async_b64(dst, bits, mapa_u32(smem_u32(&xbar[xpar]), (uint32_t)r));
@@ -997,6 +1022,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             constexpr int RL = R2 > 1 ? R2 : R1;   // radix of the last forward pass (fused with the product)
             constexpr int NPASS = R2 > 1 ? 3 : 2;
             // forward pass 0
+            #pragma unroll(SG ? 2 : 1)
             for (int it = tid; it < NC * (H / R0); it += NT) {
                 const int ql = it % NC, g = it / NC;
                 constexpr int ST = H / R0;
@@ -1005,6 +1031,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             __syncthreads();
             if constexpr (NPASS == 3) {  // forward pass 1 of 3
                 constexpr int L = H / R0, ST = L / R1;
+                #pragma unroll(SG ? 2 : 1)
                 for (int it = tid; it < NC * (H / R1); it += NT) {
                     const int ql = it % NC, g = it / NC;
                     const int blk = g / ST, b = g % ST;
@@ -1014,6 +1041,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 __syncthreads();
             }
             // last forward pass (contiguous slots), product with conj(G)/(HW), first inverse pass
+            #pragma unroll(SG ? 2 : 1)
             for (int it = tid; it < NC * (H / RL); it += NT) {
                 const int ql = it % NC, g = it / NC;
                 const int q = rank * NC + ql;
@@ -1082,6 +1110,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             }
             if constexpr (NPASS == 3) {  // inverse of forward pass 1
                 constexpr int L = H / R0, ST = L / R1;
+                #pragma unroll(SG ? 2 : 1)
                 for (int it = tid; it < NC * (H / R1); it += NT) {
                     const int ql = it % NC, g = it / NC;
                     const int blk = g / ST, b = g % ST;
@@ -1090,6 +1119,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
                 __syncthreads();
             }
+            #pragma unroll(SG ? 2 : 1)
             for (int it = tid; it < NC * (H / R0); it += NT) {
                 const int ql = it % NC, g = it / NC;
                 constexpr int ST = H / R0;

@@ -3,10 +3,14 @@ every mode (batched, single-frame cluster variant, Eq. (9) update, Eq. (8) accum
 cc_track_host) and checked for what must hold by construction -- integer circular shifts of the reference come back
 exactly (periodic boundaries) and two runs give identical bits.
 
-    python -m paper_2310_08770_b200.selftest [--only f256] [--upsample 8] [--no-session]
+    python -m paper_2310_08770_b200.selftest [--only f256] [--upsample 8] [--no-session] [--dump out.npz]
+    python -m paper_2310_08770_b200.selftest --compare a.npz b.npz
 
-It is the target of the compute-sanitizer runs recorded under profiles/ (memcheck / racecheck / synccheck need a
-program that touches every variant with little work per launch).
+Race check without compute-sanitizer (closed on the development pool; profiles/sanitizer_r2.md): `--dump` also runs a
+batch of NOISY frames per shape (near-ties and rounding-level differences make the results sensitive to any change in
+the data the kernel reads) and stores every output; the dump of the plain library must equal, bit for bit, the dumps
+of repeated runs of the schedule-fuzzing build (CC_B200_LIB=.../libcc_b200_fuzz.so, build.py --fuzz: random delays
+before every synchronisation point).
 """
 from __future__ import annotations
 
@@ -26,7 +30,7 @@ def _shapes():
     return seen
 
 
-def run(only: str = "", upsample: int = 8, session: bool = True, verbose: bool = True) -> int:
+def run(only: str = "", upsample: int = 8, session: bool = True, verbose: bool = True, dump: dict | None = None) -> int:
     import torch
     from . import Plan, RtSession
     n_checked = 0
@@ -77,6 +81,19 @@ def run(only: str = "", upsample: int = 8, session: bool = True, verbose: bool =
                     assert (x, y) == (want_x[i], want_y[i]), name + ": session shift wrong"
             finally:
                 rt.close()
+        if dump is not None:  # noisy frames, every mode: the outputs go into the dump
+            noisy = np.clip(np.stack([np.roll(ref, sft, axis=(0, 1)).astype(np.int64) for sft in shifts * 3])
+                            + rng.integers(-hi // 8, hi // 8, size=(12, H, W)), 0, np.iinfo(dt).max).astype(dt)
+            dn = plan.device_frames(noisy)
+            bign = plan.device_frames(np.concatenate([noisy] * (reps + 1)))
+            dump[name + ".batched"] = np.stack([t.cpu().numpy() for t in plan.track(bign)])
+            dump[name + ".single"] = np.array([[t.item() for t in plan.track(dn[i], 1)] for i in range(len(noisy))], np.float32)
+            dump[name + ".accumulate"] = np.stack([t.cpu().numpy() for t in plan.track_accumulate(dn)])
+            plan.update_reference_from_accumulator()
+            plan.enable_reference_update(0.1)
+            dump[name + ".running"] = np.stack([t.cpu().numpy() for t in plan.track(dn)])
+            dump[name + ".spectrum"] = plan.reference_spectrum()
+            plan.enable_reference_update(0.0)
         plan.close()
         n_checked += 1
         if verbose:
@@ -103,8 +120,19 @@ def main(argv=None):
     ap.add_argument("--only", default="", help="substring of the shape name, e.g. f256x256_uint16")
     ap.add_argument("--upsample", type=int, default=8)
     ap.add_argument("--no-session", action="store_true", help="skip the resident real-time session kernel")
+    ap.add_argument("--dump", default="", help="also run noisy frames in every mode and store all outputs in this .npz")
+    ap.add_argument("--compare", nargs=2, default=None, help="compare two dumps bit for bit and exit")
     args = ap.parse_args(argv)
-    run(args.only, args.upsample, not args.no_session)
+    if args.compare:
+        a, b = np.load(args.compare[0]), np.load(args.compare[1])
+        assert sorted(a.files) == sorted(b.files), "different sets of outputs"
+        bad = [k for k in a.files if not np.array_equal(a[k], b[k], equal_nan=True)]
+        print("%d arrays compared, %d differ%s" % (len(a.files), len(bad), (": " + ", ".join(bad)) if bad else ""))
+        sys.exit(1 if bad else 0)
+    dump = {} if args.dump else None
+    run(args.only, args.upsample, not args.no_session, dump=dump)
+    if args.dump:
+        np.savez(args.dump, **dump)
 
 
 if __name__ == "__main__":

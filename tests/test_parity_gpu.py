@@ -901,3 +901,31 @@ def test_ccsn_offline_passes(gpu, oracle_mod, ci, n, u, eps):
     ndiff = _closed_loop_compare(o, outs[0][0], outs[0][1], u, "CC-SN Eq. (8) closed loop %s" % cfg.name)
     scale = np.max(np.abs(G[1:, 1:]))
     assert np.max(np.abs(outs[0][2] - _half(G))[:, 1:]) < 1e-9 * scale + 3e-2 * scale * ndiff / (u * n)
+
+
+# ---------------------------------------------------------------- tensor-core experiment for a6 (include/cc_bench.h: cc_tc_gemm_probe)
+def test_tensor_core_probe_numerics(gpu):
+    """tcgen05.mma kind::tf32 with the accumulator in tensor memory: small-integer operands give the exact product (the
+    UMMA shared-memory layouts and descriptors address every element once); on stage-1-like operands (Dirichlet
+    weights x smooth data) one TF32 pass is ~1e-3 of the result's scale, the three-pass hi/lo split ~1e-6, i.e. FP32
+    level -- the numbers behind DESIGN.md section 9.  Not used by cc_track."""
+    rng = np.random.default_rng(17)
+    A = rng.integers(-8, 9, size=(128, 192)).astype(np.float32)
+    B = rng.integers(-8, 9, size=(192, 128)).astype(np.float32)
+    for passes in (1, 3):
+        D, sc, mc = gpu.tc_gemm_probe(A, B, passes=passes, iters=2)
+        assert np.array_equal(D, A @ B) and mc > 0
+    H, u = 256, 100
+    j = np.arange(192, dtype=np.float64)[None, :]
+    d = np.arange(128, dtype=np.float64)[:, None]
+    t = d / u - j
+    with np.errstate(divide="ignore", invalid="ignore"):
+        dirich = np.where(np.abs(np.sin(np.pi * t / H)) < 1e-12, 1.0, np.sin(np.pi * t) / (H * np.tan(np.pi * t / H)))
+    A = np.where(j < 129, dirich, 0.0).astype(np.float32)
+    B = (np.exp(-((np.arange(192)[:, None] - 20.0) / 9.0) ** 2) * (1.0 + 0.3 * rng.standard_normal((192, 128)))).astype(np.float32)
+    ref = A.astype(np.float64) @ B.astype(np.float64)
+    scale = np.abs(ref).max()
+    e1 = np.abs(gpu.tc_gemm_probe(A, B, passes=1, iters=2)[0] - ref).max() / scale
+    e3 = np.abs(gpu.tc_gemm_probe(A, B, passes=3, iters=2)[0] - ref).max() / scale
+    print("tensor-core probe: 1 x TF32 error %.2e, 3 x TF32 error %.2e of the result's scale" % (e1, e3))
+    assert 1e-5 < e1 < 1e-2 and e3 < 1e-5
