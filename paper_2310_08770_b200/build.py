@@ -20,7 +20,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 _CCV = re.compile(r"^CCV\(([^)]*)\)", re.M)
-_KEYS = ["NAME", "H", "W", "CS", "PIX", "NT", "TM1", "TN1", "TM2", "TN2", "SG", "BK1", "G2", "R2", "KS2", "NSTG", "PFD", "KS1"]
+_KEYS = ["NAME", "H", "W", "CS", "PIX", "NT", "TM1", "TN1", "TM2", "TN2", "SG", "BK1", "G2", "R2", "KS2", "NSTG", "PFD", "KS1", "TC"]
 
 
 def variants():

@@ -22,13 +22,13 @@
 #include "cc_refupdate.h"
 
 // ------------------------------------------------------------------ variants
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1) CcVariant cc_variant_##name();
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1, TC) CcVariant cc_variant_##name();
 #include "cc_variant_list.h"
 #undef CCV
 
 typedef CcVariant (*cc_variant_fn)();
 static const cc_variant_fn g_variant_fns[] = {
-#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1) &cc_variant_##name,
+#define CCV(name, H, W, CS, PIX, NT, TM1, TN1, TM2, TN2, SG, BK1, G2, R2, KS2, NSTG, PFD, KS1, TC) &cc_variant_##name,
 #include "cc_variant_list.h"
 #undef CCV
 };
@@ -59,6 +59,8 @@ struct VarPlan {
     int DS = 0, nsb = 0, DSBp = 0, nch1 = 0, KT1 = 0, nrc2 = 0, nnc2 = 0, KT2 = 0;
     int ntiles_frame = 0, tile_floats = 0, u_bytes = 0;
     int pol_smem = 0;           // latency variants: fp64 polish tables resident in shared memory
+    int N1 = 0, KS1T = 0;       // tensor-core stage 1: MMA N (offsets per super-block, multiple of 16), 8-row k-steps
+    float *eblob = nullptr;     // tensor-core stage 1: operand tiles in UMMA layout
     float *blob = nullptr;      // device: staged operand tiles
     uint32_t *sched = nullptr;  // device: per-frame tile order
     uint32_t sched_head[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -173,7 +175,7 @@ static bool plan_variant(VarPlan &vp, int M, int W, int H)
     const int NC = W / 2 / v.CS;
     const int nd = M / 2 + 1;  // offsets d = 0..c (and e = 0..c)
     const int MC1 = v.R1 * v.TM1;
-    const int T1F = v.BK1 * MC1, T2F = v.G2 * v.Cn2 * (16 + 4 * (v.TN2 - 4));
+    const int T1F = v.tc1 ? 0 : v.BK1 * MC1, T2F = v.G2 * v.Cn2 * (16 + 4 * (v.TN2 - 4));
     vp.tile_floats = std::max(T1F, T2F);
     const int NSL = std::max(1, v.NT / NC);
     const int polish = 3 * H * 8 + 3 * NSL * NC * 16 + 3 * NC * 16 + 9 * NC * 8;
@@ -182,7 +184,8 @@ static bool plan_variant(VarPlan &vp, int M, int W, int H)
     const long avail = (long)SMEM_LIMIT - (long)v.fixed_smem() - 32;
     if (avail < lower) return false;
     const int LDT = W + 4;
-    const int ds_cap = (int)((avail - red_bytes) / ((long)LDT * 4)) / 2;
+    int ds_cap = (int)((avail - red_bytes) / ((long)LDT * 4)) / 2;
+    if (v.tc1) ds_cap = std::min(ds_cap, 128 / v.CS);  // four accumulator blocks of N1 <= 128 columns in the 512 columns of tensor memory
     if (ds_cap < 1) return false;
     int nsb = 1, DS;
     for (;; ++nsb) {
@@ -198,8 +201,13 @@ static bool plan_variant(VarPlan &vp, int M, int W, int H)
     vp.nrc2 = (2 * DS + v.R2 * v.TM2 - 1) / (v.R2 * v.TM2);
     vp.nnc2 = (nd + v.Cn2 * v.TN2 - 1) / (v.Cn2 * v.TN2);
     vp.KT2 = W / (4 * v.G2);
-    vp.ntiles_frame = vp.nsb * (vp.nch1 * vp.KT1 + vp.nrc2 * vp.nnc2 * vp.KT2);
+    vp.ntiles_frame = vp.nsb * ((v.tc1 ? 0 : vp.nch1 * vp.KT1) + vp.nrc2 * vp.nnc2 * vp.KT2);
     vp.u_bytes = round_up(std::max(lower, 2 * DS * LDT * 4 + red_bytes), 16);
+    if (v.tc1) {  // staging double buffer (2 x 4 x 4 KB) + 4 operand-ring slots of 4 tables [N1][8] floats, inside the U region
+        vp.N1 = round_up(DS * v.CS, 16);
+        vp.KS1T = (H / 2 + 1 + 7) / 8;
+        vp.u_bytes = std::max(vp.u_bytes, 32768 + 4 * 4 * vp.N1 * 32);
+    }
     vp.smem_bytes = (int)v.fixed_smem() + vp.u_bytes + 32;
     if (vp.smem_bytes > SMEM_LIMIT) return false;
     // latency variants: keep the fp64 polish tables in shared memory when they fit (two L2 round trips less per frame)
@@ -259,7 +267,7 @@ static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *
     const CcVariant &v = vp.v;
     const int c = M / 2, nd = c + 1;
     const int TF = vp.tile_floats, MC1 = v.R1 * v.TM1, DSB = vp.DS * v.CS;
-    const int n1 = vp.nsb * vp.nch1 * vp.KT1, n2 = vp.nnc2 * vp.KT2;
+    const int n1 = v.tc1 ? 0 : vp.nsb * vp.nch1 * vp.KT1, n2 = vp.nnc2 * vp.KT2;
     std::vector<float> blob((size_t)(n1 + n2) * TF, 0.f);
     // position inside a staged k-row -> logical [U|V] column of the chunk (cc_tm1_* chunk layout)
     std::vector<int> col_of_pos(MC1);
@@ -268,7 +276,7 @@ static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *
             const int w = cc_tm1_width(v.TM1, ci), st = cc_tm1_start(v.TM1, ci);
             for (int i = 0; i < w; ++i) col_of_pos[v.R1 * st + tm1 * w + i] = tm1 * v.TM1 + st + i;
         }
-    for (int sb = 0; sb < vp.nsb; ++sb)
+    for (int sb = 0; sb < vp.nsb && !v.tc1; ++sb)
         for (int ch = 0; ch < vp.nch1; ++ch)
             for (int kt = 0; kt < vp.KT1; ++kt) {
                 float *tile = blob.data() + (size_t)((sb * vp.nch1 + ch) * vp.KT1 + kt) * TF;
@@ -317,9 +325,46 @@ static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *
                             tile[g * GF2 + 16 * v.Cn2 + tn * 4 + kk] = val2(k, nc2 * NCOL2 + 4 * v.Cn2 + tn);
                 }
         }
+    // tensor-core stage 1: per (super-block, 8-row k-step) four tables [N1][8] -- even weights hi / lo, odd weights hi / lo
+    // (x = hi + lo: hi = the float with its low 13 mantissa bits cleared, lo = the rest of the float64 value, likewise
+    // truncated to TF32) -- in the K-major core-matrix layout of the UMMA descriptors: element (d, k) of a table at float
+    // (d / 8) * 64 + (k / 4) * 32 + (d % 8) * 4 + (k % 4)
+    std::vector<float> eblob;
+    if (v.tc1) {
+        const int N1 = vp.N1, KS = vp.KS1T;
+        auto hi13 = [](float x) {
+            uint32_t b;
+            memcpy(&b, &x, 4);
+            b &= 0xffffe000u;
+            memcpy(&x, &b, 4);
+            return x;
+        };
+        eblob.assign((size_t)vp.nsb * KS * 4 * N1 * 8, 0.f);
+        for (int sb = 0; sb < vp.nsb; ++sb)
+            for (int ks = 0; ks < KS; ++ks) {
+                float *tile = eblob.data() + ((size_t)sb * KS + ks) * 4 * N1 * 8;
+                for (int dsb = 0; dsb < N1; ++dsb)
+                    for (int k = 0; k < 8; ++k) {
+                        const int j = ks * 8 + k, d = sb * DSB + dsb;
+                        if (j > H / 2 || dsb >= DSB || d >= nd) continue;
+                        double we, wo;
+                        if (j == 0 || j == H / 2) {
+                            we = dirichlet_host((long long)d - (long long)j * u, u, H), wo = 0.0;
+                        } else {
+                            const double dm = dirichlet_host((long long)d - (long long)j * u, u, H);
+                            const double dp = dirichlet_host((long long)d + (long long)j * u, u, H);
+                            we = 0.5 * (dm + dp), wo = 0.5 * (dm - dp);
+                        }
+                        const size_t off = (size_t)(dsb / 8) * 64 + (k / 4) * 32 + (dsb % 8) * 4 + (k % 4);
+                        const float eh = hi13((float)we), oh = hi13((float)wo);
+                        tile[off] = eh, tile[(size_t)N1 * 8 + off] = hi13((float)(we - (double)eh));
+                        tile[(size_t)2 * N1 * 8 + off] = oh, tile[(size_t)3 * N1 * 8 + off] = hi13((float)(wo - (double)oh));
+                    }
+            }
+    }
     std::vector<uint32_t> sched;
     for (int sb = 0; sb < vp.nsb; ++sb) {
-        for (int ch = 0; ch < vp.nch1; ++ch)
+        for (int ch = 0; ch < vp.nch1 && !v.tc1; ++ch)
             for (int kt = 0; kt < vp.KT1; ++kt) sched.push_back((uint32_t)((sb * vp.nch1 + ch) * vp.KT1 + kt));
         for (int rc = 0; rc < vp.nrc2; ++rc)
             for (int nc2 = 0; nc2 < vp.nnc2; ++nc2)
@@ -332,6 +377,7 @@ static cudaError_t build_tiles(VarPlan &vp, int H, int W, int u, int M, size_t *
     }
     for (int i = 0; i < 8; ++i) vp.sched_head[i] = sched.empty() ? 0u : sched[(size_t)i % sched.size()];
     cudaError_t e = upload(&vp.blob, blob, acc);
+    if (e == cudaSuccess && v.tc1) e = upload(&vp.eblob, eblob, acc);
     if (e == cudaSuccess) e = upload(&vp.sched, sched, acc);
     if (e == cudaSuccess) e = upload(&vp.nyqc, nyq, acc);
     return e;
@@ -387,7 +433,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
     cc_sn_state_destroy(plan->sn_state);
     for (VarPlan *vp : {&plan->thr, &plan->lat})
-        cudaFree(vp->Sg), cudaFree(vp->Sg_alt), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc), cudaFree(vp->XpolR);
+        cudaFree(vp->Sg), cudaFree(vp->Sg_alt), cudaFree(vp->blob), cudaFree(vp->sched), cudaFree(vp->nyqc), cudaFree(vp->XpolR), cudaFree(vp->eblob);
     for (int i = 0; i < 2; ++i) {
         if (plan->hs[i]) cudaStreamDestroy(plan->hs[i]);
         if (plan->hev[i]) cudaEventDestroy(plan->hev[i]);
@@ -587,7 +633,7 @@ extern "C" cc_status cc_plan_create_weighted(cc_plan **out, int H, int W, cc_dty
 static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
 {
     p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
-    p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg;
+    p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg, p.eblob = vp.eblob, p.N1 = vp.N1;
     for (int i = 0; i < 8; ++i) p.sched_head[i] = vp.sched_head[i];
     p.tw64 = pl->tw64, p.Dpol = pl->Dpol, p.Xpol = pl->Xpol, p.nyq64 = pl->nyq64, p.XpolR = vp.XpolR;
     p.u = pl->u, p.M = pl->M, p.c = pl->c, p.nd = pl->c + 1;

@@ -82,6 +82,9 @@ struct CcParams {
     const uint16_t *col_partner;  // [H]: slot of -ky for the frequency at slot p
     const float *blob;            // staged GEMM operand tiles (stage-1 even/odd Dirichlet tiles, stage-2 cos/sin tiles),
                                   // tile t at blob + t * tile_floats
+    const float *eblob;           // TC variants: stage-1 operand tiles in UMMA layout, tile (sb, ks) at eblob + (sb * KS + ks) * 128 * N1:
+                                  //   four tables [N1][8] (Ee_hi, Ee_lo, Eo_hi, Eo_lo), K-major 8-row x 16-byte core matrices
+    int N1;                       // TC variants: offsets per super-block rounded up to a multiple of 16 (MMA N)
     const uint32_t *sched;        // [ntiles_frame] blob tile index of the i-th tile a frame consumes
     uint32_t sched_head[8];       // sched[i % ntiles_frame], i < 8: the initial burst of the operand ring
     const float *nyqc;            // [ne_pad] cos(pi e / u): Nyquist-column weight of stage 2
@@ -145,6 +148,7 @@ struct CcVariant {
     int s_global;  // 1: spectrum array lives in global memory (L2), 0: shared memory / DSMEM
     int NSTG;
     int lat;       // 1: small-batch (latency) variant
+    int tc1;       // 1: stage 1 on the tensor cores
     size_t (*fixed_smem)();                 // bytes that do not depend on M (S, tables, misc), before U/stg
     int (*raw_scratch_bytes)();             // raw ring + FFT scratch (lower bound of the U region)
     cudaError_t (*prepare)(int smem_bytes);  // sets func attributes

@@ -112,6 +112,34 @@ __device__ __forceinline__ uint64_t globaltimer_ns()
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
+// ---- 5th-generation tensor cores (tcgen05): shared-memory matrix descriptor (no swizzle, K-major: 8-row x 16-byte core
+// matrices; lbo = byte distance of the two 16-byte K chunks, sbo = byte distance of successive 8-row groups; version 1)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) | ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) |
+           (1ull << 46);
+}
+// D[tmem] (+)= A[smem] B[smem]^T, A: 128 x 8, B: N x 8, TF32 operands, FP32 accumulator; issued by ONE thread
+__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar)  // the mbarrier completes when every MMA issued so far has
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8])  // 32 lanes x 8 columns, lane = thread
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+
 // packed FP32 pairs (Blackwell FFMA2: two fused multiply-adds per instruction, each IEEE-rounded like fmaf)
 __device__ __forceinline__ unsigned long long pack2(float x, float y)
 {
@@ -394,10 +422,12 @@ __device__ __forceinline__ Best warp_best(Best b)
 
 // ------------------------------------------------------------------ the kernel
 template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, int TM2_, int TN2_, bool SG_, int BK1_, int G2_,
-          int R2_, int KS2_, int NSTG_, int PFD_, int KS1_>
+          int R2_, int KS2_, int NSTG_, int PFD_, int KS1_, int TC_ = 0>
 struct Cfg {
+    static constexpr bool TC1 = TC_ != 0;       // stage 1 of the upsampled DFT on the tensor cores (tcgen05, 3 x TF32)
     static constexpr int NSTG = NSTG_;  // staging ring depth
-    static constexpr int NBARS = NSTG + 7;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish tables [1]
+    static constexpr int NBARS = NSTG + 13;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish
+                                             // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -426,7 +456,7 @@ struct Cfg {
     static constexpr int WR1 = 32 / WC1;
     static constexpr int WG1C = Cn1 / WC1;
     static constexpr int MC1 = R1 * TM1;          // [U|V] columns per stage-1 chunk
-    static constexpr int T1F = BK1 * MC1;         // floats of a stage-1 tile
+    static constexpr int T1F = TC1 ? 0 : BK1 * MC1;  // floats of a stage-1 tile (TC1: stage-1 operands have their own ring)
     // stage 2: thread grid R2 x Cn2 x KS2 (k-split); a warp covers WR2 x WC2 threads of one k-slice
     static constexpr int Cn2 = NT / (R2 * KS2);
     static constexpr int WC2 = Cn2 < 8 ? Cn2 : 8;
@@ -443,7 +473,7 @@ struct Cfg {
     static constexpr int RED_FLOATS = RED1_FLOATS > RED2_FLOATS ? RED1_FLOATS : RED2_FLOATS;
     static constexpr int LDT = W + 4;  // row stride (floats) of the T buffer
     static constexpr size_t S_BYTES = SG ? 0 : (size_t)H * NC * 8;
-    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN) + 16 * NWARP + 64 + 16 + 4 * NSTG;
+    static constexpr size_t MISC_BYTES = 8 * NBARS + 8 * (2 * CS * XN) + 16 * NWARP + 64 + 16 + 4 * NSTG + 16;
     static constexpr size_t FIXED_BYTES =
         S_BYTES + (size_t)NSTG * TILEF * 4 + (size_t)NTW * 8 + (size_t)W * 2 + MISC_BYTES + (LAT ? (size_t)W * 16 + 16 : 0);
     static_assert(NC >= 1 && NR >= 2 && (NR % 2) == 0, "bad split");
@@ -456,6 +486,7 @@ struct Cfg {
     static_assert(TILEF % 4 == 0 && MC1 % 4 == 0, "tile alignment");
     static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
     static_assert(NSTG <= 8, "ring (sched_head carries 8 entries)");
+    static_assert(!TC1 || (2 * NC == 128 && NT == 256 && !SG), "tensor-core stage 1: 128 spectrum floats per CTA (MMA M = 128), 8 warps");
 };
 
 template <class C>
@@ -517,12 +548,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
     uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
     uint64_t *const tbar = cbar + 1, *const pbar = tbar + 1;
+    uint64_t *const ebar = pbar + 1, *const mdone = ebar + 4;            // tensor-core stage 1: operand ring, MMA completion
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     float *const wv = reinterpret_cast<float *>(xchg + 2 * CS * XN);    // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
     float *const f00 = reinterpret_cast<float *>(wi + NWARP);          // [1]
     uint64_t *const cmdslot = reinterpret_cast<uint64_t *>(((uintptr_t)(f00 + 1) + 7) & ~(uintptr_t)7);  // [2] rt command (seq, frame)
     uint32_t *const relcnt = reinterpret_cast<uint32_t *>(cmdslot + 2);  // [NSTG] releases of each ring slot (mod NWARP)
+    uint32_t *const tmem_slot = relcnt + NSTG;                           // [1] base address of the tensor-memory allocation
 
     float2 *const scr = reinterpret_cast<float2 *>(U + C::RAWB) + (warp * RG + gp) * PADW;
     float *const Tb = reinterpret_cast<float *>(U);
@@ -598,7 +631,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     // mbarriers of all CTAs visible is split: arrive here, wait just before the first remote access (after the first
     // raw chunk has landed), so neither the table latency nor the barrier latency is exposed.
     const double2 *tw64 = p.tw64;  // (cos, sin)(2 pi j / W) in fp64; the latency variants keep a copy in shared memory
-    double2 *const t64s = reinterpret_cast<double2 *>(((uintptr_t)(relcnt + NSTG) + 15) & ~(uintptr_t)15);   // [W] (LAT)
+    double2 *const t64s = reinterpret_cast<double2 *>(((uintptr_t)(relcnt + NSTG + 4) + 15) & ~(uintptr_t)15);   // [W] (LAT)
     // resident polish tables (p.pol_smem): Dpol [M][H], this CTA's columns of Xpol [M][NC], nyq64 [M rounded up to even]
     double *const DpolS = reinterpret_cast<double *>(t64s + (C::LAT ? W : 0));
     double2 *const XpolS = reinterpret_cast<double2 *>(DpolS + (size_t)p.M * H);
@@ -609,6 +642,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
         mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1), mbar_init(cbar, 1);
         mbar_init(tbar, 1), mbar_init(pbar, 1);
+        for (int i = 0; i < 4; ++i) mbar_init(&ebar[i], 1);
+        mbar_init(&mdone[0], 2), mbar_init(&mdone[1], 2);  // the two MMA-issuing threads commit
         fence_mbar_init();
         if (!p.rt_cmd && cid < p.batch && !direct_first) issue_raw_head(p.frames, cid);
     }
@@ -621,7 +656,20 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             if (tid + e * NT < W) t64s[tid + e * NT] = r_64[e];
     }
     if constexpr (C::LAT) tw64 = t64s;
+    if constexpr (C::TC1) {  // all 512 columns of tensor memory (one CTA per SM): accumulators U and V of stage 1
+        if (warp == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
     __syncthreads();  // the mbarrier inits are visible to every thread of the CTA
+    uint32_t tmem = 0, mph[2] = {0u, 0u}, e_issued = 0u, e_cons = 0u;  // TC1: tensor-memory base, completed waits on mdone[],
+                                                                        // stage-1 operand tiles requested / consumed (thread 0)
+    if constexpr (C::TC1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tmem = *tmem_slot;
+    }
     // the copies nobody waits for yet are issued by other warps, beside the first phase: the operand ring ...
     if (tid == 32 && total_tiles > 0) {  // the first schedule entries ride in the kernel parameters: no load latency
 #pragma unroll
@@ -1243,6 +1291,136 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             float *const red = Tb + (size_t)2 * DS * LDT;  // k-split partial sums (KS1 > 1, KS2 > 1)
             for (int sb = 0; sb < p.nsb; ++sb) {
                 const int db = sb * DSB;
+                if constexpr (C::TC1) {
+                // ---------------- stage 1 on the tensor cores (tcgen05.mma kind::tf32, accumulators in tensor memory):
+                //   U[d][n] = sum_j Ee[d][j] S[(y0+j)][n],  V[d][n] = sum_j Eo[d][j] S[(y0-j)][n]   (n = my 128 spectrum floats;
+                //   the offsets d are the MMA's M = 128 rows = tensor-memory lanes, so a thread of the epilogue owns a row of T)
+                // per 8 rows j as 128 x N x 8 MMAs, each product split into TF32 passes (x = hi + lo, the low 13 mantissa
+                // bits split off exactly; lo*hi + hi*lo + hi*hi carries ~22 bits of both operands: FP32-level accuracy,
+                // profiles/r2a_tc_probe.json).  An MMA instruction costs its issuing thread ~75 cycles whatever N is, so
+                // the hi*hi and hi*lo passes are ONE instruction (B = [S_hi ; S_lo], N = 256, two accumulator halves
+                // that the epilogue adds) and U and V are issued by two different threads.  The weight tables hold only
+                // their N1 <= 128 used rows: the MMA reads 128, the rows beyond N1 produce lanes nobody reads.  The CTA's threads stage
+                // the data operand (8 rows of S -> K-major core matrices, hi and lo) into a double buffer while the MMAs
+                // of the previous 8 rows run; the plan-constant operand (Ee / Eo, hi / lo, already in UMMA layout)
+                // arrives by TMA through a 4-slot ring.  Epilogue: tensor memory -> registers, T(c+-d) = U +- V,
+                // rotation by exp(2 pi i kx x0 / W), rows to their owners.
+                {
+                    constexpr int KSTEPS = (H / 2 + 1 + 7) / 8;
+                    const int N1 = p.N1;
+                    const uint32_t etab = (uint32_t)N1 * 32u, etile = 4u * etab;   // bytes of one table / one operand tile
+                    unsigned char *const abuf = U;                                   // [2][4][4096]: U_hi, U_lo, V_hi, V_lo
+                    unsigned char *const ering = U + 32768;                          // [4][etile]: Ee_hi, Ee_lo, Eo_hi, Eo_lo
+                    const uint32_t idescA = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(256 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+                    const uint32_t idescB = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(128 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+                    const float *Sf = reinterpret_cast<const float *>(Sl);
+                    auto issue_etile = [&](int ks) {  // thread 0
+                        const uint32_t slot = e_issued & 3u;
+                        mbar_expect_tx(&ebar[slot], etile);
+                        bulk_g2s(ering + (size_t)slot * etile, p.eblob + ((size_t)sb * KSTEPS + ks) * (size_t)(etile / 4), etile, &ebar[slot]);
+                        ++e_issued;
+                    };
+                    if (tid == 0) {
+                        fence_proxy_async();  // U was written by generic stores (polish scratch) before
+                        for (int ks = 0; ks < 4 && ks < KSTEPS; ++ks) issue_etile(ks);
+                    }
+                    for (int ks = 0; ks < KSTEPS; ++ks) {
+                        const int b = ks & 1;
+                        if (ks >= 2) {  // the MMAs of step ks-2 are complete: their staging buffer and ring slot are free
+                            mbar_wait(&mdone[b], mph[b] & 1u);
+                            ++mph[b];
+                            if (tid == 0 && ks + 2 < KSTEPS) issue_etile(ks + 2);
+                        }
+                        {   // stage rows j = 8 ks .. 8 ks + 7: thread (n, kh) handles spectrum float n, rows 4 kh .. 4 kh + 3
+                            const int n = tid & 127, kh = tid >> 7;
+                            float up[4], vm[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const int j = ks * 8 + kh * 4 + i;   // rows beyond H/2 meet zero weights
+                                up[i] = Sf[(size_t)((y0 + j) & (H - 1)) * (2 * NC) + n];
+                                vm[i] = Sf[(size_t)((y0 - j) & (H - 1)) * (2 * NC) + n];
+                            }
+                            const float4 uh = make_float4(tf32_hi(up[0]), tf32_hi(up[1]), tf32_hi(up[2]), tf32_hi(up[3]));
+                            const float4 vh = make_float4(tf32_hi(vm[0]), tf32_hi(vm[1]), tf32_hi(vm[2]), tf32_hi(vm[3]));
+                            const float4 ul = make_float4(tf32_hi(up[0] - uh.x), tf32_hi(up[1] - uh.y), tf32_hi(up[2] - uh.z), tf32_hi(up[3] - uh.w));
+                            const float4 vl = make_float4(tf32_hi(vm[0] - vh.x), tf32_hi(vm[1] - vh.y), tf32_hi(vm[2] - vh.z), tf32_hi(vm[3] - vh.w));
+                            unsigned char *dst = abuf + (size_t)b * 16384 + (n >> 3) * 256 + kh * 128 + (n & 7) * 16;
+                            *reinterpret_cast<float4 *>(dst) = uh;
+                            *reinterpret_cast<float4 *>(dst + 4096) = ul;
+                            *reinterpret_cast<float4 *>(dst + 8192) = vh;
+                            *reinterpret_cast<float4 *>(dst + 12288) = vl;
+                        }
+                        fence_proxy_async();  // generic-proxy stores -> visible to the tensor core
+                        __syncthreads();
+                        if (tid == 0 || tid == 32) {  // thread 0 issues the MMAs of U, thread 32 those of V
+                            const uint32_t isV = tid == 32 ? 1u : 0u;
+                            mbar_wait(&ebar[e_cons & 3u], (e_cons >> 2) & 1u);
+                            const uint32_t eb = smem_u32(ering + (size_t)(e_cons & 3u) * etile) + isV * 2u * etab;
+                            const uint32_t ab = smem_u32(abuf + (size_t)b * 16384) + isV * 8192u;
+                            ++e_cons;
+                            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                            const uint32_t acc = ks > 0 ? 1u : 0u, d0 = tmem + isV * 256u;
+                            // [D1 | D2] (+)= E_hi [S_hi ; S_lo]^T ;  D2 += E_lo S_hi^T ;  result = D1 + D2
+                            umma_tf32(d0, umma_desc(eb, 128, 256), umma_desc(ab, 128, 256), idescA, acc);
+                            umma_tf32(d0 + 128u, umma_desc(eb + etab, 128, 256), umma_desc(ab, 128, 256), idescB, 1u);
+                            umma_commit(&mdone[b]);
+                        }
+                    }
+#pragma unroll
+                    for (int t = (KSTEPS >= 2 ? KSTEPS - 2 : 0); t < KSTEPS; ++t) {  // the last two steps complete
+                        mbar_wait(&mdone[t & 1], mph[t & 1] & 1u);
+                        ++mph[t & 1];
+                    }
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    csync();  // no CTA of the cluster stages operands in its U region any more: T rows may land there
+                    {   // thread = (offset d = lane of tensor memory, half of the 128 spectrum floats): a row segment of T
+                        const int lb = 32 * (warp & 3), dsb = lb + lane, half = warp >> 2;
+                        const bool live = dsb < DSB && db + dsb < nd;
+                        const int dr = dsb / DS, row = dsb % DS;
+                        float *Td = Tb;
+                        if constexpr (CS > 1) Td = cluster.map_shared_rank(Tb, live ? dr : rank);
+                        float *const dstp = Td + (size_t)row * LDT + rank * 2 * NC, *const dstm = dstp + (size_t)DS * LDT;
+                        const float sg = (x0 & 1) ? -1.f : 1.f;
+                        const uint32_t tb = tmem + ((uint32_t)lb << 16);
+#pragma unroll 1
+                        for (int c0 = half * 64; c0 < half * 64 + 64; c0 += 16) {  // 16 spectrum floats per round trip
+                            uint32_t r[4][2][8];
+#pragma unroll
+                            for (int a4 = 0; a4 < 4; ++a4)
+#pragma unroll
+                                for (int g = 0; g < 2; ++g) tmem_ld8(tb + (uint32_t)(a4 * 128 + c0 + 8 * g), r[a4][g]);
+                            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                            float op[16], om[16];
+#pragma unroll
+                            for (int i = 0; i < 16; i += 2) {
+                                const int g = i >> 3, k = i & 7;
+                                const float ur = __uint_as_float(r[0][g][k]) + __uint_as_float(r[1][g][k]);
+                                const float ui = __uint_as_float(r[0][g][k + 1]) + __uint_as_float(r[1][g][k + 1]);
+                                const float vr = __uint_as_float(r[2][g][k]) + __uint_as_float(r[3][g][k]);
+                                const float vi = __uint_as_float(r[2][g][k + 1]) + __uint_as_float(r[3][g][k + 1]);
+                                const float2 tp = make_float2(ur + vr, ui + vi), tm = make_float2(ur - vr, ui - vi);
+                                const int q = rank * NC + ((c0 + i) >> 1);
+                                if (q == 0) {  // packed column: (DC, Nyquist) -- the Nyquist part carries (-1)^x0
+                                    op[i] = tp.x, op[i + 1] = tp.y * sg, om[i] = tm.x, om[i + 1] = tm.y * sg;
+                                } else {
+                                    const float2 w = tw[((q * x0) & (W - 1)) * (NTW / W)];  // (cos, -sin)
+                                    const float2 a = cmulc(tp, w), bq = cmulc(tm, w);
+                                    op[i] = a.x, op[i + 1] = a.y, om[i] = bq.x, om[i + 1] = bq.y;
+                                }
+                            }
+                            if (live) {
+#pragma unroll
+                                for (int v = 0; v < 4; ++v) {
+                                    *reinterpret_cast<float4 *>(dstp + c0 + 4 * v) = make_float4(op[4 * v], op[4 * v + 1], op[4 * v + 2], op[4 * v + 3]);
+                                    *reinterpret_cast<float4 *>(dstm + c0 + 4 * v) = make_float4(om[4 * v], om[4 * v + 1], om[4 * v + 2], om[4 * v + 3]);
+                                }
+                            }
+                        }
+                    }
+                    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                    csync();  // T(c+d), T(c-d) rows are at their owners
+                }
+                } else {
                 // ---------------- stage 1: rows [U(d) | V(d)] of this super-block, my 2*NC spectrum floats
                 //   U(d) = sum_j Ee[d][j] S[(y0+j)],  V(d) = sum_j Eo[d][j] S[(y0-j)];  T(c+d) = U+V, T(c-d) = U-V
                 for (int ch = 0; ch < p.nch1; ++ch) {
@@ -1368,6 +1546,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     *pv = make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w);
                 }
                 __syncthreads();
+                }  // FP32 stage 1
                 stamp(4, f);
 
                 // ---------------- stage 2: E(m,e) = sum_q T_re w cos, O(m,e) = sum_q T_im w sin;
@@ -1632,6 +1811,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
     }
     csync();  // no CTA of the cluster exits while peers may still address its shared memory
+    if constexpr (C::TC1) {
+        if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
     if (RT && rank == 0 && tid == 0) {
         *reinterpret_cast<volatile int *>(p.rt_alive) = 0;  // the session kernel is gone (quit or idle timeout)
         __threadfence_system();
@@ -1688,6 +1870,7 @@ struct Launcher {
         v.s_global = C::SG ? 1 : 0;
         v.NSTG = C::NSTG;
         v.lat = C::LAT ? 1 : 0;
+        v.tc1 = C::TC1 ? 1 : 0;
         v.fixed_smem = &fixed_smem;
         v.raw_scratch_bytes = &raw_scratch_bytes;
         v.prepare = &prepare;

@@ -3,7 +3,7 @@
 #include "cc_fused.cuh"
 
 using VariantCfg = ccf::Cfg<CCV_H, CCV_W, CCV_CS, CCV_PIX, CCV_NT, CCV_TM1, CCV_TN1, CCV_TM2, CCV_TN2, CCV_SG, CCV_BK1, CCV_G2,
-                            CCV_R2, CCV_KS2, CCV_NSTG, CCV_PFD, CCV_KS1>;
+                            CCV_R2, CCV_KS2, CCV_NSTG, CCV_PFD, CCV_KS1, CCV_TC>;
 
 #define CCV_CAT2(a, b) a##b
 #define CCV_CAT(a, b) CCV_CAT2(a, b)
