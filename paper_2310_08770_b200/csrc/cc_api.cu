@@ -84,6 +84,7 @@ struct cc_plan {
     float4 *ab = nullptr;
     double2 *tw64 = nullptr, *Xpol = nullptr;  // fp64 tables of the argmax polish steps
     double *Dpol = nullptr, *nyq64 = nullptr;
+    double *DpolPlain = nullptr;  // Dirichlet rows for S holding the plain Q (tensor-core variants)
     // running reference image (Eq. (9)): scratch spectrum of the current frame, running mean, slot -> frequency table
     float2 *ri_Fs = nullptr;
     float4 *ri_Fab = nullptr;
@@ -428,7 +429,7 @@ extern "C" cc_status cc_plan_destroy(cc_plan *plan)
     if (!plan) return CC_OK;
     cudaFree(plan->tw), cudaFree(plan->Gt), cudaFree(plan->row_slot), cudaFree(plan->col_partner);
     cudaFree(plan->ab);
-    cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64);
+    cudaFree(plan->tw64), cudaFree(plan->Xpol), cudaFree(plan->Dpol), cudaFree(plan->nyq64), cudaFree(plan->DpolPlain);
     cudaFree(plan->ri_Fs), cudaFree(plan->ri_Fab), cudaFree(plan->ri_emean), cudaFree(plan->col_freq);
     cudaFree(plan->acc_G), cudaFree(plan->acc_ab), cudaFree(plan->acc_mean);
     cc_sn_state_destroy(plan->sn_state);
@@ -588,6 +589,12 @@ extern "C" cc_status cc_plan_create_weighted(cc_plan **out, int H, int W, cc_dty
             }
         }
         if (e == cudaSuccess) e = upload(&pl->Dpol, Dpol, &pl->table_bytes);
+        if (pl->thr.v.tc1 || (pl->has_lat && pl->lat.v.tc1)) {
+            std::vector<double> Dplain((size_t)M * H);
+            for (int m = 0; m < M; ++m)
+                for (int j = 0; j < H; ++j) Dplain[(size_t)m * H + j] = (double)dirichlet_l((long long)(m - c) - (long long)j * u, u, H);
+            if (e == cudaSuccess) e = upload(&pl->DpolPlain, Dplain, &pl->table_bytes);
+        }
         if (e == cudaSuccess) e = upload(&pl->Xpol, Xpol, &pl->table_bytes);
         if (e == cudaSuccess) e = upload(&pl->nyq64, nyq64, &pl->table_bytes);
         if (e == cudaSuccess) e = build_tiles(pl->thr, H, W, u, M, &pl->table_bytes);
@@ -635,7 +642,7 @@ static void fill_params(const cc_plan *pl, const VarPlan &vp, CcParams &p)
     p.tw = pl->tw, p.row_slot = pl->row_slot, p.Gt = pl->Gt, p.ab = pl->ab, p.col_partner = pl->col_partner;
     p.blob = vp.blob, p.sched = vp.sched, p.nyqc = vp.nyqc, p.Sg = vp.Sg, p.eblob = vp.eblob, p.N1 = vp.N1;
     for (int i = 0; i < 8; ++i) p.sched_head[i] = vp.sched_head[i];
-    p.tw64 = pl->tw64, p.Dpol = pl->Dpol, p.Xpol = pl->Xpol, p.nyq64 = pl->nyq64, p.XpolR = vp.XpolR;
+    p.tw64 = pl->tw64, p.Dpol = pl->Dpol, p.DpolPlain = pl->DpolPlain, p.Xpol = pl->Xpol, p.nyq64 = pl->nyq64, p.XpolR = vp.XpolR;
     p.u = pl->u, p.M = pl->M, p.c = pl->c, p.nd = pl->c + 1;
     p.DS = vp.DS, p.nsb = vp.nsb, p.DSBp = vp.DSBp, p.nch1 = vp.nch1, p.KT1 = vp.KT1, p.nrc2 = vp.nrc2, p.nnc2 = vp.nnc2;
     p.ntiles_frame = pl->u > 1 ? vp.ntiles_frame : 0, p.tile_floats = vp.tile_floats;

@@ -93,6 +93,8 @@ struct CcParams {
     const double2 *tw64;          // [W] (cos, sin)(2 pi j / W)
     const double *Dpol;           // [M][H] Dirichlet weights of grid row m for the physical rows (y0+j) mod H of the
                                   //        sum/difference layout: j = 0, H/2: D_H(t-j); 0 < j < H/2: even part; H-j: odd part
+    const double *DpolPlain;      // [M][H] the same weights for S holding the plain Q: D_H((m - c)/u - j) for row (y0+j) mod H
+                                  //        (tensor-core variants, which form the sums / differences while staging)
     const double2 *Xpol;          // [M][W/2] (cos, sin)(2 pi q (n - c) / (u W))
     const double *nyq64;          // [M] cos(pi (n - c) / u)
     const double2 *XpolR;         // latency variants with pol_smem: Xpol regrouped by cluster rank, [CS][M][NC], else null

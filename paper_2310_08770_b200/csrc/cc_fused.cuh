@@ -426,8 +426,8 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
 struct Cfg {
     static constexpr bool TC1 = TC_ != 0;       // stage 1 of the upsampled DFT on the tensor cores (tcgen05, 3 x TF32)
     static constexpr int NSTG = NSTG_;  // staging ring depth
-    static constexpr int NBARS = NSTG + 13;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish
-                                             // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2]
+    static constexpr int NBARS = NSTG + 15;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish
+                                             // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2], staged [2]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -548,7 +548,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
     uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
     uint64_t *const tbar = cbar + 1, *const pbar = tbar + 1;
-    uint64_t *const ebar = pbar + 1, *const mdone = ebar + 4;            // tensor-core stage 1: operand ring, MMA completion
+    uint64_t *const ebar = pbar + 1, *const mdone = ebar + 4, *const afull = mdone + 2;  // tensor-core stage 1: operand ring,
+                                                                                         // MMA completion, operands staged
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     float *const wv = reinterpret_cast<float *>(xchg + 2 * CS * XN);    // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
@@ -644,6 +645,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         mbar_init(tbar, 1), mbar_init(pbar, 1);
         for (int i = 0; i < 4; ++i) mbar_init(&ebar[i], 1);
         mbar_init(&mdone[0], 2), mbar_init(&mdone[1], 2);  // the two MMA-issuing threads commit
+        mbar_init(&afull[0], 128), mbar_init(&afull[1], 128);  // the four staging warps arrive
         fence_mbar_init();
         if (!p.rt_cmd && cid < p.batch && !direct_first) issue_raw_head(p.frames, cid);
     }
@@ -664,7 +666,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();  // the mbarrier inits are visible to every thread of the CTA
-    uint32_t tmem = 0, mph[2] = {0u, 0u}, e_issued = 0u, e_cons = 0u;  // TC1: tensor-memory base, completed waits on mdone[],
+    uint32_t tmem = 0, mph[2] = {0u, 0u}, aph[2] = {0u, 0u}, e_issued = 0u, e_cons = 0u;  // TC1: tensor-memory base, completed waits on mdone[],
                                                                         // stage-1 operand tiles requested / consumed (thread 0)
     if constexpr (C::TC1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -1220,6 +1222,21 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             y0 = g.i / W;
             x0 = g.i % W;
             stamp(2, f);
+            if constexpr (C::TC1) {
+                // the first four weight tiles of stage 1 go into their ring now (the FFT scratch they overwrite is dead; the
+                // fp64 polish below uses the first bytes of U only): their latency runs under the polish
+                if (tid == 0 && u > 1) {
+                    constexpr int KSTEPS = (H / 2 + 1 + 7) / 8;
+                    const uint32_t etile = 4u * (uint32_t)p.N1 * 32u;
+                    fence_proxy_async();
+                    for (int ks = 0; ks < 4 && ks < KSTEPS; ++ks) {
+                        const uint32_t slot = e_issued & 3u;
+                        mbar_expect_tx(&ebar[slot], etile);
+                        bulk_g2s(U + 32768 + (size_t)slot * etile, p.eblob + (size_t)ks * (size_t)(etile / 4), etile, &ebar[slot]);
+                        ++e_issued;
+                    }
+                }
+            }
 
             // fp64 re-evaluation of the 3x3 neighbourhood of the fp32 winner
             double *terms = reinterpret_cast<double *>(U);
@@ -1267,12 +1284,15 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         // =============================================================== a6/a7: upsampled DFT as two symmetric FP32 GEMMs
         // Row pairs about the integer peak become their sum and difference (in place):
         //   S[(y0+j)] <- Q(y0+j) + Q(y0-j),  S[(y0-j)] <- Q(y0+j) - Q(y0-j),  0 < j < H/2.
-        for (int idx = tid; idx < (H / 2 - 1) * NC; idx += NT) {
-            const int j = 1 + idx / NC, ql = idx % NC;
-            float2 *pa = Sl + (size_t)((y0 + j) & (H - 1)) * NC + ql, *pb = Sl + (size_t)((y0 - j) & (H - 1)) * NC + ql;
-            const float2 a = *pa, b = *pb;
-            *pa = make_float2(a.x + b.x, a.y + b.y);
-            *pb = make_float2(a.x - b.x, a.y - b.y);
+        // (tensor-core stage 1 forms the sums and differences while it stages its operand: S keeps the plain Q there)
+        if constexpr (!C::TC1) {
+            for (int idx = tid; idx < (H / 2 - 1) * NC; idx += NT) {
+                const int j = 1 + idx / NC, ql = idx % NC;
+                float2 *pa = Sl + (size_t)((y0 + j) & (H - 1)) * NC + ql, *pb = Sl + (size_t)((y0 - j) & (H - 1)) * NC + ql;
+                const float2 a = *pa, b = *pb;
+                *pa = make_float2(a.x + b.x, a.y + b.y);
+                *pb = make_float2(a.x - b.x, a.y - b.y);
+            }
         }
         __syncthreads();
 
@@ -1320,52 +1340,80 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         bulk_g2s(ering + (size_t)slot * etile, p.eblob + ((size_t)sb * KSTEPS + ks) * (size_t)(etile / 4), etile, &ebar[slot]);
                         ++e_issued;
                     };
-                    if (tid == 0) {
-                        fence_proxy_async();  // U was written by generic stores (polish scratch) before
+                    if (tid == 0 && sb > 0) {  // (super-block 0: requested right after the integer argmax)
+                        fence_proxy_async();
                         for (int ks = 0; ks < 4 && ks < KSTEPS; ++ks) issue_etile(ks);
                     }
-                    for (int ks = 0; ks < KSTEPS; ++ks) {
-                        const int b = ks & 1;
-                        if (ks >= 2) {  // the MMAs of step ks-2 are complete: their staging buffer and ring slot are free
-                            mbar_wait(&mdone[b], mph[b] & 1u);
-                            ++mph[b];
-                            if (tid == 0 && ks + 2 < KSTEPS) issue_etile(ks + 2);
-                        }
-                        {   // stage rows j = 8 ks .. 8 ks + 7: thread (n, kh) handles spectrum float n, rows 4 kh .. 4 kh + 3
-                            const int n = tid & 127, kh = tid >> 7;
-                            float up[4], vm[4];
+                    // Producer / consumer: warps 0-3 stage the data operand (thread n: spectrum float n, the 8 rows of the step,
+                    // sums and differences of the row pairs formed on the way: S keeps the plain Q) and arrive on afull[b];
+                    // lane 0 of warp 6 (U) and of warp 7 (V) wait for it, issue the MMAs and commit to mdone[b], which frees
+                    // buffer b two steps later.  No CTA barrier inside the loop.
+                    if (warp < 4) {  // thread n: spectrum float n, the 8 rows of the step (two 16-byte K chunks per table)
+                        const int sn = tid;
+                        for (int ks = 0; ks < KSTEPS; ++ks) {
+                            const int b = ks & 1;
+                            float qa[8], qb[8];
 #pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const int j = ks * 8 + kh * 4 + i;   // rows beyond H/2 meet zero weights
-                                up[i] = Sf[(size_t)((y0 + j) & (H - 1)) * (2 * NC) + n];
-                                vm[i] = Sf[(size_t)((y0 - j) & (H - 1)) * (2 * NC) + n];
+                            for (int i = 0; i < 8; ++i) {
+                                const int j = ks * 8 + i;   // rows beyond H/2 meet zero weights
+                                qa[i] = Sf[(size_t)((y0 + j) & (H - 1)) * (2 * NC) + sn];
+                                qb[i] = Sf[(size_t)((y0 - j) & (H - 1)) * (2 * NC) + sn];
                             }
-                            const float4 uh = make_float4(tf32_hi(up[0]), tf32_hi(up[1]), tf32_hi(up[2]), tf32_hi(up[3]));
-                            const float4 vh = make_float4(tf32_hi(vm[0]), tf32_hi(vm[1]), tf32_hi(vm[2]), tf32_hi(vm[3]));
-                            const float4 ul = make_float4(tf32_hi(up[0] - uh.x), tf32_hi(up[1] - uh.y), tf32_hi(up[2] - uh.z), tf32_hi(up[3] - uh.w));
-                            const float4 vl = make_float4(tf32_hi(vm[0] - vh.x), tf32_hi(vm[1] - vh.y), tf32_hi(vm[2] - vh.z), tf32_hi(vm[3] - vh.w));
-                            unsigned char *dst = abuf + (size_t)b * 16384 + (n >> 3) * 256 + kh * 128 + (n & 7) * 16;
-                            *reinterpret_cast<float4 *>(dst) = uh;
-                            *reinterpret_cast<float4 *>(dst + 4096) = ul;
-                            *reinterpret_cast<float4 *>(dst + 8192) = vh;
-                            *reinterpret_cast<float4 *>(dst + 12288) = vl;
+                            float up[8], vm[8];  // Q(y0+j) + Q(y0-j), Q(y0+j) - Q(y0-j); rows j = 0 and H/2 stand alone
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) {
+                                const int j = ks * 8 + i;
+                                const bool alone = j == 0 || j == H / 2;
+                                up[i] = alone ? qa[i] : qa[i] + qb[i];
+                                vm[i] = qa[i] - qb[i];
+                            }
+                            if (ks >= 2) {
+                                if (lane == 0) mbar_wait(&mdone[b], mph[b] & 1u);  // one poller per warp
+                                __syncwarp();
+                                ++mph[b];
+                                if (tid == 0 && ks + 2 < KSTEPS) issue_etile(ks + 2);
+                            }
+                            unsigned char *dst = abuf + (size_t)b * 16384 + (sn >> 3) * 256 + (sn & 7) * 16;
+#pragma unroll
+                            for (int kh = 0; kh < 2; ++kh) {
+                                const float4 uh = make_float4(tf32_hi(up[4 * kh]), tf32_hi(up[4 * kh + 1]), tf32_hi(up[4 * kh + 2]), tf32_hi(up[4 * kh + 3]));
+                                const float4 vh = make_float4(tf32_hi(vm[4 * kh]), tf32_hi(vm[4 * kh + 1]), tf32_hi(vm[4 * kh + 2]), tf32_hi(vm[4 * kh + 3]));
+                                const float4 ul = make_float4(tf32_hi(up[4 * kh] - uh.x), tf32_hi(up[4 * kh + 1] - uh.y), tf32_hi(up[4 * kh + 2] - uh.z),
+                                                              tf32_hi(up[4 * kh + 3] - uh.w));
+                                const float4 vl = make_float4(tf32_hi(vm[4 * kh] - vh.x), tf32_hi(vm[4 * kh + 1] - vh.y), tf32_hi(vm[4 * kh + 2] - vh.z),
+                                                              tf32_hi(vm[4 * kh + 3] - vh.w));
+                                *reinterpret_cast<float4 *>(dst + kh * 128) = uh;
+                                *reinterpret_cast<float4 *>(dst + kh * 128 + 4096) = ul;
+                                *reinterpret_cast<float4 *>(dst + kh * 128 + 8192) = vh;
+                                *reinterpret_cast<float4 *>(dst + kh * 128 + 12288) = vl;
+                            }
+                            fence_proxy_async();  // generic-proxy stores -> visible to the tensor core
+                            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&afull[b])) : "memory");
                         }
-                        fence_proxy_async();  // generic-proxy stores -> visible to the tensor core
-                        __syncthreads();
-                        if (tid == 0 || tid == 32) {  // thread 0 issues the MMAs of U, thread 32 those of V
-                            const uint32_t isV = tid == 32 ? 1u : 0u;
-                            mbar_wait(&ebar[e_cons & 3u], (e_cons >> 2) & 1u);
-                            const uint32_t eb = smem_u32(ering + (size_t)(e_cons & 3u) * etile) + isV * 2u * etab;
-                            const uint32_t ab = smem_u32(abuf + (size_t)b * 16384) + isV * 8192u;
+                    } else if (warp < 6) {
+                        for (int ks = 2; ks < KSTEPS; ++ks) ++mph[ks & 1];  // keeps the completion count of every thread in step
+                    } else {
+                        for (int ks = 0; ks < KSTEPS; ++ks) {
+                            const int b = ks & 1;
+                            if (ks >= 2) ++mph[b];  // keeps the completion count of every thread in step
+                            if (lane == 0) {
+                                const uint32_t isV = warp == 7 ? 1u : 0u;
+                                mbar_wait(&afull[b], aph[b] & 1u);
+                                mbar_wait(&ebar[e_cons & 3u], (e_cons >> 2) & 1u);
+                                const uint32_t eb = smem_u32(ering + (size_t)(e_cons & 3u) * etile) + isV * 2u * etab;
+                                const uint32_t ab = smem_u32(abuf + (size_t)b * 16384) + isV * 8192u;
+                                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                                const uint32_t acc = ks > 0 ? 1u : 0u, d0 = tmem + isV * 256u;
+                                // [D1 | D2] (+)= E_hi [S_hi ; S_lo]^T ;  D2 += E_lo S_hi^T ;  result = D1 + D2
+                                umma_tf32(d0, umma_desc(eb, 128, 256), umma_desc(ab, 128, 256), idescA, acc);
+                                umma_tf32(d0 + 128u, umma_desc(eb + etab, 128, 256), umma_desc(ab, 128, 256), idescB, 1u);
+                                umma_commit(&mdone[b]);
+                            }
+                            ++aph[b];
                             ++e_cons;
-                            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                            const uint32_t acc = ks > 0 ? 1u : 0u, d0 = tmem + isV * 256u;
-                            // [D1 | D2] (+)= E_hi [S_hi ; S_lo]^T ;  D2 += E_lo S_hi^T ;  result = D1 + D2
-                            umma_tf32(d0, umma_desc(eb, 128, 256), umma_desc(ab, 128, 256), idescA, acc);
-                            umma_tf32(d0 + 128u, umma_desc(eb + etab, 128, 256), umma_desc(ab, 128, 256), idescB, 1u);
-                            umma_commit(&mdone[b]);
                         }
                     }
+                    if (warp < 6) e_cons += (uint32_t)KSTEPS;  // every thread counts the consumed tiles alike
 #pragma unroll
                     for (int t = (KSTEPS >= 2 ? KSTEPS - 2 : 0); t < KSTEPS; ++t) {  // the last two steps complete
                         mbar_wait(&mdone[t & 1], mph[t & 1] & 1u);
@@ -1723,7 +1771,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         if (e < 3 * H) {
                             const int a = e / H, j = e % H;
                             const int mm = ms - 1 + a;
-                            dtab[e] = (mm >= 0 && mm < M) ? __ldg(&p.Dpol[(size_t)mm * H + j]) : 0.0;
+                            dtab[e] = (mm >= 0 && mm < M) ? __ldg(&(C::TC1 ? p.DpolPlain : p.Dpol)[(size_t)mm * H + j]) : 0.0;
                         }
                     }
                     __syncthreads();
