@@ -33,8 +33,8 @@ from paper_2310_08770_b200 import workloads as wl  # noqa: E402
 NOMINAL_SM_MHZ = 1965.0
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one 10,000-frame launch, from the committed capture
-TRAFFIC_BYTES_PER_10K_LAUNCH = 1.3173e9
-TRAFFIC_SOURCE = ("ncu --set full capture of one 10,000-frame launch, raw rows in profiles/r2a_cfg3_raw_metrics.csv "
+TRAFFIC_BYTES_PER_10K_LAUNCH = 1.3166e9
+TRAFFIC_SOURCE = ("ncu --set full capture of one 10,000-frame launch, raw rows in profiles/r2b_cfg3_raw_metrics.csv "
                   "(dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes 1.3108e9")
 
 
@@ -55,6 +55,16 @@ def executed_flops_per_frame(H, W, u):
     nd = M // 2 + 1
     fft = 5.0 * H * W * np.log2(H * W)
     return fft + 6.0 * H * (W // 2) + 2.0 * (2.0 * nd * (H // 2 + 1) * W) + 2.0 * (M * nd * W)
+
+
+def tensor_core_flops_per_frame(H, info):
+    """Flop the tensor cores are handed per frame when stage 1 runs on them: per CTA, pass over
+    the offsets and 8-row step, two accumulators (U, V) x (128 x 256 x 8 + 128 x 128 x 8) multiply-adds: the three TF32
+    passes of the hi/lo split, MMA M = 128 whatever the number of offsets in use."""
+    if not info.get("tensor_core_stage1"):
+        return 0.0
+    ksteps = (H // 2 + 1 + 7) // 8
+    return 2.0 * info["cluster_size"] * info["super_blocks"] * ksteps * 2 * (128 * 256 * 8 + 128 * 128 * 8)
 
 
 class ClockSampler:
@@ -502,7 +512,11 @@ def main():
     roofline = {
         "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
         "achieved_is": "ALGORITHMIC flop of SURVEY.md 8(d) (naive two-product upsampled DFT, 56.7 MFLOP per frame) / kernel time; "
-                       "the kernel's even/odd formulation executes 21.3 MFLOP per frame: see frac_executed",
+                       "the kernel's even/odd formulation needs 21.3 MFLOP per frame: see frac_executed.  Stage 1 of it (10.0 MFLOP at 256x256, u = 100) "
+                       "runs on the tensor cores as three TF32 passes where tensor_core_stage1 is 1, the rest on the FP32 pipes "
+                       "the peak is derived from",
+        "tensor_core_stage1": int(info.get("tensor_core_stage1", 0)),
+        "tensor_core_tflops_issued": tensor_core_flops_per_frame(cfg.H, info) * B / (kern_ms * 1e-3) / 1e12,
         "frac_executed": executed_flops_per_frame(cfg.H, cfg.W, cfg.upsample) * B / (kern_ms * 1e-3) / 1e12 / peak_tf,
         "traffic": TRAFFIC_BYTES_PER_10K_LAUNCH * B / 10000.0, "traffic_source": TRAFFIC_SOURCE,
         "kernel": "cc_fused_kernel<256,256,CS=2>", "kernel_ms": kern_ms,

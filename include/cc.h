@@ -69,6 +69,8 @@ typedef struct {
     long long table_bytes;    /* plan-owned constant tables (reference spectrum, upsampling tables) */
     int super_blocks;         /* passes of the upsampled DFT over the offsets d (T buffer capacity), throughput variant */
     int offsets_per_cta;      /* offsets d per CTA per pass                                                             */
+    int tensor_core_stage1;   /* 1 if stage 1 of the upsampled DFT runs on the tensor cores (tcgen05.mma kind::tf32,   */
+                              /* three-pass hi/lo split) in the throughput variant, 0 if on the FP32 pipes              */
 } cc_plan_info_t;
 
 /*

@@ -39,7 +39,8 @@ class PlanInfo(ctypes.Structure):
                 ("smem_bytes", ctypes.c_int), ("max_clusters", ctypes.c_int),
                 ("lat_cluster_size", ctypes.c_int), ("lat_max_clusters", ctypes.c_int),
                 ("scratch_bytes", ctypes.c_longlong), ("table_bytes", ctypes.c_longlong),
-                ("super_blocks", ctypes.c_int), ("offsets_per_cta", ctypes.c_int)]
+                ("super_blocks", ctypes.c_int), ("offsets_per_cta", ctypes.c_int),
+                ("tensor_core_stage1", ctypes.c_int)]
 
 
 _lib = None

@@ -1290,6 +1290,7 @@ extern "C" cc_status cc_plan_info(const cc_plan *plan, cc_plan_info_t *info)
     info->scratch_bytes = (long long)(plan->thr.sg_bytes + (plan->has_lat ? plan->lat.sg_bytes : 0));
     info->table_bytes = (long long)plan->table_bytes;
     info->super_blocks = plan->thr.nsb, info->offsets_per_cta = plan->thr.DS;
+    info->tensor_core_stage1 = plan->thr.v.tc1;
     return CC_OK;
 }
 
