@@ -97,6 +97,13 @@ __device__ __forceinline__ void st_async_b64(uint32_t raddr, uint64_t v, uint32_
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr), "l"(v), "r"(rbar)
                  : "memory");
 }
+// 16-byte flavour (four floats)
+__device__ __forceinline__ void st_async_v4(uint32_t raddr, float4 v, uint32_t rbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(raddr),
+                 "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "r"(rbar)
+                 : "memory");
+}
 __device__ __forceinline__ void ld_sys_v2u64(const volatile unsigned long long *p, uint64_t &a, uint64_t &b)
 {
     unsigned long long x, y;
@@ -426,8 +433,8 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
 struct Cfg {
     static constexpr bool TC1 = TC_ != 0;       // stage 1 of the upsampled DFT on the tensor cores (tcgen05, 3 x TF32)
     static constexpr int NSTG = NSTG_;  // staging ring depth
-    static constexpr int NBARS = NSTG + 15;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], tables [1], polish
-                                             // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2], staged [2]
+    static constexpr int NBARS = NSTG + 16;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], row scatter [1], polish
+                                             // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2], staged [2]; T rows [1]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
     static constexpr int H = H_, W = W_, CS = CS_, NT = NT_;
     static constexpr int TM1 = TM1_, TN1 = TN1_, TM2 = TM2_, TN2 = TN2_;
@@ -547,9 +554,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     misc = reinterpret_cast<unsigned char *>(((uintptr_t)misc + 15) & ~(uintptr_t)15);
     uint64_t *const bars = reinterpret_cast<uint64_t *>(misc);         // full[NSTG], empty[NSTG], raw ring [2]
     uint64_t *const bfull = bars, *const braw = bars + NSTG, *const xbar = braw + 2, *const cbar = xbar + 2;
-    uint64_t *const tbar = cbar + 1, *const pbar = tbar + 1;
+    uint64_t *const sbar = cbar + 1, *const pbar = sbar + 1;   // sbar: the peers' rows of the row-FFT scatter have landed
     uint64_t *const ebar = pbar + 1, *const mdone = ebar + 4, *const afull = mdone + 2;  // tensor-core stage 1: operand ring,
                                                                                          // MMA completion, operands staged
+    uint64_t *const trow = afull + 2;                          // the peers' rows of T (stage-1 output) have landed
     double *const xchg = reinterpret_cast<double *>(bars + NBARS);     // [2][CS][XN]
     float *const wv = reinterpret_cast<float *>(xchg + 2 * CS * XN);    // [NWARP]
     int *const wi = reinterpret_cast<int *>(wv + NWARP);               // [NWARP]
@@ -568,10 +576,25 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         if constexpr (CS > 1) return cluster.map_shared_rank(Ssm, r);
         return Ssm;
     };
+    // Cluster barriers.  csync(): release / acquire at cluster scope -- a MEMBAR.ALL.GPU per warp, measured at 430
+    // cycles with nothing outstanding, 1000 after global stores and 1300-2000 after remote shared-memory stores (the
+    // fence waits for their acknowledgements).  It is kept where GLOBAL data crosses CTAs (the L2-resident spectrum of
+    // the SG variants).  Remote shared-memory data travels by st.async instead: the bytes complete on an mbarrier of the
+    // receiving CTA (sbar, trow, the exchange barriers), one-way latency and no fence.  What is left is control:
+    // csync_ctl() = CTA barrier (this CTA's shared-memory accesses are performed) + relaxed arrive + wait, 120 cycles:
+    // "my peers may now read what I wrote into MY shared memory" / "I no longer touch the region you are about to fill".
     auto csync = [&]() {
         CC_JITTER();
         if constexpr (CS > 1) cluster.sync();
         else __syncthreads();
+    };
+    auto csync_ctl = [&]() {
+        CC_JITTER();
+        __syncthreads();
+        if constexpr (CS > 1) {
+            if constexpr (SG) cluster.sync();
+            else asm volatile("barrier.cluster.arrive.relaxed.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        }
     };
 
     PIX *const raw = reinterpret_cast<PIX *>(U);
@@ -612,7 +635,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         CC_JITTER();
         __syncwarp();
         if (lane == 0) {
-            __threadfence_block();  // this warp's reads of the slot are done before the count says so
+            // (every value the warp loaded from the slot has been consumed by an FMA above, so the loads have completed;
+            //  a __threadfence_block() here also waited for the refill_ti load in flight: 5-8 % of the GEMM phases)
             const uint32_t old = atomicAdd(&relcnt[c_slot], 1u);
             if ((old + 1u) % (uint32_t)NWARP == 0u && (total_tiles == 0xffffffffu || g_cons + (uint32_t)NSTG < total_tiles)) {
                 fence_proxy_async();  // generic-proxy reads of the slot before the async-proxy write
@@ -638,16 +662,17 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     double2 *const XpolS = reinterpret_cast<double2 *>(DpolS + (size_t)p.M * H);
     double *const nyqS = reinterpret_cast<double *>(XpolS + (size_t)p.M * NC);
     const bool POLS = C::LAT && p.pol_smem != 0;
-    if (tid == 0) {
-        for (int i = 0; i < NSTG; ++i) mbar_init(&bfull[i], 1), relcnt[i] = 0u;
-        mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
-        mbar_init(&xbar[0], 1), mbar_init(&xbar[1], 1), mbar_init(cbar, 1);
-        mbar_init(tbar, 1), mbar_init(pbar, 1);
-        for (int i = 0; i < 4; ++i) mbar_init(&ebar[i], 1);
-        mbar_init(&mdone[0], 2), mbar_init(&mdone[1], 2);  // the two MMA-issuing threads commit
-        mbar_init(&afull[0], 128), mbar_init(&afull[1], 128);  // the four staging warps arrive
+    static_assert(NBARS <= 32, "one lane of warp 0 per mbarrier");
+    if (tid < NBARS) {  // one barrier per lane (a single thread took 900 cycles over them); thread 0 also the raw ring's
+        uint64_t *const b = bars + tid;
+        const bool is_raw = b == &braw[0] || b == &braw[1];
+        // counts: the two MMA-issuing threads commit to mdone[]; the four staging warps arrive on afull[]; else 1
+        const uint32_t cnt = (b == &mdone[0] || b == &mdone[1]) ? 2u : (b == &afull[0] || b == &afull[1]) ? 128u : 1u;
+        if (!is_raw) mbar_init(b, cnt);
+        if (tid < NSTG) relcnt[tid] = 0u;
+        if (tid == 0) mbar_init(&braw[0], 1), mbar_init(&braw[1], 1);
         fence_mbar_init();
-        if (!p.rt_cmd && cid < p.batch && !direct_first) issue_raw_head(p.frames, cid);
+        if (tid == 0 && !p.rt_cmd && cid < p.batch && !direct_first) issue_raw_head(p.frames, cid);
     }
 #pragma unroll
     for (int e = 0; e < NI_TW; ++e)
@@ -693,7 +718,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     }
     bool csync_pending = false;  // the cluster half of the setup barrier: arrive now, wait before the first remote access
     if constexpr (CS > 1) {
-        asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+        // relaxed: what the peers need (the mbarrier inits) was published by fence.mbarrier_init.release.cluster
+        asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
         csync_pending = true;
     }
     auto setup_cluster_wait = [&]() {
@@ -705,6 +731,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         }
     };
     bool pol_pending = POLS;
+    uint32_t sph = 0u, tph1 = 0u;  // phase parities of sbar and trow
     uint32_t ph = 0;   // phase parity bits of the raw ring
     int xpar = 0;      // exchange buffer parity
     uint32_t xph = 0;  // phase parity bits of the two exchange barriers
@@ -778,8 +805,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     // returns R[a][ql] to all of them (it may shuffle inside the 8-lane group); lanes sub = b < 3 then form the
     // term of column phase b.  The packed column (rank 0, ql 0) holds (dc, nyq) and uses nyq_c[b].
     // phase(b, q) -> (cos, sin) of the column phase from the plan's fp64 tables.  Scratch `terms` =
-    // double[9][NC].  Result: out[a*3+b] valid in all threads of all CTAs.  Summation order is fixed.
-    auto xeval9 = [&](auto getR, auto phase, const double *nyq_c, double *terms, double *out) {
+    // double[9][NC].  Result: lane k < 9 of every warp of every CTA returns the value of candidate k = a*3+b (other
+    // lanes: 0).  Summation order is fixed.
+    auto xeval9 = [&](auto getR, auto phase, const double *nyq_c, double *terms) -> double {
         static_assert((24 * NC) % 32 == 0, "whole warps per (a, ql) group sweep");
         constexpr int XIT = (24 * NC + NT - 1) / NT;
 #pragma unroll
@@ -817,8 +845,23 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         double mine = 0.0;  // lane k < 9 of every warp: sum over the ranks, in rank order
         if (lane < 9)
             for (int r = 0; r < CS; ++r) mine += res[r * XN + lane];
+        return mine;
+    };
+    // The decision over the nine candidates: lane k < 9 holds (value, index, valid); larger value wins, then the smaller
+    // index -- a 16-lane butterfly instead of nine broadcasts and a nine-way compare chain (this code runs once per
+    // launch in the single-frame variants, from a cold instruction cache: its size is its cost).  All lanes return the
+    // winner's value and candidate number.
+    auto best9 = [&](double v, int idx, bool valid, double &bv, int &bk) {
+        if (!valid || lane >= 9) v = -INFINITY, idx = 0x7fffffff;
+        int k = lane;
 #pragma unroll
-        for (int k = 0; k < 9; ++k) out[k] = __shfl_sync(0xffffffffu, mine, k);
+        for (int o = 8; o >= 1; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, v, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, idx, o), ok = __shfl_xor_sync(0xffffffffu, k, o);
+            if (ov > v || (ov == v && oi < idx)) v = ov, idx = oi, k = ok;
+        }
+        bv = __shfl_sync(0xffffffffu, v, 0);
+        bk = __shfl_sync(0xffffffffu, k, 0);
     };
 
     long long tph = t_entry;  // the first frame's phase 0 includes the kernel setup
@@ -937,7 +980,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     float2 gpre[GPRE ? RLc : 1];
     for (int f = cid; RT || f < p.batch; f += ncl) {
         const void *frames = p.frames;
-        if (RT) {
+        if (__builtin_expect(RT, false)) {
             // ---- real-time session (one displacement per camera frame, as it arrives): rank 0
             // polls the host's command word; (seq, frame pointer) go to every CTA of the cluster by st.async
             f = 0;
@@ -988,6 +1031,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         {
             const PIX *fbase = reinterpret_cast<const PIX *>(frames) + (size_t)f * H * W + (size_t)rank * NR * W;
             if (tid == 0 && !RT && f != cid) issue_raw_head(frames, f);  // the first frame's rows were requested during the setup
+            if constexpr (!SG && CS > 1) {  // the other CTAs' rows of my columns arrive by st.async
+                if (tid == 0) mbar_expect_tx(sbar, (uint32_t)((CS - 1) * NR * NC * 8));
+            }
             // latency variants: every thread owns at most one butterfly of the fused column pass; its RL values of
             // conj(G)/(HW) are requested now (L2 latency hidden behind the ingest and the row FFTs)
             if constexpr (GPRE) {
@@ -1049,9 +1095,21 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                 A = make_float2(0.5f * (z1[i].x + z2[i].x), 0.5f * (z1[i].y - z2[i].y));
                                 B = make_float2(0.5f * (z1[i].y + z2[i].y), -0.5f * (z1[i].x - z2[i].x));
                             }
-                            float2 *Sd = Sof(k / NC);
-                            Sd[(size_t)ya * NC + (k % NC)] = A;
-                            Sd[(size_t)yb * NC + (k % NC)] = B;
+                            const int dr = k / NC;
+                            if constexpr (SG || CS == 1) {
+                                float2 *Sd = Sof(dr);
+                                Sd[(size_t)ya * NC + (k % NC)] = A;
+                                Sd[(size_t)yb * NC + (k % NC)] = B;
+                            } else if (dr == rank) {
+                                Ssm[(size_t)ya * NC + (k % NC)] = A;
+                                Ssm[(size_t)yb * NC + (k % NC)] = B;
+                            } else {  // a peer's columns: the bytes complete on the peer's sbar (no fence, no cluster barrier)
+                                const uint32_t rb = mapa_u32(smem_u32(sbar), (uint32_t)dr);
+                                st_async_b64(mapa_u32(smem_u32(Ssm + (size_t)ya * NC + (k % NC)), (uint32_t)dr),
+                                             (uint64_t)__float_as_uint(A.x) | ((uint64_t)__float_as_uint(A.y) << 32), rb);
+                                st_async_b64(mapa_u32(smem_u32(Ssm + (size_t)yb * NC + (k % NC)), (uint32_t)dr),
+                                             (uint64_t)__float_as_uint(B.x) | ((uint64_t)__float_as_uint(B.y) << 32), rb);
+                            }
                         }
                     }
                     __syncwarp();
@@ -1063,7 +1121,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
             }
         }
-        csync();  // every F_row[y][kx] is at its column owner
+        // every F_row[y][kx] is at its column owner: my own rows by the CTA barrier above, the peers' rows when their bytes
+        // have completed on sbar
+        if constexpr (SG || CS == 1) {
+            csync();
+        } else {
+            mbar_wait(sbar, sph);
+            sph ^= 1u;
+        }
         stamp(0, f);
 
         // =============================================================== a2/a3/a4: column FFT (x) Gc, column inverse
@@ -1176,7 +1241,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 fft_bfly<R0, true, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
             }
         }
-        csync();  // Q[y][kx] complete everywhere
+        csync_ctl();  // Q[y][kx] complete everywhere (every CTA wrote its own block; the peers read it remotely)
         stamp(1, f);
 
         // =============================================================== a4/a5: row C2R streamed into the integer argmax
@@ -1240,40 +1305,35 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 
             // fp64 re-evaluation of the 3x3 neighbourhood of the fp32 winner
             double *terms = reinterpret_cast<double *>(U);
-            double nyq[3], c9[9];
+            double nyq[3];
 #pragma unroll
             for (int b = 0; b < 3; ++b) nyq[b] = ((x0 - 1 + b) & 1) ? -1.0 : 1.0;
-            xeval9(
+            const double mine = xeval9(
                 [&](int a, int ql, int) {
                     const float2 v = Sl[(size_t)((y0 - 1 + a) & (H - 1)) * NC + ql];
                     return make_double2((double)v.x, (double)v.y);
                 },
-                [&](int b, int q) { return tw64[(q * ((x0 - 1 + b) & (W - 1))) & (W - 1)]; }, nyq, terms, c9);
-            double bv = -INFINITY;
-            int bi = 0x7fffffff;
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-#pragma unroll
-                for (int b = 0; b < 3; ++b) {
-                    const int yy = (y0 - 1 + a) & (H - 1), xx = (x0 - 1 + b) & (W - 1);
-                    const int idx = yy * W + xx;
-                    const double v = c9[a * 3 + b];
-                    if (v > bv || (v == bv && idx < bi)) bv = v, bi = idx;
-                }
-            y0 = bi / W;
-            x0 = bi % W;
+                [&](int b, int q) { return tw64[(q * ((x0 - 1 + b) & (W - 1))) & (W - 1)]; }, nyq, terms);
+            double bv;
+            int bk;  // candidate k = a*3+b sits at ((y0-1+a) mod H, (x0-1+b) mod W); equal values: the smaller pixel index
+            {
+                const int a = lane / 3, b = lane % 3;
+                best9(mine, (((y0 - 1 + a) & (H - 1)) * W) + ((x0 - 1 + b) & (W - 1)), true, bv, bk);
+            }
+            y0 = (y0 - 1 + bk / 3) & (H - 1);
+            x0 = (x0 - 1 + bk % 3) & (W - 1);
             cc_peak = bv;
         }
         stamp(3, f);
         const int wy = (2 * y0 >= H) ? y0 - H : y0;
         const int wx = (2 * x0 >= W) ? x0 - W : x0;
 
-        if (u == 1) {
+        if (__builtin_expect(u == 1, false)) {
             if (rank == 0 && tid == 0) {
                 const double Em = p.ri_emean ? __ldcg(p.ri_emean) : p.Emean;
                 emit(f, (float)wy, (float)wx, (float)(p.peak_sign * (cc_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
             }
-            if (RI) {
+            if (__builtin_expect(RI, false)) {
                 __syncthreads();  // the reference mean was read before it is rewritten
                 ri_update((long long)wy, (long long)wx);
             }
@@ -1311,6 +1371,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             float *const red = Tb + (size_t)2 * DS * LDT;  // k-split partial sums (KS1 > 1, KS2 > 1)
             for (int sb = 0; sb < p.nsb; ++sb) {
                 const int db = sb * DSB;
+                // stage-1 output rows reach their owner by st.async: my live offsets x 2 rows x the peers' 2 NC floats each
+                if constexpr (!SG && CS > 1) {
+                    if (tid == 0) {
+                        const int n_live = min(max(nd - db - rank * DS, 0), DS);
+                        mbar_expect_tx(trow, (uint32_t)((CS - 1) * n_live * 2 * (2 * NC) * 4));
+                    }
+                }
                 if constexpr (C::TC1) {
                 // ---------------- stage 1 on the tensor cores (tcgen05.mma kind::tf32, accumulators in tensor memory):
                 //   U[d][n] = sum_j Ee[d][j] S[(y0+j)][n],  V[d][n] = sum_j Eo[d][j] S[(y0-j)][n]   (n = my 128 spectrum floats;
@@ -1420,14 +1487,18 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         ++mph[t & 1];
                     }
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    csync();  // no CTA of the cluster stages operands in its U region any more: T rows may land there
+                    csync_ctl();  // no CTA of the cluster stages operands in its U region any more: T rows may land there
                     {   // thread = (offset d = lane of tensor memory, half of the 128 spectrum floats): a row segment of T
                         const int lb = 32 * (warp & 3), dsb = lb + lane, half = warp >> 2;
                         const bool live = dsb < DSB && db + dsb < nd;
                         const int dr = dsb / DS, row = dsb % DS;
-                        float *Td = Tb;
-                        if constexpr (CS > 1) Td = cluster.map_shared_rank(Tb, live ? dr : rank);
-                        float *const dstp = Td + (size_t)row * LDT + rank * 2 * NC, *const dstm = dstp + (size_t)DS * LDT;
+                        float *const dstp = Tb + (size_t)row * LDT + rank * 2 * NC, *const dstm = dstp + (size_t)DS * LDT;
+                        const bool remote = CS > 1 && live && dr != rank;
+                        uint32_t rp = 0, rm = 0, rb = 0;  // the owner's copy of the two rows and its trow barrier
+                        if constexpr (CS > 1) {
+                            if (remote) rp = mapa_u32(smem_u32(dstp), (uint32_t)dr), rm = mapa_u32(smem_u32(dstm), (uint32_t)dr),
+                                        rb = mapa_u32(smem_u32(trow), (uint32_t)dr);
+                        }
                         const float sg = (x0 & 1) ? -1.f : 1.f;
                         const uint32_t tb = tmem + ((uint32_t)lb << 16);
 #pragma unroll 1
@@ -1456,7 +1527,13 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                     op[i] = a.x, op[i + 1] = a.y, om[i] = bq.x, om[i + 1] = bq.y;
                                 }
                             }
-                            if (live) {
+                            if (remote) {
+#pragma unroll
+                                for (int v = 0; v < 4; ++v) {
+                                    st_async_v4(rp + (uint32_t)(c0 + 4 * v) * 4u, make_float4(op[4 * v], op[4 * v + 1], op[4 * v + 2], op[4 * v + 3]), rb);
+                                    st_async_v4(rm + (uint32_t)(c0 + 4 * v) * 4u, make_float4(om[4 * v], om[4 * v + 1], om[4 * v + 2], om[4 * v + 3]), rb);
+                                }
+                            } else if (live) {
 #pragma unroll
                                 for (int v = 0; v < 4; ++v) {
                                     *reinterpret_cast<float4 *>(dstp + c0 + 4 * v) = make_float4(op[4 * v], op[4 * v + 1], op[4 * v + 2], op[4 * v + 3]);
@@ -1466,7 +1543,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         }
                     }
                     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                    csync();  // T(c+d), T(c-d) rows are at their owners
+                    __syncthreads();  // my own rows of T(c+d), T(c-d) ...
+                    if constexpr (CS > 1) {  // ... and the peers' (their bytes have completed on trow)
+                        mbar_wait(trow, tph1);
+                        tph1 ^= 1u;
+                    }
                 }
                 } else {
                 // ---------------- stage 1: rows [U(d) | V(d)] of this super-block, my 2*NC spectrum floats
@@ -1572,18 +1653,37 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         const int dsb = gc0 + i - (isV ? DSBp : 0);
                         if (dsb < DSB && db + dsb < nd) {
                             const int dr = dsb / DS, row = dsb % DS + (isV ? DS : 0);
-                            float *Td = Tb;
-                            if constexpr (CS > 1) Td = cluster.map_shared_rank(Tb, dr);
-                            float *dst = Td + (size_t)row * LDT + rank * 2 * NC + tn1 * 4;
+                            float *dst = Tb + (size_t)row * LDT + rank * 2 * NC + tn1 * 4;
+                            if constexpr (SG || CS == 1) {
+                                if constexpr (CS > 1) dst = cluster.map_shared_rank(dst, dr);
 #pragma unroll
-                            for (int v = 0; v < TN1 / 4; ++v)
-                                *reinterpret_cast<float4 *>(dst + v * Cn1 * 4) =
-                                    make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]);
+                                for (int v = 0; v < TN1 / 4; ++v)
+                                    *reinterpret_cast<float4 *>(dst + v * Cn1 * 4) =
+                                        make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]);
+                            } else if (dr == rank) {
+#pragma unroll
+                                for (int v = 0; v < TN1 / 4; ++v)
+                                    *reinterpret_cast<float4 *>(dst + v * Cn1 * 4) =
+                                        make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]);
+                            } else {  // the owner's copy of the row; the bytes complete on its trow barrier
+                                const uint32_t rd = mapa_u32(smem_u32(dst), (uint32_t)dr), rb = mapa_u32(smem_u32(trow), (uint32_t)dr);
+#pragma unroll
+                                for (int v = 0; v < TN1 / 4; ++v)
+                                    st_async_v4(rd + (uint32_t)(v * Cn1 * 4) * 4u,
+                                                make_float4(acc[i][4 * v], acc[i][4 * v + 1], acc[i][4 * v + 2], acc[i][4 * v + 3]), rb);
+                            }
                         }
                     }
                     }  // ks1 == 0
                 }
-                csync();  // U, V rows are at their owners
+                // U, V rows are at their owners: mine after the CTA barrier, the peers' when their bytes have completed
+                if constexpr (SG || CS == 1) {
+                    csync();
+                } else {
+                    __syncthreads();
+                    mbar_wait(trow, tph1);
+                    tph1 ^= 1u;
+                }
                 // rows dl and DS+dl become T(c+d) = U+V and T(c-d) = U-V
                 for (int idx = tid; idx < DS * (W / 4); idx += NT) {
                     const int dl = idx / (W / 4), c4 = idx % (W / 4);
@@ -1733,7 +1833,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                 }
                 stamp(5, f);
-                if (sb + 1 < p.nsb) csync();  // T is overwritten by the next super-block
+                if (sb + 1 < p.nsb) csync_ctl();  // T is overwritten by the next super-block
             }
         }
         int ms, ns;
@@ -1791,7 +1891,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     part[(1 * NSL + sl) * NC + ql] = s1;
                     part[(2 * NSL + sl) * NC + ql] = s2;
                 }
-                double nyq[3], c9[9];
+                double nyq[3];
                 const double sgx = (x0 & 1) ? -1.0 : 1.0;
 #pragma unroll
                 for (int b = 0; b < 3; ++b) {
@@ -1799,7 +1899,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     nyq[b] = sgx * (POLS ? nyqS[nn] : __ldg(&p.nyq64[nn]));
                 }
                 __syncthreads();
-                xeval9(
+                const double mine = xeval9(
                     [&](int a, int ql, int sub) {  // sum of the j-slices, 8 lanes per (a, ql)
                         double sx = 0.0, sy = 0.0;
                         for (int sl = sub; sl < NSL; sl += 8) {
@@ -1820,19 +1920,14 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         const double2 w1 = POLS ? XpolS[(size_t)nn * NC + (q - rank * NC)] : __ldg(&p.Xpol[(size_t)nn * (W / 2) + q]);
                         return make_double2(w0.x * w1.x - w0.y * w1.y, w0.x * w1.y + w0.y * w1.x);
                     },
-                    nyq, terms, c9);
-                double bv = -INFINITY;
-                int ba = 1, bb = 1, bi = 0x7fffffff;
-#pragma unroll
-                for (int a = 0; a < 3; ++a)
-#pragma unroll
-                    for (int b = 0; b < 3; ++b) {
-                        const int mm = ms - 1 + a, nn = ns - 1 + b;
-                        if (mm < 0 || mm >= M || nn < 0 || nn >= M) continue;
-                        const int idx = mm * M + nn;
-                        const double v = c9[a * 3 + b];
-                        if (v > bv || (v == bv && idx < bi)) bv = v, bi = idx, ba = a, bb = b;
-                    }
+                    nyq, terms);
+                double bv;
+                int bk;  // candidate k = a*3+b is grid point (ms-1+a, ns-1+b); points outside the M x M grid do not compete
+                {
+                    const int mm = ms - 1 + lane / 3, nn = ns - 1 + lane % 3;
+                    best9(mine, mm * M + nn, mm >= 0 && mm < M && nn >= 0 && nn < M, bv, bk);
+                }
+                const int ba = bk / 3, bb = bk % 3;
                 up_peak = bv;
                 if (ba == 1 && bb == 1) break;
                 ms += ba - 1;
@@ -1846,7 +1941,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
                  (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
         }
-        if (RI) {
+        if (__builtin_expect(RI, false)) {  // (cold paths are marked so that the hot path stays one straight run of code)
             __syncthreads();  // the reference mean was read before it is rewritten
             ri_update((long long)wy * u + (ms - cM), (long long)wx * u + (ns - cM));
         }
@@ -1858,7 +1953,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             if (++c_slot == NSTG) c_slot = 0, c_par ^= 1u;
         }
     }
-    csync();  // no CTA of the cluster exits while peers may still address its shared memory
+    csync_ctl();  // no CTA of the cluster exits while peers may still address its shared memory
     if constexpr (C::TC1) {
         if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
     }
