@@ -413,18 +413,16 @@ struct Best {
     int i;
 };
 __device__ __forceinline__ bool better(float v1, int i1, float v2, int i2) { return v1 > v2 || (v1 == v2 && i1 < i2); }
+// Over a warp: two hardware reductions (redux.sync) instead of five shuffle rounds -- the maximum of an order-preserving
+// integer image of the value (-0 folded into +0 so that equal values have equal keys), then the smallest index among the
+// lanes that hold it.
 __device__ __forceinline__ Best warp_best(Best b)
 {
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) {
-        const float v = __shfl_xor_sync(0xffffffffu, b.v, o);
-        const int i = __shfl_xor_sync(0xffffffffu, b.i, o);
-        if (better(v, i, b.v, b.i)) {
-            b.v = v;
-            b.i = i;
-        }
-    }
-    return b;
+    const uint32_t u = __float_as_uint(b.v + 0.0f);
+    const uint32_t key = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    const uint32_t kmax = __reduce_max_sync(0xffffffffu, key);
+    const int imin = __reduce_min_sync(0xffffffffu, key == kmax ? b.i : 0x7fffffff);
+    return Best{__uint_as_float((kmax & 0x80000000u) ? (kmax & 0x7fffffffu) : ~kmax), imin};
 }
 
 // ------------------------------------------------------------------ the kernel
@@ -883,17 +881,17 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     uint64_t rt_seq = 0;    // sequence number of the command being served
     uint32_t cph = 0;       // phase parity of the command barrier
     auto emit = [&](int f, float dyv, float dxv, float pkv, int wyv, int wxv) {
-        if (RT) {  // one 16-byte store; the sequence number is the last word
-            asm volatile("st.volatile.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p.rt_res), "f"(dxv), "f"(dyv), "f"(pkv),
-                         "f"(__uint_as_float((uint32_t)rt_seq))
-                         : "memory");
-            __threadfence_system();
-        } else {
+        if (__builtin_expect(!RT, true)) {
             p.dy[f] = dyv;
             p.dx[f] = dxv;
             if (p.peak) p.peak[f] = pkv;
             if (p.iy) p.iy[f] = wyv;
             if (p.ix) p.ix[f] = wxv;
+        } else {  // one 16-byte store; the sequence number is the last word
+            asm volatile("st.volatile.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p.rt_res), "f"(dxv), "f"(dyv), "f"(pkv),
+                         "f"(__uint_as_float((uint32_t)rt_seq))
+                         : "memory");
+            __threadfence_system();
         }
     };
 
@@ -1941,7 +1939,10 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             emit(f, (float)((double)wy + (double)(ms - cM) / (double)u), (float)((double)wx + (double)(ns - cM) / (double)u),
                  (float)(p.peak_sign * (up_peak + ((double)*f00 + c0d * H * W) * Em)), wy, wx);
         }
-        if (__builtin_expect(RI, false)) {  // (cold paths are marked so that the hot path stays one straight run of code)
+        // this cluster's last frame of a plain launch goes straight to the exit (single-frame calls run this code from a
+        // cold instruction cache: every taken branch to code not yet fetched costs ~250 cycles)
+        if (__builtin_expect(!RT && !RI && f + ncl >= p.batch, true)) break;
+        if (__builtin_expect(RI, false)) {
             __syncthreads();  // the reference mean was read before it is rewritten
             ri_update((long long)wy * u + (ms - cM), (long long)wx * u + (ns - cM));
         }
