@@ -491,7 +491,7 @@ struct Cfg {
     static_assert(TILEF % 4 == 0 && MC1 % 4 == 0, "tile alignment");
     static_assert(NT % NC == 0 || NC % NT == 0, "threads vs columns");
     static_assert(NSTG <= 8, "ring (sched_head carries 8 entries)");
-    static_assert(!TC1 || (2 * NC == 128 && NT == 256 && !SG), "tensor-core stage 1: 128 spectrum floats per CTA (MMA M = 128), 8 warps");
+    static_assert(!TC1 || (2 * NC == 128 && NT == 256), "tensor-core stage 1: 128 spectrum floats per CTA (MMA N = 128), 8 warps");
 };
 
 template <class C>
@@ -589,10 +589,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
     auto csync_ctl = [&]() {
         CC_JITTER();
         __syncthreads();
-        if constexpr (CS > 1) {
-            if constexpr (SG) cluster.sync();
-            else asm volatile("barrier.cluster.arrive.relaxed.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-        }
+        if constexpr (CS > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
     };
 
     PIX *const raw = reinterpret_cast<PIX *>(U);
@@ -1239,7 +1236,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 fft_bfly<R0, true, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
             }
         }
-        csync_ctl();  // Q[y][kx] complete everywhere (every CTA wrote its own block; the peers read it remotely)
+        // Q[y][kx] complete everywhere: every CTA wrote its own block, the peers read it remotely (SG: through L2, fenced)
+        if constexpr (SG) csync();
+        else csync_ctl();
         stamp(1, f);
 
         // =============================================================== a4/a5: row C2R streamed into the integer argmax
@@ -1370,7 +1369,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
             for (int sb = 0; sb < p.nsb; ++sb) {
                 const int db = sb * DSB;
                 // stage-1 output rows reach their owner by st.async: my live offsets x 2 rows x the peers' 2 NC floats each
-                if constexpr (!SG && CS > 1) {
+                if constexpr (CS > 1) {
                     if (tid == 0) {
                         const int n_live = min(max(nd - db - rank * DS, 0), DS);
                         mbar_expect_tx(trow, (uint32_t)((CS - 1) * n_live * 2 * (2 * NC) * 4));
@@ -1415,15 +1414,19 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     // buffer b two steps later.  No CTA barrier inside the loop.
                     if (warp < 4) {  // thread n: spectrum float n, the 8 rows of the step (two 16-byte K chunks per table)
                         const int sn = tid;
-                        for (int ks = 0; ks < KSTEPS; ++ks) {
-                            const int b = ks & 1;
-                            float qa[8], qb[8];
+                        float qa[8], qb[8];
+                        auto load_rows = [&](int ks) {
 #pragma unroll
                             for (int i = 0; i < 8; ++i) {
                                 const int j = ks * 8 + i;   // rows beyond H/2 meet zero weights
                                 qa[i] = Sf[(size_t)((y0 + j) & (H - 1)) * (2 * NC) + sn];
                                 qb[i] = Sf[(size_t)((y0 - j) & (H - 1)) * (2 * NC) + sn];
                             }
+                        };
+                        if constexpr (SG) load_rows(0);
+                        for (int ks = 0; ks < KSTEPS; ++ks) {
+                            const int b = ks & 1;
+                            if constexpr (!SG) load_rows(ks);
                             float up[8], vm[8];  // Q(y0+j) + Q(y0-j), Q(y0+j) - Q(y0-j); rows j = 0 and H/2 stand alone
 #pragma unroll
                             for (int i = 0; i < 8; ++i) {
@@ -1431,6 +1434,9 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                                 const bool alone = j == 0 || j == H / 2;
                                 up[i] = alone ? qa[i] : qa[i] + qb[i];
                                 vm[i] = qa[i] - qb[i];
+                            }
+                            if constexpr (SG) {  // spectrum block in L2: the next step's rows are requested a step ahead
+                                if (ks + 1 < KSTEPS) load_rows(ks + 1);
                             }
                             if (ks >= 2) {
                                 if (lane == 0) mbar_wait(&mdone[b], mph[b] & 1u);  // one poller per warp
@@ -1463,8 +1469,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                             if (ks >= 2) ++mph[b];  // keeps the completion count of every thread in step
                             if (lane == 0) {
                                 const uint32_t isV = warp == 7 ? 1u : 0u;
+                                mbar_wait(&ebar[e_cons & 3u], (e_cons >> 2) & 1u);  // (landed long ago: first, off the critical path)
                                 mbar_wait(&afull[b], aph[b] & 1u);
-                                mbar_wait(&ebar[e_cons & 3u], (e_cons >> 2) & 1u);
                                 const uint32_t eb = smem_u32(ering + (size_t)(e_cons & 3u) * etile) + isV * 2u * etab;
                                 const uint32_t ab = smem_u32(abuf + (size_t)b * 16384) + isV * 8192u;
                                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -1652,8 +1658,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                         if (dsb < DSB && db + dsb < nd) {
                             const int dr = dsb / DS, row = dsb % DS + (isV ? DS : 0);
                             float *dst = Tb + (size_t)row * LDT + rank * 2 * NC + tn1 * 4;
-                            if constexpr (SG || CS == 1) {
-                                if constexpr (CS > 1) dst = cluster.map_shared_rank(dst, dr);
+                            if constexpr (CS == 1) {
 #pragma unroll
                                 for (int v = 0; v < TN1 / 4; ++v)
                                     *reinterpret_cast<float4 *>(dst + v * Cn1 * 4) =
@@ -1675,10 +1680,8 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }  // ks1 == 0
                 }
                 // U, V rows are at their owners: mine after the CTA barrier, the peers' when their bytes have completed
-                if constexpr (SG || CS == 1) {
-                    csync();
-                } else {
-                    __syncthreads();
+                __syncthreads();
+                if constexpr (CS > 1) {
                     mbar_wait(trow, tph1);
                     tph1 ^= 1u;
                 }

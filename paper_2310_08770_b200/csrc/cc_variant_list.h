@@ -22,8 +22,8 @@ CCV(f256_u16,      256,  256, 2, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,
 CCV(f256_u8,       256,  256, 2, uint8_t,  256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1, 1)
 CCV(f512_u16,      512,  512, 8, uint16_t, 256,  5, 4,  2, 5, false, 16,  8,  8,  4,  3,  2,  1, 0)
 CCV(f512_u8,       512,  512, 8, uint8_t,  256,  5, 4,  2, 5, false, 16,  8,  8,  4,  3,  2,  1, 0)
-CCV(f1024_u16,    1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1, 0)
-CCV(f1024_u8,     1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1, 0)
+CCV(f1024_u16,    1024, 1024, 8, uint16_t, 256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1, 1)
+CCV(f1024_u8,     1024, 1024, 8, uint8_t,  256, 10, 8,  5, 5, true,  16, 16,  4,  4,  3,  2,  1, 1)
 // non-square camera formats of the paper's Table I; H = rows, W = columns
 CCV(f128x256_u16,  128,  256, 1, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1, 0)
 CCV(f256x128_u16,  256,  128, 1, uint16_t, 256, 10, 8,  5, 5, false, 12,  4, 16,  1,  2,  2,  1, 0)
