@@ -1127,34 +1127,45 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
         stamp(0, f);
 
         // =============================================================== a2/a3/a4: column FFT (x) Gc, column inverse
-        {
+        // (SG: the CTA's spectrum block lives in L2; its columns pass through shared memory NCB at a time -- one read and
+        //  one write of the block per frame instead of one per pass: the column passes at 1024 x 1024 were L2-bandwidth bound)
+        constexpr int NCB = SG ? 8 : NC;  // columns per block (SG: H x 8 complex in the U region, free during this phase)
+        static_assert(!SG || ((size_t)H * NCB * 8 <= (size_t)C::RAWB + C::SCRB && NC % NCB == 0), "column block fits the raw + scratch region");
+        for (int cb = 0; cb < NC / NCB; ++cb) {
             constexpr int R0 = cc_radix_col(H, 0), R1 = cc_radix_col(H, 1), R2 = cc_radix_col(H, 2);
             constexpr int RL = R2 > 1 ? R2 : R1;   // radix of the last forward pass (fused with the product)
             constexpr int NPASS = R2 > 1 ? 3 : 2;
+            float2 *const Sb = SG ? reinterpret_cast<float2 *>(U) : Sl;  // [H][NCB]
+            if constexpr (SG) {
+#pragma unroll 4
+                for (int idx = tid; idx < H * NCB / 2; idx += NT) {
+                    const int y = idx / (NCB / 2), c2 = idx % (NCB / 2);
+                    *reinterpret_cast<float4 *>(Sb + (size_t)y * NCB + 2 * c2) =
+                        __ldcg(reinterpret_cast<const float4 *>(Sl + (size_t)y * NC + cb * NCB + 2 * c2));
+                }
+                __syncthreads();
+            }
             // forward pass 0
-            #pragma unroll(SG ? 2 : 1)
-            for (int it = tid; it < NC * (H / R0); it += NT) {
-                const int ql = it % NC, g = it / NC;
+            for (int it = tid; it < NCB * (H / R0); it += NT) {
+                const int ql = it % NCB, g = it / NCB;
                 constexpr int ST = H / R0;
-                fft_bfly<R0, false, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
+                fft_bfly<R0, false, true, NTW>([&](int i) { return Sb + (size_t)(g + i * ST) * NCB + ql; }, g * (NTW / H), tw);
             }
             __syncthreads();
             if constexpr (NPASS == 3) {  // forward pass 1 of 3
                 constexpr int L = H / R0, ST = L / R1;
-                #pragma unroll(SG ? 2 : 1)
-                for (int it = tid; it < NC * (H / R1); it += NT) {
-                    const int ql = it % NC, g = it / NC;
+                for (int it = tid; it < NCB * (H / R1); it += NT) {
+                    const int ql = it % NCB, g = it / NCB;
                     const int blk = g / ST, b = g % ST;
-                    fft_bfly<R1, false, true, NTW>([&](int i) { return Sl + (size_t)(blk * L + b + i * ST) * NC + ql; },
+                    fft_bfly<R1, false, true, NTW>([&](int i) { return Sb + (size_t)(blk * L + b + i * ST) * NCB + ql; },
                                                    b * (NTW / L), tw);
                 }
                 __syncthreads();
             }
             // last forward pass (contiguous slots), product with conj(G)/(HW), first inverse pass
-            #pragma unroll(SG ? 2 : 1)
-            for (int it = tid; it < NC * (H / RL); it += NT) {
-                const int ql = it % NC, g = it / NC;
-                const int q = rank * NC + ql;
+            for (int it = tid; it < NCB * (H / RL); it += NT) {
+                const int ql = it % NCB, g = it / NCB;
+                const int q = rank * NC + cb * NCB + ql;
                 // the butterfly's RL values of conj(G)/(HW) are requested first (through L2: the RI update rewrites Gt),
                 // so their latency runs under the shared-memory loads and the forward DFT
                 float2 gv[RL];
@@ -1167,12 +1178,12 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 }
                 float2 v[RL];
 #pragma unroll
-                for (int i = 0; i < RL; ++i) v[i] = Sl[(size_t)(g * RL + i) * NC + ql];
+                for (int i = 0; i < RL; ++i) v[i] = Sb[(size_t)(g * RL + i) * NCB + ql];
                 dft_reg<RL, false>(v);
                 constexpr int bits = ilog2c(RL);
                 if (q == 0) {  // packed DC/Nyquist column: needs the -ky partner, handled below
 #pragma unroll
-                    for (int k = 0; k < RL; ++k) Sl[(size_t)(g * RL + k) * NC + ql] = v[brev(k, bits)];
+                    for (int k = 0; k < RL; ++k) Sb[(size_t)(g * RL + k) * NCB + ql] = v[brev(k, bits)];
                 } else {
                     float2 w[RL];
 #pragma unroll
@@ -1183,11 +1194,11 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                     }
                     dft_reg<RL, true>(w);
 #pragma unroll
-                    for (int n = 0; n < RL; ++n) Sl[(size_t)(g * RL + n) * NC + ql] = w[brev(n, bits)];
+                    for (int n = 0; n < RL; ++n) Sb[(size_t)(g * RL + n) * NCB + ql] = w[brev(n, bits)];
                 }
             }
             __syncthreads();
-            if (rank == 0) {
+            if (rank == 0 && cb == 0) {
                 // two real columns (kx = 0 and kx = W/2) ride in one complex FFT: split them with the -ky
                 // partner, multiply each by its conj(G) column, re-pack as PA + i PB.  The split is done
                 // first so that exact zeros stay exact (a constant frame must give P = 0, not rounding noise).
@@ -1197,7 +1208,7 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
                 for (int e = 0; e < PER; ++e) {
                     const int s = tid + e * NT;
                     if (s < H) {
-                        const float2 z = Sl[(size_t)s * NC], zp = Sl[(size_t)p.col_partner[s] * NC];
+                        const float2 z = Sb[(size_t)s * NCB], zp = Sb[(size_t)p.col_partner[s] * NCB];
                         const float4 g = __ldcg(&p.ab[s]);  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
@@ -1211,29 +1222,37 @@ __global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
 #pragma unroll
                 for (int e = 0; e < PER; ++e) {
                     const int s = tid + e * NT;
-                    if (s < H) Sl[(size_t)s * NC] = o[e];
+                    if (s < H) Sb[(size_t)s * NCB] = o[e];
                 }
                 __syncthreads();
                 for (int g = tid; g < H / RL; g += NT)
-                    fft_bfly<RL, true, false, NTW>([&](int i) { return Sl + (size_t)(g * RL + i) * NC; }, 0, tw);
+                    fft_bfly<RL, true, false, NTW>([&](int i) { return Sb + (size_t)(g * RL + i) * NCB; }, 0, tw);
                 __syncthreads();
             }
             if constexpr (NPASS == 3) {  // inverse of forward pass 1
                 constexpr int L = H / R0, ST = L / R1;
-                #pragma unroll(SG ? 2 : 1)
-                for (int it = tid; it < NC * (H / R1); it += NT) {
-                    const int ql = it % NC, g = it / NC;
+                for (int it = tid; it < NCB * (H / R1); it += NT) {
+                    const int ql = it % NCB, g = it / NCB;
                     const int blk = g / ST, b = g % ST;
-                    fft_bfly<R1, true, true, NTW>([&](int i) { return Sl + (size_t)(blk * L + b + i * ST) * NC + ql; },
+                    fft_bfly<R1, true, true, NTW>([&](int i) { return Sb + (size_t)(blk * L + b + i * ST) * NCB + ql; },
                                                   b * (NTW / L), tw);
                 }
                 __syncthreads();
             }
-            #pragma unroll(SG ? 2 : 1)
-            for (int it = tid; it < NC * (H / R0); it += NT) {
-                const int ql = it % NC, g = it / NC;
+            for (int it = tid; it < NCB * (H / R0); it += NT) {
+                const int ql = it % NCB, g = it / NCB;
                 constexpr int ST = H / R0;
-                fft_bfly<R0, true, true, NTW>([&](int i) { return Sl + (size_t)(g + i * ST) * NC + ql; }, g * (NTW / H), tw);
+                fft_bfly<R0, true, true, NTW>([&](int i) { return Sb + (size_t)(g + i * ST) * NCB + ql; }, g * (NTW / H), tw);
+            }
+            if constexpr (SG) {  // the finished block goes back to L2
+                __syncthreads();
+#pragma unroll 4
+                for (int idx = tid; idx < H * NCB / 2; idx += NT) {
+                    const int y = idx / (NCB / 2), c2 = idx % (NCB / 2);
+                    __stcg(reinterpret_cast<float4 *>(Sl + (size_t)y * NC + cb * NCB + 2 * c2),
+                           *reinterpret_cast<const float4 *>(Sb + (size_t)y * NCB + 2 * c2));
+                }
+                __syncthreads();
             }
         }
         // Q[y][kx] complete everywhere: every CTA wrote its own block, the peers read it remotely (SG: through L2, fenced)
