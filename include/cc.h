@@ -120,6 +120,31 @@ cc_status cc_track(const cc_plan *plan, const void *frames, int batch,
                    float *dx, float *dy, float *peak, void *stream);
 
 /*
+ * cc_track_static -- cc_track for callers that cannot tolerate a device allocation anywhere near the call (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same computation, same results, same
+ * arguments as cc_track (Eq. (4)), but:
+ *   - the global spectrum scratch of the shapes that need one (1024 x 1024: the half spectrum of a frame, H*W/2
+ *     complex64 = 4 MiB per frame in flight, does not fit a cluster's shared memory) is NOT the plan's cudaMalloc'ed
+ *     buffer but a file-scope `static __device__` array of CC_STATIC_SCRATCH_BYTES inside the library; every GPU that
+ *     loads the library holds that array until the process exits;
+ *   - the launch is a plain kernel launch (no graph object); the call performs no cudaMalloc / cudaFree and calls no
+ *     allocating library routine.  The first call on a device resolves the array's device address
+ *     (cudaGetSymbolAddress, once per device, with that device current): make that call outside a stream capture.
+ * Limits: the call launches min(batch, resident clusters) clusters like cc_track and is rejected with
+ * CC_ERR_UNSUPPORTED (cc_last_error names the largest batch) when their spectrum blocks exceed the array -- at
+ * 1024 x 1024 batch <= 2; shapes whose spectrum stays in shared memory (all others) need no scratch and take any
+ * batch.  Plans with the reference update of Eq. (9) switched on are rejected (CC_ERR_UNSUPPORTED): use cc_track.
+ * Sharing: ALL calls on a device, from every plan and stream, use the same array.  Nothing in it has to start at zero
+ * (the kernel writes each element of a spectrum block before it reads it), so calls need no clearing between them,
+ * but two calls that OVERLAP on the GPU (different streams, or a cc_track_static racing another process thread's)
+ * overwrite each other's spectra: serialise them (same stream, or an event).  cc_track is not affected.
+ * Arguments, ownership and error behaviour otherwise as cc_track.
+ */
+#define CC_STATIC_SCRATCH_BYTES (8u << 20)
+cc_status cc_track_static(const cc_plan *plan, const void *frames, int batch,
+                          float *dx, float *dy, float *peak, void *stream);
+
+/*
  * cc_track_debug -- cc_track that additionally returns the wrapped integer
  * peak of step a5 (PAPER.md:L90 sentence 1).
  *   iy, ix   DEVICE pointers, batch int32 each, or NULL

@@ -20,7 +20,7 @@ CC_U8, CC_U16 = 0, 1
 _STATUS = {0: "CC_OK", 1: "CC_ERR_INVALID_ARG", 2: "CC_ERR_UNSUPPORTED", 3: "CC_ERR_NOMEM",
            4: "CC_ERR_CUDA", 5: "CC_ERR_ARCH"}
 
-EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_debug", "cc_track_profile", "cc_track_host",
+EXPORTS = ["cc_plan_create", "cc_plan_create_weighted", "cc_track", "cc_track_static", "cc_track_debug", "cc_track_profile", "cc_track_host",
            "cc_plan_set_host_chunk", "cc_plan_destroy",
            "cc_plan_info", "cc_plan_enable_reference_update", "cc_plan_get_reference_spectrum", "cc_plan_get_reference_spectrum_f64", "cc_track_accumulate",
            "cc_plan_update_reference_from_accumulator", "cc_drift_correct", "cc_fp32_peak_probe", "cc_fp32_tile_probe", "cc_tc_gemm_probe", "cc_track_latency_probe",
@@ -61,6 +61,8 @@ def load_library() -> ctypes.CDLL:
         lib.cc_plan_create_weighted.restype = ci
         lib.cc_track.argtypes = [vp, vp, ci, vp, vp, vp, vp]
         lib.cc_track.restype = ci
+        lib.cc_track_static.argtypes = [vp, vp, ci, vp, vp, vp, vp]
+        lib.cc_track_static.restype = ci
         lib.cc_track_debug.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp, vp]
         lib.cc_track_debug.restype = ci
         lib.cc_track_profile.argtypes = [vp, vp, ci, vp, vp, vp, vp, vp]
@@ -228,6 +230,19 @@ class Plan:
                                       iy.data_ptr(), ix.data_ptr(), s))
             return dx, dy, pk, iy, ix
         _check(lib.cc_track(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(), pkp, s))
+        return dx, dy, pk
+
+    def track_static(self, frames_dev, out, batch: int | None = None, stream=None):
+        """cc_track_static: cc_track without any allocation -- the global spectrum scratch (1024 x 1024 shapes) is a
+        static array inside the library (include/cc.h for the limits); `out` = caller's (dx, dy, peak) device tensors."""
+        torch = _torch()
+        fb = self.H * self.W * self.np_dtype.itemsize
+        if batch is None:
+            batch = frames_dev.numel() * frames_dev.element_size() // fb
+        dx, dy, pk = out
+        s = (stream.cuda_stream if stream is not None else torch.cuda.current_stream(frames_dev.device).cuda_stream)
+        _check(load_library().cc_track_static(self._h, frames_dev.data_ptr(), batch, dx.data_ptr(), dy.data_ptr(),
+                                              pk.data_ptr() if pk is not None else None, s))
         return dx, dy, pk
 
     def track_profile(self, frames_dev, batch: int | None = None):

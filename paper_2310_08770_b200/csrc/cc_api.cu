@@ -721,6 +721,79 @@ extern "C" cc_status cc_track(const cc_plan *plan, const void *frames, int batch
     return track_impl(plan, frames, batch, dx, dy, peak, nullptr, nullptr, nullptr, stream);
 }
 
+// ------------------------------------------------------------------ cc_track_static: the same launch, no allocation anywhere
+// The spectrum scratch of the shapes whose spectrum block lives in global memory (the 1024 x 1024 variants, Cfg::SG)
+// comes from this file-scope array instead of the plan's cudaMalloc'ed one.  In HOST code the name is only a handle:
+// the device address is resolved once per device by cudaGetSymbolAddress (static_scratch_setup) and that pointer is
+// what the kernel receives.  Every GPU that loads the library holds the array until the process exits.
+static __device__ __align__(256) unsigned char cc_static_scratch[CC_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+void *g_static_ptr[kMaxDevices] = {};  // device address of cc_static_scratch, per device ordinal
+
+// Set-up, once per device, with that device current: resolve the device address of the array.
+cc_status static_scratch_setup(void **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices) return fail(CC_ERR_UNSUPPORTED, "cc_track_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, cc_static_scratch);
+        if (e != cudaSuccess || !ptr) return fail_cuda(e != cudaSuccess ? e : cudaErrorInvalidSymbol, "cudaGetSymbolAddress(cc_static_scratch)");
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return CC_OK;
+}
+}  // namespace
+
+extern "C" cc_status cc_track_static(const cc_plan *plan, const void *frames, int batch, float *dx, float *dy, float *peak,
+                                     void *stream)
+{
+    if (!plan || batch < 0) return fail(CC_ERR_INVALID_ARG, "cc_track_static: bad plan or batch");
+    if (batch == 0) return CC_OK;
+    if (!frames || !dx || !dy) return fail(CC_ERR_INVALID_ARG, "cc_track_static: null pointer");
+    if (((uintptr_t)frames & 15u) != 0) return fail(CC_ERR_INVALID_ARG, "cc_track_static: frames must be 16-byte aligned");
+    if (plan->ri_a0 > 0.0)
+        return fail(CC_ERR_UNSUPPORTED, "cc_track_static: the plan updates its reference image (Eq. (9)); that path uses "
+                                        "plan-owned scratch and, for CC-SN, separate kernels: use cc_track");
+    // the variant cc_track would take, launched plainly (no graph object, no plan-owned scratch)
+    const VarPlan *vp = &plan->thr;
+    if (plan->has_lat && batch <= plan->lat.max_clusters && batch * plan->lat.v.CS <= plan->thr.max_clusters * plan->thr.v.CS)
+        vp = &plan->lat;
+    const int ncl = std::min(batch, vp->max_clusters);
+    CcParams p{};
+    fill_params(plan, *vp, p);
+    p.frames = frames, p.batch = batch, p.dx = dx, p.dy = dy, p.peak = peak;
+    p.Sg = nullptr;
+    if (vp->v.s_global) {
+        // one spectrum block (H x W/2 complex64) per cluster in flight.  The kernel writes every element of its block
+        // (row-FFT scatter) before it reads any, so nothing has to be cleared between calls.
+        const size_t need = (size_t)ncl * plan->H * (size_t)(plan->W / 2) * sizeof(float2);
+        if (need > (size_t)CC_STATIC_SCRATCH_BYTES) {
+            char msg[256];
+            snprintf(msg, sizeof msg,
+                     "cc_track_static: batch %d needs %zu bytes of spectrum scratch (%d frames in flight), the static array holds "
+                     "%zu: at %d x %d the largest batch is %zu (use cc_track for more)",
+                     batch, need, ncl, (size_t)CC_STATIC_SCRATCH_BYTES, plan->H, plan->W,
+                     (size_t)CC_STATIC_SCRATCH_BYTES / ((size_t)plan->H * (size_t)(plan->W / 2) * sizeof(float2)));
+            return fail(CC_ERR_UNSUPPORTED, msg);
+        }
+        void *scratch = nullptr;
+        const cc_status st = static_scratch_setup(&scratch);
+        if (st != CC_OK) return st;
+        p.Sg = reinterpret_cast<float2 *>(scratch);
+    }
+    const cudaError_t e = vp->v.launch(p, ncl, vp->smem_bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e, "kernel launch");
+    return CC_OK;
+}
+
 extern "C" cc_status cc_plan_set_host_chunk(cc_plan *plan, int frames_per_chunk)
 {
     if (!plan || frames_per_chunk < 0) return fail(CC_ERR_INVALID_ARG, "cc_plan_set_host_chunk: bad plan or chunk");
