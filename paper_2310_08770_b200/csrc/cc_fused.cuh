@@ -431,6 +431,7 @@ template <int H_, int W_, int CS_, typename PIX_, int NT_, int TM1_, int TN1_, i
 struct Cfg {
     static constexpr bool TC1 = TC_ != 0;       // stage 1 of the upsampled DFT on the tensor cores (tcgen05, 3 x TF32)
     static constexpr int NSTG = NSTG_;  // staging ring depth
+    static constexpr int MINB = (H_ * W_ <= 64 * 64 && CS_ == 1) ? 2 : 1;  // CTAs per SM the register budget is set for
     static constexpr int NBARS = NSTG + 16;  // full[NSTG], raw ring [2], cluster exchange [2], rt command [1], row scatter [1], polish
                                              // tables [1], tensor-core stage 1: operand ring [4], MMA completion [2], staged [2]; T rows [1]
     static constexpr bool LAT = PFD_ > 4;       // small-batch (latency) variant: whole-frame operand prefetch, fp64 twiddles in smem
@@ -495,7 +496,7 @@ struct Cfg {
 };
 
 template <class C>
-__global__ void __launch_bounds__(C::NT, 1) cc_fused_kernel(const CcParams p)
+__global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams p)
 {
     constexpr int H = C::H, W = C::W, CS = C::CS, NT = C::NT, NC = C::NC, NR = C::NR;
     constexpr int NWARP = C::NWARP, NTW = C::NTW, PADW = C::PADW;

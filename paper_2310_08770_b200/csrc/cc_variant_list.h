@@ -12,8 +12,8 @@
 //   TC  : 1 = stage 1 of the upsampled DFT on the tensor cores (tcgen05.mma kind::tf32, three-pass hi/lo split, accumulators
 //         in tensor memory; needs 2 * W/2/CS == 128 spectrum floats per CTA), 0 = FP32 register-tiled loop
 // build.py compiles cc_variant.cu once per line.
-CCV(f64_u16,        64,   64, 1, uint16_t, 256,  5, 8, 10, 5, false, 11, 16, 16,  1,  3,  2,  1, 0)
-CCV(f64_u8,         64,   64, 1, uint8_t,  256,  5, 8, 10, 5, false, 11, 16, 16,  1,  3,  2,  1, 0)
+CCV(f64_u16,        64,   64, 1, uint16_t, 256,  5, 8,  5, 5, false, 11, 16, 32,  1,  3,  2,  1, 0)
+CCV(f64_u8,         64,   64, 1, uint8_t,  256,  5, 8,  5, 5, false, 11, 16, 32,  1,  3,  2,  1, 0)
 CCV(f128_u8,       128,  128, 1, uint8_t,  256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4,  1, 0)
 CCV(f128_u16,      128,  128, 1, uint16_t, 256,  2, 8,  4, 4, false, 16,  8,  8,  8,  6,  4,  1, 0)
 CCV(f128_u8_c8,    128,  128, 8, uint8_t,  256,  2, 4,  1, 4, false, 68, 32,  8,  8,  8,  6,  4, 0)
