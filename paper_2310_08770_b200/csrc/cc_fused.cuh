@@ -1876,6 +1876,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 mbar_wait(pbar, 0u);
                 pol_pending = false;
             }
+            static_assert(NSL * NC == NT, "one (column, slice) element per thread in the fp64 polish");
+            // the three row sums  sum_j D[m][j] Q[(y0+j)][q]  of rows ms-1, ms, ms+1: a move along n keeps all of them, a
+            // move along m keeps two -- only what entered the window is evaluated again (need: bit a = row a)
+            double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
+            int need = 7;
             for (int iter = 0; iter < 8; ++iter) {
                 // weights of the physical rows (y0+j) mod H, which hold Q(y0), Q(y0+H/2), the sums
                 // Q(y0+j)+Q(y0-j) (0 < j < H/2) and the differences Q(y0+j')-Q(y0-j') (j = H-j'):
@@ -1897,16 +1902,27 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                     }
                     __syncthreads();
                 }
-                for (int e = tid; e < NSL * NC; e += NT) {
-                    const int ql = e % NC, sl = e / NC;
-                    double2 s0 = make_double2(0.0, 0.0), s1 = s0, s2 = s0;
-                    for (int j = sl; j < H; j += NSL) {
-                        const float2 v = Sl[(size_t)((y0 + j) & (H - 1)) * NC + ql];
-                        const double vx = (double)v.x, vy = (double)v.y;
-                        const double d0 = dr0[j], d1 = dr1[j], d2 = dr2[j];
-                        s0.x = fma(d0, vx, s0.x), s0.y = fma(d0, vy, s0.y);
-                        s1.x = fma(d1, vx, s1.x), s1.y = fma(d1, vy, s1.y);
-                        s2.x = fma(d2, vx, s2.x), s2.y = fma(d2, vy, s2.y);
+                {   // (NSL * NC == NT: one (column, slice) element per thread, whose three row sums live across the iterations)
+                    const int ql = tid % NC, sl = tid / NC;
+                    if (need == 7) {
+                        for (int j = sl; j < H; j += NSL) {
+                            const float2 v = Sl[(size_t)((y0 + j) & (H - 1)) * NC + ql];
+                            const double vx = (double)v.x, vy = (double)v.y;
+                            const double d0 = dr0[j], d1 = dr1[j], d2 = dr2[j];
+                            s0.x = fma(d0, vx, s0.x), s0.y = fma(d0, vy, s0.y);
+                            s1.x = fma(d1, vx, s1.x), s1.y = fma(d1, vy, s1.y);
+                            s2.x = fma(d2, vx, s2.x), s2.y = fma(d2, vy, s2.y);
+                        }
+                    } else if (need != 0) {  // after a move along m: only the row that entered the window (same order of additions)
+                        const double *const dn = need == 1 ? dr0 : dr2;
+                        double2 sn = make_double2(0.0, 0.0);
+                        for (int j = sl; j < H; j += NSL) {
+                            const float2 v = Sl[(size_t)((y0 + j) & (H - 1)) * NC + ql];
+                            const double d = dn[j];
+                            sn.x = fma(d, (double)v.x, sn.x), sn.y = fma(d, (double)v.y, sn.y);
+                        }
+                        if (need == 1) s0 = sn;
+                        else s2 = sn;
                     }
                     part[(0 * NSL + sl) * NC + ql] = s0;
                     part[(1 * NSL + sl) * NC + ql] = s1;
@@ -1953,6 +1969,9 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 if (ba == 1 && bb == 1) break;
                 ms += ba - 1;
                 ns += bb - 1;
+                if (ba == 0) s2 = s1, s1 = s0, need = 1;
+                else if (ba == 2) s0 = s1, s1 = s2, need = 4;
+                else need = 0;
                 __syncthreads();
             }
         }
