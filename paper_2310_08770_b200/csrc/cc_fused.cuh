@@ -294,7 +294,16 @@ __device__ __forceinline__ void fft_bfly(Addr addr, int twstep, const float2 *tw
     fft_bfly<R, INV, TW>(addr, [&](int i) { return tw[(i * twstep) & (NTW - 1)]; });
 }
 
-__device__ __forceinline__ int padi(int i) { return i + (i >> 4); }  // 1 float2 of padding per 16
+// Index into a padded scratch row of a length-N row FFT: one float2 of padding per 16, and for the long rows one more
+// per 128 (N = 512) / per 256 (N = 1024).  With the first term alone the untangle / C2R accesses at the slots of
+// consecutive frequencies (stride N / r0 = 64) met only 4 distinct bank groups -- 4.5 wavefronts per access at
+// N = 1024 by ncu's source counters; a bank simulation of every access pattern of the row passes gives 720 -> 416
+// wavefronts per row pair at N = 1024 (ideal 384) and 352 -> 272 at N = 512 (with the lane order of pass 1 below).
+template <int N>
+__device__ __forceinline__ int padi(int i)
+{
+    return i + (i >> 4) + (N == 1024 ? (i >> 8) : N == 512 ? (i >> 7) : 0);
+}
 
 // Slot holding frequency k after the forward row FFT of length N (cc_common.h: k = k1 + r0 k2 + r0 r1 k3  <->
 // p = k1 N/r0 + k2 N/(r0 r1) + k3): powers of two throughout, so a few shifts instead of a table lookup.
@@ -345,11 +354,14 @@ __device__ __forceinline__ void warp_fft_pass(float2 *sc, const float2 *rt, int 
     CC_JITTER();
 #pragma unroll
     for (int n = 0; n < NB; ++n) {
-        const int g = gl + LP * n;
+        int g = gl + LP * n;
+        // N = 1024, pass 1 (blocks of 64, 8 lanes each): a half-warp takes blocks (0, 2) / (1, 3) instead of (0, 1) /
+        // (2, 3) -- their scratch offsets differ by half the bank window, so its 16 accesses meet 32 distinct banks
+        if constexpr (N == 1024 && L == 64 && LP == 32) g = (g & ~0x18) | ((g & 0x08) << 1) | ((g & 0x10) >> 1);
         if (g < N / R) {
             const int blk = g / ST, b = g % ST;
             const int base = blk * L + b;
-            fft_bfly<R, INV, (ST > 1)>([&](int i) { return sc + padi(base + i * ST); },
+            fft_bfly<R, INV, (ST > 1)>([&](int i) { return sc + padi<N>(base + i * ST); },
                                        [&](int i) { return rt[(SETS > 1 ? n : 0) * (R - 1) + i - 1]; });
         }
     }
@@ -382,7 +394,7 @@ __device__ __forceinline__ void warp_fft_fwd_from(float2 *sc, const RowTw<N, NTW
     for (int n = 0; n < T::NB0; ++n) {
         const int g = gl + LP * n;
         if (g < ST)
-            fft_bfly_io<R0, false, true>([&](int i) { return in(g + i * ST); }, [&](int k, float2 o) { sc[padi(g + k * ST)] = o; },
+            fft_bfly_io<R0, false, true>([&](int i) { return in(g + i * ST); }, [&](int k, float2 o) { sc[padi<N>(g + k * ST)] = o; },
                                          [&](int i) { return rt.t0[n * (R0 - 1) + i - 1]; });
     }
     __syncwarp();
@@ -401,7 +413,7 @@ __device__ __forceinline__ void warp_fft_inv_to(float2 *sc, const RowTw<N, NTW> 
     for (int n = 0; n < T::NB0; ++n) {
         const int g = gl + LP * n;
         if (g < ST)
-            fft_bfly_io<R0, true, true>([&](int i) { return sc[padi(g + i * ST)]; }, [&](int k, float2 o) { out(g + k * ST, o); },
+            fft_bfly_io<R0, true, true>([&](int i) { return sc[padi<N>(g + i * ST)]; }, [&](int k, float2 o) { out(g + k * ST, o); },
                                         [&](int i) { return rt.t0[n * (R0 - 1) + i - 1]; });
     }
     __syncwarp();
@@ -444,7 +456,7 @@ struct Cfg {
     static constexpr int NR = H / CS;       // frame rows per CTA
     static constexpr int NWARP = NT / 32;
     static constexpr int NTW = H > W ? H : W;
-    static constexpr int PADW = W + W / 16;
+    static constexpr int PADW = W + W / 16 + (W == 1024 ? W / 256 : W == 512 ? W / 128 : 0);  // padi<W>(W)
     static constexpr int rch0 = 16384 / (W * (int)sizeof(PIX));
     static constexpr int RG = cc_row_group(W);  // row pairs per warp in the row FFT phases
     static constexpr int LP = 32 / RG;
@@ -1077,8 +1089,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
 #pragma unroll
                         for (int i = 0; i < NK; ++i) {
                             const int k = gl + i * LP;
-                            z1[i] = scr[padi(row_slot_of<W>(k))];
-                            z2[i] = scr[padi(row_slot_of<W>(k == 0 ? W / 2 : W - k))];
+                            z1[i] = scr[padi<W>(row_slot_of<W>(k))];
+                            z2[i] = scr[padi<W>(row_slot_of<W>(k == 0 ? W / 2 : W - k))];
                         }
 #pragma unroll
                         for (int i = 0; i < NK; ++i) {
@@ -1137,11 +1149,18 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
             constexpr int RL = R2 > 1 ? R2 : R1;   // radix of the last forward pass (fused with the product)
             constexpr int NPASS = R2 > 1 ? 3 : 2;
             float2 *const Sb = SG ? reinterpret_cast<float2 *>(U) : Sl;  // [H][NCB]
+            // element (y, ql) of the block.  SG: a row is 64 bytes, so rows y and y + 8 (two lanes of the contiguous-slot
+            // passes) would meet the same banks: odd groups of 8 rows swap the two rows of each pair
+            auto sbx = [&](int y, int ql) -> int {
+                int a = y * NCB + ql;
+                if constexpr (SG) a ^= ((y >> 3) & 1) << 3;
+                return a;
+            };
             if constexpr (SG) {
 #pragma unroll 4
                 for (int idx = tid; idx < H * NCB / 2; idx += NT) {
                     const int y = idx / (NCB / 2), c2 = idx % (NCB / 2);
-                    *reinterpret_cast<float4 *>(Sb + (size_t)y * NCB + 2 * c2) =
+                    *reinterpret_cast<float4 *>(Sb + sbx(y, 2 * c2)) =
                         __ldcg(reinterpret_cast<const float4 *>(Sl + (size_t)y * NC + cb * NCB + 2 * c2));
                 }
                 __syncthreads();
@@ -1150,7 +1169,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
             for (int it = tid; it < NCB * (H / R0); it += NT) {
                 const int ql = it % NCB, g = it / NCB;
                 constexpr int ST = H / R0;
-                fft_bfly<R0, false, true, NTW>([&](int i) { return Sb + (size_t)(g + i * ST) * NCB + ql; }, g * (NTW / H), tw);
+                fft_bfly<R0, false, true, NTW>([&](int i) { return Sb + sbx(g + i * ST, ql); }, g * (NTW / H), tw);
             }
             __syncthreads();
             if constexpr (NPASS == 3) {  // forward pass 1 of 3
@@ -1158,7 +1177,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 for (int it = tid; it < NCB * (H / R1); it += NT) {
                     const int ql = it % NCB, g = it / NCB;
                     const int blk = g / ST, b = g % ST;
-                    fft_bfly<R1, false, true, NTW>([&](int i) { return Sb + (size_t)(blk * L + b + i * ST) * NCB + ql; },
+                    fft_bfly<R1, false, true, NTW>([&](int i) { return Sb + sbx(blk * L + b + i * ST, ql); },
                                                    b * (NTW / L), tw);
                 }
                 __syncthreads();
@@ -1179,12 +1198,12 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 }
                 float2 v[RL];
 #pragma unroll
-                for (int i = 0; i < RL; ++i) v[i] = Sb[(size_t)(g * RL + i) * NCB + ql];
+                for (int i = 0; i < RL; ++i) v[i] = Sb[sbx(g * RL + i, ql)];
                 dft_reg<RL, false>(v);
                 constexpr int bits = ilog2c(RL);
                 if (q == 0) {  // packed DC/Nyquist column: needs the -ky partner, handled below
 #pragma unroll
-                    for (int k = 0; k < RL; ++k) Sb[(size_t)(g * RL + k) * NCB + ql] = v[brev(k, bits)];
+                    for (int k = 0; k < RL; ++k) Sb[sbx(g * RL + k, ql)] = v[brev(k, bits)];
                 } else {
                     float2 w[RL];
 #pragma unroll
@@ -1195,7 +1214,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                     }
                     dft_reg<RL, true>(w);
 #pragma unroll
-                    for (int n = 0; n < RL; ++n) Sb[(size_t)(g * RL + n) * NCB + ql] = w[brev(n, bits)];
+                    for (int n = 0; n < RL; ++n) Sb[sbx(g * RL + n, ql)] = w[brev(n, bits)];
                 }
             }
             __syncthreads();
@@ -1209,7 +1228,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 for (int e = 0; e < PER; ++e) {
                     const int s = tid + e * NT;
                     if (s < H) {
-                        const float2 z = Sb[(size_t)s * NCB], zp = Sb[(size_t)p.col_partner[s] * NCB];
+                        const float2 z = Sb[sbx(s, 0)], zp = Sb[sbx((int)p.col_partner[s], 0)];
                         const float4 g = __ldcg(&p.ab[s]);  // (G0c.re, G0c.im, Gnc.re, Gnc.im)
                         const float2 fa = make_float2(0.5f * (z.x + zp.x), 0.5f * (z.y - zp.y));
                         const float2 fb = make_float2(0.5f * (z.y + zp.y), -0.5f * (z.x - zp.x));
@@ -1223,11 +1242,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
 #pragma unroll
                 for (int e = 0; e < PER; ++e) {
                     const int s = tid + e * NT;
-                    if (s < H) Sb[(size_t)s * NCB] = o[e];
+                    if (s < H) Sb[sbx(s, 0)] = o[e];
                 }
                 __syncthreads();
                 for (int g = tid; g < H / RL; g += NT)
-                    fft_bfly<RL, true, false, NTW>([&](int i) { return Sb + (size_t)(g * RL + i) * NCB; }, 0, tw);
+                    fft_bfly<RL, true, false, NTW>([&](int i) { return Sb + sbx(g * RL + i, 0); }, 0, tw);
                 __syncthreads();
             }
             if constexpr (NPASS == 3) {  // inverse of forward pass 1
@@ -1235,7 +1254,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 for (int it = tid; it < NCB * (H / R1); it += NT) {
                     const int ql = it % NCB, g = it / NCB;
                     const int blk = g / ST, b = g % ST;
-                    fft_bfly<R1, true, true, NTW>([&](int i) { return Sb + (size_t)(blk * L + b + i * ST) * NCB + ql; },
+                    fft_bfly<R1, true, true, NTW>([&](int i) { return Sb + sbx(blk * L + b + i * ST, ql); },
                                                   b * (NTW / L), tw);
                 }
                 __syncthreads();
@@ -1243,7 +1262,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
             for (int it = tid; it < NCB * (H / R0); it += NT) {
                 const int ql = it % NCB, g = it / NCB;
                 constexpr int ST = H / R0;
-                fft_bfly<R0, true, true, NTW>([&](int i) { return Sb + (size_t)(g + i * ST) * NCB + ql; }, g * (NTW / H), tw);
+                fft_bfly<R0, true, true, NTW>([&](int i) { return Sb + sbx(g + i * ST, ql); }, g * (NTW / H), tw);
             }
             if constexpr (SG) {  // the finished block goes back to L2
                 __syncthreads();
@@ -1251,7 +1270,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                 for (int idx = tid; idx < H * NCB / 2; idx += NT) {
                     const int y = idx / (NCB / 2), c2 = idx % (NCB / 2);
                     __stcg(reinterpret_cast<float4 *>(Sl + (size_t)y * NC + cb * NCB + 2 * c2),
-                           *reinterpret_cast<const float4 *>(Sb + (size_t)y * NCB + 2 * c2));
+                           *reinterpret_cast<const float4 *>(Sb + sbx(y, 2 * c2)));
                 }
                 __syncthreads();
             }
@@ -1285,11 +1304,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) cc_fused_kernel(const CcParams
                     for (int i = 0; i < NK; ++i) {
                         const int k = gl + i * LP;
                         if (k == 0) {
-                            scr[padi(row_slot_of<W>(0))] = make_float2(qa[i].x, qb[i].x);
-                            scr[padi(row_slot_of<W>(W / 2))] = make_float2(qa[i].y, qb[i].y);
+                            scr[padi<W>(row_slot_of<W>(0))] = make_float2(qa[i].x, qb[i].x);
+                            scr[padi<W>(row_slot_of<W>(W / 2))] = make_float2(qa[i].y, qb[i].y);
                         } else {
-                            scr[padi(row_slot_of<W>(k))] = make_float2(qa[i].x - qb[i].y, qa[i].y + qb[i].x);
-                            scr[padi(row_slot_of<W>(W - k))] = make_float2(qa[i].x + qb[i].y, qb[i].x - qa[i].y);
+                            scr[padi<W>(row_slot_of<W>(k))] = make_float2(qa[i].x - qb[i].y, qa[i].y + qb[i].x);
+                            scr[padi<W>(row_slot_of<W>(W - k))] = make_float2(qa[i].x + qb[i].y, qb[i].x - qa[i].y);
                         }
                     }
                 }
