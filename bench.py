@@ -33,8 +33,8 @@ from paper_2310_08770_b200 import workloads as wl  # noqa: E402
 NOMINAL_SM_MHZ = 1965.0
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one 10,000-frame launch, from the committed capture
-TRAFFIC_BYTES_PER_10K_LAUNCH = 1.3172e9
-TRAFFIC_SOURCE = ("ncu --set full capture of one 10,000-frame launch, raw rows in profiles/r2c_cfg3_raw_metrics.csv "
+TRAFFIC_BYTES_PER_10K_LAUNCH = 1.3175e9
+TRAFFIC_SOURCE = ("ncu --set full capture of one 10,000-frame launch, raw rows in profiles/r2d_cfg3_raw_metrics.csv "
                   "(dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes 1.3108e9")
 
 
