@@ -384,6 +384,27 @@ def test_non_square_formats(gpu, oracle_mod, H, W, method, eps):
     assert np.median(np.hypot(dx - sh[:, 1], dy - sh[:, 0])) < 0.1
 
 
+@pytest.mark.parametrize("H,W", [(128, 256), (512, 256), (128, 1024)])
+def test_non_square_formats_u8(gpu, oracle_mod, H, W):
+    """The same formats for 8-bit pixels (uint8 kernel variants), batched and single frame."""
+    import torch
+    rng = np.random.default_rng(H * 3 + W)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float64)
+    spot = lambda sy, sx: 180.0 * np.exp(-((y - H / 2 - sy) ** 2 + (x - W / 2 - sx) ** 2) / (2 * 3.5 ** 2)) + 6.0
+    ref = spot(0.0, 0.0).astype(np.float32)
+    sh = rng.uniform(-10, 10, size=(20, 2))
+    fr = np.stack([rng.poisson(spot(a, b)) for a, b in sh]).clip(0, 255).astype(np.uint8)
+    o = oracle_mod.track(fr, ref, 32)
+    plan = gpu.Plan(H, W, fr.dtype, 32, ref)
+    d = plan.device_frames(fr)
+    dx, dy, pk, iy, ix = [t.cpu().numpy() for t in plan.track(d, debug=True)]
+    _compare(o, dx, dy, pk, iy, ix, "%dx%d u8" % (H, W))
+    one = [plan.track(d[i], 1) for i in range(4)]      # the single-frame (cluster) variant
+    torch.cuda.synchronize()
+    assert np.array_equal(np.array([t[0].item() for t in one]), dx[:4]) and np.array_equal(np.array([t[1].item() for t in one]), dy[:4])
+    plan.close()
+
+
 @pytest.mark.parametrize("H,W,u", [(256, 256, 128), (256, 256, 1024), (128, 256, 512)])
 def test_table1_upsampling_factors(gpu, oracle_mod, H, W, u):
     """The paper's benchmark settings (Table I: CC-SN, u = 128 ... 1024): grids of up to
